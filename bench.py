@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py -- X-engine throughput on B200 (BASELINE.json metric: Tops/s at 8 ops per complex MAC).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl reference]
+
+A "step" is one pass of the whole hot path (S0-S3 of SURVEY 8(a): staging if needed, tile schedule,
+tcgen05 X-engine, packing epilogue) over one synthetic input block through the C-ABI library.
+Default workload = BASELINE.json configs[1] (N=128, F=1024, T=1000).  Prints ONE JSON line.
+
+  value        whole-job Tops/s, inputs resident in HBM (ops = 8 * F * T * N(2N+1), Eq. 5)
+  e2e          same metric through xc_correlate_host with HOST buffers (H2D + X-engine + D2H per step)
+  roofline     dominant kernel against the measured HBM / int8-tensor peak (MEASURED_PEAKS.json)
+  cpu_baseline the oracle (oracle/xo_oracle.c, as it stands) on the box's host cores, bounded sample
+  by_config    kernel-only Tops/s for the other BASELINE configs (the metric is "vs N stations")
+
+N > 1 (torchrun): every rank runs its own block of F channels (channels are independent, PAPER.md:65,
+285): no data-path collective, "scaling": "weak"; time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+NOMINAL_I8_OVER_BF16 = 2.0          # 4.5 / 2.25 PFLOP/s dense (B200_PROFILING.md nominal table)
+FALLBACK_HBM_GBS, FALLBACK_BF16_TF = 6650.0, 1590.0
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            m = json.load(fh)
+        return {"hbm_gbs": float(m["hbm_gbs"]), "bf16_burst": float(m["bf16_tflops"]),
+                "bf16_sustained": float(m.get("bf16_tflops_sustained", m["bf16_tflops"])), "source": "measured"}
+    return {"hbm_gbs": FALLBACK_HBM_GBS, "bf16_burst": FALLBACK_BF16_TF, "bf16_sustained": 1400.0,
+            "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def window(self, t0, t1):
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ts, line in self.rows:
+            if ts < t0 - 0.05 or ts > t1 + 0.15:
+                continue
+            tok = [t.strip() for t in line.split(",")]
+            try:
+                sm.append(float(tok[0]))
+                mx = max(mx, float(tok[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, tok[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx or None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+
+
+def workload_desc(w):
+    return (f"{w.name}: N={w.N} stations x 2 pol, F={w.F} channels, T={w.T} samples, int8 {w.kind} "
+            f"sigma={w.sigma}, seed {w.seed}, layout [t][f][station][pol][re,im]")
+
+
+def cpu_sample(w, x, target_s=12.0):
+    """Oracle on a bounded sample of channels of the same workload; returns (Tops/s, cores, text)."""
+    from oracle import xo
+    cores = xo.num_threads()
+    per_ch = w.T * w.N * (2 * w.N + 1)
+    t0 = time.perf_counter()
+    xo.channels_i8(x, list(range(min(cores, w.F))))
+    dt = time.perf_counter() - t0
+    n0 = min(cores, w.F)
+    rate = n0 * per_ch / dt
+    nsel = int(max(n0, min(w.F, (target_s * rate / per_ch) // cores * cores)))
+    t0 = time.perf_counter()
+    xo.channels_i8(x, list(range(nsel)))
+    dt = time.perf_counter() - t0
+    tops = 8.0 * nsel * per_ch / dt / 1e12
+    return tops, cores, f"{nsel} of {w.F} channels of {w.name}, all baselines, {dt:.1f} s"
+
+
+def run_reference(args, rank):
+    """--impl reference: the CPU oracle as it stands, on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    import xc_workloads as wl
+    from oracle import xo
+    w = wl.CONFIGS[args.workload]
+    cores = xo.num_threads()
+    per_ch = w.T * w.N * (2 * w.N + 1)
+    # a step = `nch` channels of the workload (bounded sample; channels are independent)
+    nch = max(1, min(w.F, cores))
+    sub = wl.Workload(w.name, w.N, nch, w.T, w.kind, w.sigma, w.seed)
+    x = wl.make_input(sub)
+    sel = list(range(nch))
+    for _ in range(args.warmup):
+        xo.channels_i8(x, sel)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        xo.channels_i8(x, sel)
+    dt = time.perf_counter() - t0
+    tops = 8.0 * args.steps * nch * per_ch / dt / 1e12
+    sample = f"{nch} of {w.F} channels of {w.name} per step, all baselines"
+    print(json.dumps({
+        "impl": "reference", "metric": "X-engine Tops/s (8 ops per cMAC)", "value": tops, "unit": "Tops/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8", "data": "synthetic",
+        "config": {"workload": workload_desc(w), "sample": sample},
+        "cpu_baseline": {"value": tops, "unit": "Tops/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": tops, "unit": "Tops/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def time_kernel(p, xd, vis, stream, steps, warmup):
+    """Per-launch durations (ms) with CUDA events on the launching stream."""
+    import torch
+    with torch.cuda.stream(stream):
+        for _ in range(warmup):
+            p.correlate(xd, vis, stream=stream)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        stream.synchronize()
+        for a, b in evs:
+            a.record(stream)
+            p.correlate(xd, vis, stream=stream)
+            b.record(stream)
+        stream.synchronize()
+    return [a.elapsed_time(b) for a, b in evs]
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--impl", default="native", choices=["native", "reference"])
+    ap.add_argument("--no-sweep", action="store_true", help="skip the by_config sweep")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "native" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    import paper_1107_4264_b200 as xcb
+    import xc_workloads as wl
+    from paper_1107_4264_b200 import build as xc_build
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the X-engine has no CPU path")
+    if rank == 0:
+        xc_build.build()
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist.barrier()
+    xcb.load_library()
+
+    peaks = load_peaks()
+    w = wl.CONFIGS[args.workload]
+    # weak scaling: every rank holds its own block of F channels (seed differs per rank)
+    x_np = wl.make_input(w, seed=w.seed + 7919 * rank)
+    p = xcb.Plan(w.N, w.F, w.T)
+    stream = torch.cuda.Stream()
+    xh = torch.from_numpy(x_np).pin_memory()
+    xd = xh.cuda()
+    vis = p.new_vis()
+    torch.cuda.synchronize()
+
+    # ---- device-resident timing: exactly K steps between barrier + synchronize ----------------
+    sampler = ClockSampler(torch.cuda.current_device())
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            p.correlate(xd, vis, stream=stream)
+    launches_per_step = p.last_launches
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    t_wall0 = time.perf_counter()
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for _ in range(args.steps):
+            p.correlate(xd, vis, stream=stream)
+        e1.record(stream)
+    torch.cuda.synchronize()
+    t_wall1 = time.perf_counter()
+    ms_total = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+        dist.barrier()
+    clocks = sampler.window(t_wall0, t_wall1)
+    ms_step = ms_total / args.steps
+    tops = world * w.ops / (ms_step * 1e-3) / 1e12
+
+    # ---- per-launch duration of the dominant kernel (events around each launch) -------------
+    per = time_kernel(p, xd, vis, stream, args.steps, 1)
+    k_ms = sum(per) / len(per)
+    alg_bytes = w.in_bytes + w.vis_bytes                      # input once + output once
+    i8_peak = peaks["bf16_burst"] * NOMINAL_I8_OVER_BF16      # Tops/s: measured bf16 x nominal int8/bf16 ratio
+    t_hbm = alg_bytes / (peaks["hbm_gbs"] * 1e9)
+    t_tc = w.ops / (i8_peak * 1e12)
+    traffic = TRAFFIC_NCU.get(w.name)
+    if t_hbm >= t_tc:
+        ach = alg_bytes / (k_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": ach / peaks["hbm_gbs"], "traffic": traffic}
+    else:
+        ach = w.ops / (k_ms * 1e-3) / 1e12
+        roof = {"bound": "tensor", "achieved": ach, "peak": i8_peak, "unit": "Tops/s", "frac": ach / i8_peak,
+                "traffic": traffic}
+    roof.update({"kernel": "xc_i8_tc_kernel", "kernel_ms": k_ms, "peak_source": peaks["source"] +
+                 (" hbm_gbs" if roof["bound"] == "hbm" else " bf16_tflops (burst) x 2 (nominal int8/bf16)"),
+                 "algorithmic_bytes": alg_bytes, "algorithmic_ops": w.ops,
+                 "other_roof_frac": (w.ops / (k_ms * 1e-3) / 1e12 / i8_peak) if roof["bound"] == "hbm"
+                 else (alg_bytes / (k_ms * 1e-3) / 1e9 / peaks["hbm_gbs"])})
+
+    # ---- end to end through the C ABI with HOST buffers ---------------------------------------
+    vh = torch.empty(p.vis_shape(), dtype=torch.int32).pin_memory()
+    e2e_steps = max(3, min(args.steps, 10))
+    p.correlate_host(xh, vh, xd, vis, stream=stream)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        p.correlate_host(xh, vh, xd, vis, stream=stream)       # synchronises the stream itself
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e = {"value": world * w.ops / e2e_s / 1e12, "unit": "Tops/s", "h2d_bytes_per_step": world * w.in_bytes,
+           "d2h_bytes_per_step": world * w.vis_bytes, "ms_per_step": 1e3 * e2e_s, "steps": e2e_steps,
+           "api": "xc_correlate_host (pinned host in/out)"}
+
+    # ---- the metric "vs N stations": kernel-only numbers for the other configs (rank 0, N=1) -----
+    by_config = {}
+    if rank == 0 and world == 1 and not args.no_sweep:
+        del xd, vis, xh, vh
+        torch.cuda.empty_cache()
+        for name in ["cfg3", "cfg4", "cfg5_N32", "cfg5_N64", "cfg5_N100", "cfg5_N500", "cfg5_N1024"]:
+            if name == args.workload:
+                continue
+            ww = wl.CONFIGS[name]
+            xx = torch.from_numpy(wl.make_input(ww)).cuda()
+            pp = xcb.Plan(ww.N, ww.F, ww.T)
+            vv = pp.new_vis()
+            d = time_kernel(pp, xx, vv, stream, 10, 3)
+            ms = sorted(d)[len(d) // 2]
+            by_config[name] = {"N": ww.N, "F": ww.F, "T": ww.T, "kernel_ms": ms,
+                               "tops": ww.ops / (ms * 1e-3) / 1e12,
+                               "frac_i8_peak": ww.ops / (ms * 1e-3) / 1e12 / i8_peak,
+                               "hbm_gbs": (ww.in_bytes + ww.vis_bytes) / (ms * 1e-3) / 1e9,
+                               "l2": "cold (input > L2)" if ww.in_bytes > 126e6 else "warm (input fits L2)"}
+            pp.close()
+            del xx, vv
+            torch.cuda.empty_cache()
+
+    # ---- CPU baseline: the oracle on a bounded sample (rank 0 at N=1 only) --------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        v, cores, sample = cpu_sample(w, x_np)
+        cpu = {"value": v, "unit": "Tops/s", "cores": cores, "kind": "oracle", "sample": sample}
+    sampler.stop()
+
+    if rank == 0:
+        out = {
+            "metric": "X-engine Tops/s (8 ops per cMAC)", "value": tops, "unit": "Tops/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int8", "data": "synthetic",
+            "config": {"workload": workload_desc(w), "global_channels": world * w.F,
+                       "parallelism": f"channel-sharded x{world}, no collective",
+                       "l2": "input block (%.0f MB) + output (%.0f MB) exceed the 126 MB L2: every step is cold"
+                             % (w.in_bytes / 1e6, w.vis_bytes / 1e6)},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * launches_per_step,
+            "roofline": roof, "cpu_baseline": cpu, "by_config": by_config,
+            "frac_of_int8_peak": tops / world / i8_peak, "int8_peak_tops": i8_peak,
+            "paper_context": "1058 GFLOPS = 79% of fp32 peak on a GeForce GTX 480 (PAPER.md:267); other hardware",
+        }
+        print(json.dumps(out))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of xc_i8_tc_kernel from `ncu --set full`
+# captures (see profiles/*.md for the command and the raw numbers); null until captured.
+TRAFFIC_NCU: dict = {}
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,171 @@
+/*
+ * xc.h -- C ABI of the B200-native X-engine (radio-astronomy cross-correlator).
+ *
+ * Operation (Sec. 2.1, Eq. 4): for every frequency channel f, the
+ * time-integrated self outer product of the complex sample vector of N stations x 2
+ * polarisations,
+ *
+ *      V_f[(i,pi),(j,pj)] = sum_{t<T}  x_{t,f,i,pi} * conj(x_{t,f,j,pj})
+ *
+ * kept for the lower-triangle station pairs 0 <= i <= j < N ("1/2 N(N+1) correlation
+ * pairs including the auto-correlation of self pairs"), all four
+ * polarisation products per pair.
+ *
+ * Layouts (BASELINE.json north_star; input order = PAPER.md:149 "station fastest, then
+ * frequency, then time", i.e. the corner turn is already applied):
+ *
+ *   in  : [t][f][station][pol][re,im]      flat ((((t*F + f)*N + s)*2 + p)*2 + c)
+ *         int8 for the integer path, float for the fp32 path
+ *   vis : [f][b][pol_i][pol_j][re,im]      flat ((((f*NB + b)*2 + pi)*2 + pj)*2 + c)
+ *         b = j(j+1)/2 + i  (the paper's triangular block order, applied at
+ *         station level),  NB = N(N+1)/2;  int32 for the integer path, float for fp32
+ *
+ * Every *_dev pointer is DEVICE memory owned by the caller (allocate it with PyTorch);
+ * every *_host pointer is HOST memory owned by the caller.  The library never frees or
+ * retains caller memory beyond the call (except the workspace handed to
+ * xc_set_workspace, which it uses until the plan is destroyed or the workspace replaced).
+ * Streams are cudaStream_t passed as void*; all device work is enqueued on the stream
+ * given, asynchronously, with no hidden device synchronisation unless stated.
+ *
+ * Every function returns an xc_status (0 = OK, negative = error); nothing is thrown
+ * across this boundary; on error no output is promised.  There is no CPU fallback: on a
+ * machine without an sm_100 GPU every compute entry point returns XC_ERR_CUDA /
+ * XC_ERR_UNSUPPORTED.
+ */
+#ifndef XC_H_
+#define XC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct xc_plan_s xc_plan_t; /* opaque; created by xc_plan, freed by xc_destroy */
+
+typedef enum {
+    XC_OK = 0,
+    XC_ERR_INVALID_ARG = -1,  /* null pointer, N/F/T < 1, bad option ...                      */
+    XC_ERR_UNSUPPORTED = -2,  /* P != 2, unknown layout, device is not sm_100                  */
+    XC_ERR_OVERFLOW = -3,     /* T > XC_MAX_T: one call could leave int32 (2*128^2*T >= 2^31)  */
+    XC_ERR_ALIGNMENT = -4,    /* pointer alignment not met and no staging workspace available  */
+    XC_ERR_CUDA = -5,         /* a CUDA call failed; see xc_last_cuda_error                    */
+    XC_ERR_NO_WORKSPACE = -6  /* staging needed but workspace too small                        */
+} xc_status;
+
+typedef enum {
+    XC_LAYOUT_TFSPC = 0 /* [t][f][station][pol][re,im] -- PAPER.md:149; the only layout */
+} xc_layout;
+
+/* Largest T of one integer call: |V| <= 2 * 128^2 * T must stay < 2^31 ("a larger number of
+ * bits used for the accumulator to prevent overflow"). Across xc_correlate_acc
+ * calls the caller owns the bound. */
+#define XC_MAX_T 65535
+
+/* Kernel choice for the integer path (xc_set_option(XC_OPT_I8_KERNEL, ...)). */
+enum {
+    XC_I8_KERNEL_AUTO = 0, /* tcgen05 tensor-core kernel (the product path)                   */
+    XC_I8_KERNEL_TC = 1,   /* same, forced                                                    */
+    XC_I8_KERNEL_SIMT = 2  /* plain CUDA-core kernel, one thread per baseline: a debugging    */
+                           /* aid that shares no device code with the tensor-core kernel     */
+};
+typedef enum {
+    XC_OPT_I8_KERNEL = 0, /* one of XC_I8_KERNEL_*                                            */
+    XC_OPT_MAX_CTAS = 1,  /* cap on persistent CTAs of the tensor-core kernel (0 = SM count)  */
+    XC_OPT_FORCE_STAGE = 2 /* 1 = always run the staging (pad/copy) kernel, for testing S0     */
+} xc_option;
+
+/* xc_plan -- north_star's xc_plan(N, P=2, F, T, layout).
+ *   N stations (>=1), P polarisations (must be 2), F channels (>=1), T samples per call
+ *   (1..XC_MAX_T), layout = XC_LAYOUT_TFSPC.  Builds the triangular tile schedule
+ *   (only tiles that intersect i <= j are scheduled) and uploads it to the
+ *   current CUDA device (plan-owned, a few KB).  *out receives the plan.
+ *   Errors: INVALID_ARG, UNSUPPORTED, OVERFLOW, CUDA. */
+int xc_plan(xc_plan_t** out, int N, int P, int F, int T, int layout);
+
+/* Frees the plan and the device memory it owns (tile table, and a staging workspace only if
+ * the library allocated it itself).  NULL is allowed. */
+void xc_destroy(xc_plan_t* plan);
+
+/* Sizes in bytes of one input block / one output cube for this plan. */
+size_t xc_in_bytes(const xc_plan_t* plan);      /* int8 path:  4*N*F*T            */
+size_t xc_in_bytes_f32(const xc_plan_t* plan);  /* fp32 path: 16*N*F*T            */
+size_t xc_vis_bytes(const xc_plan_t* plan);     /* 32*NB*F (int32 and float alike) */
+/* N(N+1)/2. */
+size_t xc_n_baselines(const xc_plan_t* plan);
+
+/* Staging.  The tensor-core kernel reads the input through TMA, which
+ * needs a 16-byte-aligned base and 16-byte-multiple row pitch (4N bytes -> N % 4 == 0).
+ * Otherwise the input is first copied by a padding kernel into a workspace of
+ * xc_workspace_bytes() bytes (0 when never needed).  The caller may hand one in (device
+ * memory, 128-byte aligned, kept until xc_destroy or replaced); if none was set the
+ * library cudaMallocs one on first need (a synchronising call) and frees it in xc_destroy. */
+size_t xc_workspace_bytes(const xc_plan_t* plan);
+int xc_set_workspace(xc_plan_t* plan, void* ws_dev, size_t bytes);
+
+int xc_set_option(xc_plan_t* plan, int option, int value);
+
+/* xc_correlate -- vis = X-engine(in)  (Eq. 4).  Overwrites all F*NB*8 int32 of vis_dev; old
+ *   contents are not read.  in_dev: int8 [T][F][N][2][2]; vis_dev: int32 [F][NB][2][2][2],
+ *   4-byte aligned at least (32-byte alignment gives full-sector stores).  Exact for the whole
+ *   int8 range including -128.  Bit-exact to the definition; independent of tile schedule.
+ * xc_correlate_acc -- vis += X-engine(in)  ("matrix_d <- X-engine(matrix_d, buffer_d)",
+ *   PAPER.md:244; I = N_p * I').  int32 two's-complement addition. */
+int xc_correlate(xc_plan_t* plan, const int8_t* in_dev, int32_t* vis_dev, void* cuda_stream);
+int xc_correlate_acc(xc_plan_t* plan, const int8_t* in_dev, int32_t* vis_dev, void* cuda_stream);
+
+/* xc_correlate_f32 -- same operation on float samples with fp32 FMA arithmetic on the CUDA
+ *   cores (the paper's own arithmetic: PAPER.md:75, 16 FMAs per station pair per sample;
+ *   warp-level register tiling as in PAPER.md:130-147).  in_dev: float [T][F][N][2][2] (16-byte
+ *   aligned); vis_dev: float [F][NB][2][2][2].  accumulate != 0 adds to vis_dev.  Summation
+ *   order over t is fixed (ascending, one accumulator per output) so results are
+ *   deterministic; they agree with an fp64 evaluation to about T * 2^-24 relative to
+ *   sqrt(V_ii V_jj). */
+int xc_correlate_f32(xc_plan_t* plan, const float* in_dev, float* vis_dev, int accumulate, void* cuda_stream);
+
+/* xc_correlate_pipelined -- Algorithm 1 read as textbook double
+ *   buffering: n_blocks input blocks of xc_in_bytes() each lie back to back in PINNED host
+ *   memory at in_host; block p+1 is copied host->device on copy_stream into one half of
+ *   dev_buf2 (2 * xc_in_bytes() bytes of device memory, 128-byte aligned) while block p is
+ *   correlated on compute_stream from the other half; events order the two streams (no host
+ *   synchronisation inside).  vis_dev = sum over blocks (first block overwrites).  The result
+ *   stays on the device.  Returns after enqueueing; the caller synchronises
+ *   compute_stream.  compute_stream and copy_stream must differ for any overlap to happen. */
+int xc_correlate_pipelined(xc_plan_t* plan, const int8_t* in_host_pinned, int n_blocks, int8_t* dev_buf2,
+                           int32_t* vis_dev, void* compute_stream, void* copy_stream);
+
+/* xc_correlate_host -- convenience end-to-end call with HOST buffers: copies in_host
+ *   (xc_in_bytes(), pinned for full speed) to in_dev_scratch, runs xc_correlate, copies the
+ *   result back into vis_host (xc_vis_bytes()) and synchronises the stream before returning.
+ *   in_dev_scratch / vis_dev_scratch are caller-owned device buffers of the plan's sizes. */
+int xc_correlate_host(xc_plan_t* plan, const int8_t* in_host, int32_t* vis_host, int8_t* in_dev_scratch,
+                      int32_t* vis_dev_scratch, void* cuda_stream);
+
+/* Tile schedule introspection (for tests of the triangular map).
+ *   xc_tile_count: number of scheduled tiles per channel for the integer path.
+ *   xc_tile_get:   tile k -> (block row bi on the i side, block column bj on the j side) and
+ *                  the tile's extent in stations (si stations on the i side, sj on the j side). */
+int xc_tile_count(const xc_plan_t* plan);
+int xc_tile_get(const xc_plan_t* plan, int k, int* bi, int* bj, int* si, int* sj);
+
+/* The paper's closed-form triangular map and its inverse:
+ *   g = by(by+1)/2 + bx,  by = floor(-1/2 + sqrt(1/4 + 2g)),  bx = g - by(by+1)/2,
+ *   with an integer fix-up so it is exact for every g (SURVEY 8(c) reading 12). */
+int64_t xc_tri_index(int64_t bx, int64_t by);
+void xc_tri_inverse(int64_t g, int64_t* bx, int64_t* by);
+
+/* Number of launches of this library's own kernels enqueued by the last compute call on this
+ * plan (staging + X-engine), for bench accounting. */
+int xc_last_launches(const xc_plan_t* plan);
+
+const char* xc_status_string(int status);
+/* Text of the last CUDA error seen by this plan ("" if none). */
+const char* xc_last_cuda_error(const xc_plan_t* plan);
+/* Library version string. */
+const char* xc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* XC_H_ */

@@ -1,0 +1,10 @@
+"""paper_1107_4264_b200 -- a B200-native X-engine (FX-correlator cross-multiply stage).
+
+Thin Python binding over the C-ABI library `libxc.so` (see include/xc.h): argument marshalling
+only; every step of the path runs in the library's own CUDA kernels.  PyTorch is used for
+device memory and streams.  There is no CPU fallback: if the library cannot be loaded, or no
+sm_100 GPU is present, calls raise.
+"""
+from .binding import (XcError, Plan, lib, load_library, tri_index, tri_inverse, version,  # noqa: F401
+                      I8_KERNEL_AUTO, I8_KERNEL_TC, I8_KERNEL_SIMT, OPT_I8_KERNEL, OPT_MAX_CTAS,
+                      OPT_FORCE_STAGE, MAX_T, EXPORTED_SYMBOLS, shard_channels)

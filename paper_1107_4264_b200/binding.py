@@ -1,0 +1,253 @@
+"""ctypes binding for libxc.so -- same names as include/xc.h, argument marshalling only.
+
+Tensors are torch CUDA tensors (device memory) or pinned CPU tensors (host memory); only their
+data pointers and the stream handle cross the boundary.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libxc.so")
+
+MAX_T = 65535
+I8_KERNEL_AUTO, I8_KERNEL_TC, I8_KERNEL_SIMT = 0, 1, 2
+OPT_I8_KERNEL, OPT_MAX_CTAS, OPT_FORCE_STAGE = 0, 1, 2
+
+# every symbol include/xc.h declares
+EXPORTED_SYMBOLS = (
+    "xc_plan", "xc_destroy", "xc_in_bytes", "xc_in_bytes_f32", "xc_vis_bytes", "xc_n_baselines",
+    "xc_workspace_bytes", "xc_set_workspace", "xc_set_option", "xc_correlate", "xc_correlate_acc",
+    "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_tile_count", "xc_tile_get",
+    "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error",
+    "xc_version",
+)
+
+
+class XcError(RuntimeError):
+    def __init__(self, code: int, where: str, detail: str = ""):
+        name = lib().xc_status_string(code).decode() if _lib is not None else str(code)
+        super().__init__(f"{where}: {name} ({code}){': ' + detail if detail else ''}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library(path: str | None = None) -> ctypes.CDLL:
+    """Loads libxc.so; raises (never falls back) if it is missing -- build it with
+    `python -m paper_1107_4264_b200.build`."""
+    global _lib
+    path = path or LIB_PATH
+    if not os.path.exists(path):
+        raise FileNotFoundError(f"{path} not built: run `python -m paper_1107_4264_b200.build` "
+                                "(there is no CPU fallback)")
+    L = ctypes.CDLL(path)
+    i, p, sz, i64 = ctypes.c_int, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int64
+    pp = ctypes.POINTER(ctypes.c_void_p)
+    sig = {
+        "xc_plan": (i, [pp, i, i, i, i, i]),
+        "xc_destroy": (None, [p]),
+        "xc_in_bytes": (sz, [p]), "xc_in_bytes_f32": (sz, [p]), "xc_vis_bytes": (sz, [p]),
+        "xc_n_baselines": (sz, [p]), "xc_workspace_bytes": (sz, [p]),
+        "xc_set_workspace": (i, [p, p, sz]),
+        "xc_set_option": (i, [p, i, i]),
+        "xc_correlate": (i, [p, p, p, p]), "xc_correlate_acc": (i, [p, p, p, p]),
+        "xc_correlate_f32": (i, [p, p, p, i, p]),
+        "xc_correlate_pipelined": (i, [p, p, i, p, p, p, p]),
+        "xc_correlate_host": (i, [p, p, p, p, p, p]),
+        "xc_tile_count": (i, [p]),
+        "xc_tile_get": (i, [p, i, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i)]),
+        "xc_tri_index": (i64, [i64, i64]),
+        "xc_tri_inverse": (None, [i64, ctypes.POINTER(i64), ctypes.POINTER(i64)]),
+        "xc_last_launches": (i, [p]),
+        "xc_status_string": (ctypes.c_char_p, [i]),
+        "xc_last_cuda_error": (ctypes.c_char_p, [p]),
+        "xc_version": (ctypes.c_char_p, []),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = L
+    return L
+
+
+def lib() -> ctypes.CDLL:
+    return _lib if _lib is not None else load_library()
+
+
+def version() -> str:
+    return lib().xc_version().decode()
+
+
+def tri_index(bx: int, by: int) -> int:
+    """g = by(by+1)/2 + bx."""
+    return int(lib().xc_tri_index(bx, by))
+
+
+def tri_inverse(g: int) -> tuple[int, int]:
+    """(bx, by) from g (with the integer fix-up)."""
+    bx, by = ctypes.c_int64(), ctypes.c_int64()
+    lib().xc_tri_inverse(g, ctypes.byref(bx), ctypes.byref(by))
+    return int(bx.value), int(by.value)
+
+
+def shard_channels(F: int, world_size: int, rank: int) -> tuple[int, int]:
+    """Contiguous channel range [f_lo, f_hi) of `rank`: channels are independent and
+    the paper's multi-GPU plan is to give each GPU different channels, so sharding
+    needs no collective.  Sizes differ by at most one."""
+    base, rem = divmod(F, world_size)
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)
+
+
+def _stream_handle(stream) -> ctypes.c_void_p:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+class Plan:
+    """xc_plan(N, P=2, F, T, layout) + the calls of include/xc.h as methods."""
+
+    def __init__(self, N: int, F: int, T: int, P: int = 2, layout: int = 0):
+        self._h = ctypes.c_void_p()
+        rc = lib().xc_plan(ctypes.byref(self._h), N, P, F, T, layout)
+        if rc != 0:
+            self._h = ctypes.c_void_p()
+            raise XcError(rc, f"xc_plan(N={N}, P={P}, F={F}, T={T})")
+        self.N, self.P, self.F, self.T = N, P, F, T
+        self.NB = int(lib().xc_n_baselines(self._h))
+        self._ws = None
+
+    def close(self) -> None:
+        if getattr(self, "_h", None) and self._h.value:
+            lib().xc_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    __del__ = close
+
+    def _check(self, rc: int, where: str) -> None:
+        if rc != 0:
+            raise XcError(rc, where, lib().xc_last_cuda_error(self._h).decode())
+
+    # sizes ---------------------------------------------------------------------------------
+    @property
+    def in_bytes(self) -> int:
+        return int(lib().xc_in_bytes(self._h))
+
+    @property
+    def in_bytes_f32(self) -> int:
+        return int(lib().xc_in_bytes_f32(self._h))
+
+    @property
+    def vis_bytes(self) -> int:
+        return int(lib().xc_vis_bytes(self._h))
+
+    @property
+    def workspace_bytes(self) -> int:
+        return int(lib().xc_workspace_bytes(self._h))
+
+    @property
+    def last_launches(self) -> int:
+        return int(lib().xc_last_launches(self._h))
+
+    def in_shape(self):
+        return (self.T, self.F, self.N, 2, 2)
+
+    def vis_shape(self):
+        return (self.F, self.NB, 2, 2, 2)
+
+    # options / schedule --------------------------------------------------------------------
+    def set_option(self, option: int, value: int) -> None:
+        self._check(lib().xc_set_option(self._h, option, value), "xc_set_option")
+
+    def set_workspace(self, ws) -> None:
+        """ws: torch uint8/int8 CUDA tensor of at least workspace_bytes (kept alive by the plan)."""
+        self._check(lib().xc_set_workspace(self._h, ctypes.c_void_p(ws.data_ptr()), ws.numel() * ws.element_size()),
+                    "xc_set_workspace")
+        self._ws = ws
+
+    def tiles(self):
+        """[(bi, bj, si, sj)] of the integer path's per-channel tile schedule."""
+        out = []
+        bi, bj, si, sj = (ctypes.c_int() for _ in range(4))
+        for k in range(int(lib().xc_tile_count(self._h))):
+            self._check(lib().xc_tile_get(self._h, k, ctypes.byref(bi), ctypes.byref(bj), ctypes.byref(si),
+                                          ctypes.byref(sj)), "xc_tile_get")
+            out.append((bi.value, bj.value, si.value, sj.value))
+        return out
+
+    # compute -------------------------------------------------------------------------------
+    def _chk_in(self, x, dtype):
+        import torch
+        if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == dtype and x.is_contiguous()
+                and tuple(x.shape) == self.in_shape()):
+            raise ValueError(f"input must be a contiguous CUDA {dtype} tensor of shape {self.in_shape()}")
+
+    def _chk_vis(self, v, dtype):
+        import torch
+        if not (isinstance(v, torch.Tensor) and v.is_cuda and v.dtype == dtype and v.is_contiguous()
+                and tuple(v.shape) == self.vis_shape()):
+            raise ValueError(f"vis must be a contiguous CUDA {dtype} tensor of shape {self.vis_shape()}")
+
+    def new_vis(self, dtype=None, device="cuda"):
+        import torch
+        return torch.empty(self.vis_shape(), dtype=dtype or torch.int32, device=device)
+
+    def correlate(self, x, vis=None, stream=None):
+        """vis = X-engine(x).  x: int8 CUDA [T][F][N][2][2] -> int32 CUDA [F][NB][2][2][2]."""
+        import torch
+        self._chk_in(x, torch.int8)
+        if vis is None:
+            vis = self.new_vis(torch.int32, x.device)
+        self._chk_vis(vis, torch.int32)
+        self._check(lib().xc_correlate(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(vis.data_ptr()),
+                                       _stream_handle(stream)), "xc_correlate")
+        return vis
+
+    def correlate_acc(self, x, vis, stream=None):
+        """vis += X-engine(x)."""
+        import torch
+        self._chk_in(x, torch.int8)
+        self._chk_vis(vis, torch.int32)
+        self._check(lib().xc_correlate_acc(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(vis.data_ptr()),
+                                           _stream_handle(stream)), "xc_correlate_acc")
+        return vis
+
+    def correlate_f32(self, x, vis=None, accumulate=False, stream=None):
+        import torch
+        self._chk_in(x, torch.float32)
+        if vis is None:
+            vis = self.new_vis(torch.float32, x.device)
+        self._chk_vis(vis, torch.float32)
+        self._check(lib().xc_correlate_f32(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(vis.data_ptr()),
+                                           1 if accumulate else 0, _stream_handle(stream)), "xc_correlate_f32")
+        return vis
+
+    def correlate_pipelined(self, blocks_host, dev_buf2, vis, compute_stream, copy_stream):
+        """blocks_host: pinned CPU int8 tensor [n_blocks][T][F][N][2][2]; dev_buf2: CUDA int8 tensor of
+        2 * in_bytes; vis: CUDA int32.  Enqueues Algorithm 1 and returns; sync compute_stream."""
+        import torch
+        if not (blocks_host.dtype == torch.int8 and blocks_host.is_contiguous() and not blocks_host.is_cuda
+                and tuple(blocks_host.shape[1:]) == self.in_shape()):
+            raise ValueError("blocks_host must be a contiguous CPU int8 tensor [n_blocks][T][F][N][2][2]")
+        if dev_buf2.numel() * dev_buf2.element_size() < 2 * self.in_bytes:
+            raise ValueError("dev_buf2 too small")
+        self._chk_vis(vis, torch.int32)
+        self._check(lib().xc_correlate_pipelined(
+            self._h, ctypes.c_void_p(blocks_host.data_ptr()), int(blocks_host.shape[0]),
+            ctypes.c_void_p(dev_buf2.data_ptr()), ctypes.c_void_p(vis.data_ptr()),
+            ctypes.c_void_p(compute_stream.cuda_stream), ctypes.c_void_p(copy_stream.cuda_stream)),
+            "xc_correlate_pipelined")
+        return vis
+
+    def correlate_host(self, x_host, vis_host, in_dev, vis_dev, stream=None):
+        """End to end with HOST buffers (H2D copy, X-engine, D2H copy, stream sync)."""
+        self._check(lib().xc_correlate_host(
+            self._h, ctypes.c_void_p(x_host.data_ptr()), ctypes.c_void_p(vis_host.data_ptr()),
+            ctypes.c_void_p(in_dev.data_ptr()), ctypes.c_void_p(vis_dev.data_ptr()), _stream_handle(stream)),
+            "xc_correlate_host")
+        return vis_host

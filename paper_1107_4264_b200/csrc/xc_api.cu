@@ -1,0 +1,425 @@
+// xc_api.cu -- the C ABI of include/xc.h: plan (tile schedule, S1), dispatch of the staging (S0),
+// tensor-core (S2-S4), fp32 (S5) and two-stream (S6) paths.  Host code only launches this
+// library's own kernels; there is no CPU compute path.
+#include "../../include/xc.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "xc_f32.cuh"
+#include "xc_i8_tc.cuh"
+#include "xc_simt.cuh"
+
+namespace {
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// Tiles (bi on the i side in blocks of si stations, bj on the j side in blocks of sj stations)
+// that contain at least one stored pair i <= j < N, in the paper's triangular order
+// (PAPER.md:157): block row bj outermost, bi ascending inside it.
+std::vector<uint32_t> build_tiles(int N, int si, int sj) {
+    std::vector<uint32_t> t;
+    const int nbj = (N + sj - 1) / sj;
+    const int nbi = (N + si - 1) / si;
+    for (int bj = 0; bj < nbj; ++bj) {
+        const int jmax = (bj + 1) * sj - 1 < N - 1 ? (bj + 1) * sj - 1 : N - 1;
+        for (int bi = 0; bi < nbi; ++bi) {
+            if (bi * si <= jmax) t.push_back(static_cast<uint32_t>(bi) | (static_cast<uint32_t>(bj) << 16));
+        }
+    }
+    return t;
+}
+
+}  // namespace
+
+struct xc_plan_s {
+    int N = 0, P = 0, F = 0, T = 0;
+    long long NB = 0;
+    int Npad = 0;
+    int umma_n = 256;
+    std::vector<uint32_t> tiles_tc, tiles_f32;
+    // device state (created lazily on the device current at first compute call)
+    bool dev_ready = false;
+    int device = -1, sm_count = 0;
+    uint32_t* d_tiles_tc = nullptr;
+    uint32_t* d_tiles_f32 = nullptr;
+    PFN_encodeTiled encode = nullptr;
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    bool ws_owned = false;
+    int opt_kernel = XC_I8_KERNEL_AUTO, opt_max_ctas = 0, opt_force_stage = 0;
+    CUtensorMap tmap;
+    const void* tmap_src = nullptr;
+    int tmap_nrow = 0;
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_entry = nullptr;
+    int last_launches = 0;
+    std::string last_err;
+};
+
+namespace {
+
+int cuda_fail(xc_plan_t* p, cudaError_t e, const char* where) {
+    if (p) p->last_err = std::string(where) + ": " + cudaGetErrorString(e);
+    (void)cudaGetLastError();
+    return XC_ERR_CUDA;
+}
+#define XC_CUDA(p, call)                                              \
+    do {                                                              \
+        cudaError_t e__ = (call);                                     \
+        if (e__ != cudaSuccess) return cuda_fail((p), e__, #call);    \
+    } while (0)
+
+int ensure_device(xc_plan_t* p) {
+    if (p->dev_ready) return XC_OK;
+    int dev = 0;
+    XC_CUDA(p, cudaGetDevice(&dev));
+    int major = 0, sms = 0;
+    XC_CUDA(p, cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    XC_CUDA(p, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (major != 10) {
+        p->last_err = "device is not sm_100 (tcgen05/TMEM required); there is no fallback path";
+        return XC_ERR_UNSUPPORTED;
+    }
+    p->device = dev;
+    p->sm_count = sms;
+    XC_CUDA(p, cudaMalloc(&p->d_tiles_tc, p->tiles_tc.size() * sizeof(uint32_t)));
+    XC_CUDA(p, cudaMemcpy(p->d_tiles_tc, p->tiles_tc.data(), p->tiles_tc.size() * sizeof(uint32_t),
+                          cudaMemcpyHostToDevice));
+    XC_CUDA(p, cudaMalloc(&p->d_tiles_f32, p->tiles_f32.size() * sizeof(uint32_t)));
+    XC_CUDA(p, cudaMemcpy(p->d_tiles_f32, p->tiles_f32.data(), p->tiles_f32.size() * sizeof(uint32_t),
+                          cudaMemcpyHostToDevice));
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    XC_CUDA(p, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) {
+        p->last_err = "cuTensorMapEncodeTiled not available from the driver";
+        return XC_ERR_CUDA;
+    }
+    p->encode = reinterpret_cast<PFN_encodeTiled>(fn);
+    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    xc::TcCfg<256>::SMEM_BYTES));
+    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    xc::TcCfg<128>::SMEM_BYTES));
+    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    xc::F32_SMEM_BYTES));
+    p->dev_ready = true;
+    return XC_OK;
+}
+
+// S0: decide whether the padding kernel is needed and run it; *src / *nrow describe what TMA reads.
+int stage_if_needed(xc_plan_t* p, const int8_t* in_dev, cudaStream_t st, const void** src, int* nrow) {
+    const bool need = p->opt_force_stage || (p->N % 4 != 0) || (reinterpret_cast<uintptr_t>(in_dev) & 15u);
+    if (!need) {
+        *src = in_dev;
+        *nrow = p->N;
+        return XC_OK;
+    }
+    const size_t want = xc_workspace_bytes(p);
+    if (!p->ws) {
+        XC_CUDA(p, cudaMalloc(&p->ws, want));  // synchronising; documented in xc.h
+        p->ws_bytes = want;
+        p->ws_owned = true;
+    }
+    if (p->ws_bytes < want) return XC_ERR_NO_WORKSPACE;
+    const long long rows = static_cast<long long>(p->T) * p->F;
+    const long long total = rows * p->Npad;
+    long long blocks = (total + 255) / 256;
+    if (blocks > 148LL * 32) blocks = 148LL * 32;
+    xc::xc_stage_pad_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in_dev, static_cast<uint32_t*>(p->ws), rows,
+                                                                             p->N, p->Npad);
+    XC_CUDA(p, cudaGetLastError());
+    p->last_launches += 1;
+    *src = p->ws;
+    *nrow = p->Npad;
+    return XC_OK;
+}
+
+int encode_tmap(xc_plan_t* p, const void* src, int nrow) {
+    if (p->tmap_src == src && p->tmap_nrow == nrow) return XC_OK;
+    const cuuint64_t gdim[3] = {static_cast<cuuint64_t>(4) * nrow, static_cast<cuuint64_t>(p->F),
+                                static_cast<cuuint64_t>(p->T)};
+    const cuuint64_t gstride[2] = {static_cast<cuuint64_t>(4) * nrow,
+                                   static_cast<cuuint64_t>(4) * nrow * static_cast<cuuint64_t>(p->F)};
+    const cuuint32_t box[3] = {128, 1, static_cast<cuuint32_t>(xc::TC_BK)};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = p->encode(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(src), gdim, gstride, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        char buf[96];
+        snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed with CUresult %d", static_cast<int>(r));
+        p->last_err = buf;
+        p->tmap_src = nullptr;
+        return XC_ERR_CUDA;
+    }
+    p->tmap_src = src;
+    p->tmap_nrow = nrow;
+    return XC_OK;
+}
+
+int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* stream, int accumulate) {
+    if (!p || !in_dev || !vis_dev) return XC_ERR_INVALID_ARG;
+    if (reinterpret_cast<uintptr_t>(vis_dev) & 7u) return XC_ERR_ALIGNMENT;
+    int rc = ensure_device(p);
+    if (rc != XC_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    p->last_launches = 0;
+
+    if (p->opt_kernel == XC_I8_KERNEL_SIMT) {
+        if (p->F > 65535) return XC_ERR_UNSUPPORTED;
+        xc::SimtParams sp{p->N, p->F, p->T, p->NB, in_dev, vis_dev, accumulate};
+        const long long nb = (p->N + xc::SIMT_B - 1) / xc::SIMT_B;
+        dim3 grid(static_cast<unsigned>(nb * (nb + 1) / 2), static_cast<unsigned>(p->F));
+        xc::xc_i8_simt_kernel<<<grid, dim3(xc::SIMT_B, xc::SIMT_B), 0, st>>>(sp);
+        XC_CUDA(p, cudaGetLastError());
+        p->last_launches += 1;
+        return XC_OK;
+    }
+
+    const void* src = nullptr;
+    int nrow = 0;
+    rc = stage_if_needed(p, in_dev, st, &src, &nrow);
+    if (rc != XC_OK) return rc;
+    rc = encode_tmap(p, src, nrow);
+    if (rc != XC_OK) return rc;
+
+    xc::TcParams tp;
+    tp.N = p->N;
+    tp.F = p->F;
+    tp.T = p->T;
+    tp.tiles_per_f = static_cast<int>(p->tiles_tc.size());
+    tp.total_tiles = static_cast<long long>(p->F) * tp.tiles_per_f;
+    tp.NB = p->NB;
+    tp.tiles = p->d_tiles_tc;
+    tp.vis = vis_dev;
+    tp.accumulate = accumulate;
+    long long ctas = p->opt_max_ctas > 0 ? p->opt_max_ctas : p->sm_count;
+    if (ctas > tp.total_tiles) ctas = tp.total_tiles;
+    if (p->umma_n == 256) {
+        xc::xc_i8_tc_kernel<256><<<static_cast<unsigned>(ctas), xc::TC_THREADS, xc::TcCfg<256>::SMEM_BYTES, st>>>(p->tmap, tp);
+    } else {
+        xc::xc_i8_tc_kernel<128><<<static_cast<unsigned>(ctas), xc::TC_THREADS, xc::TcCfg<128>::SMEM_BYTES, st>>>(p->tmap, tp);
+    }
+    XC_CUDA(p, cudaGetLastError());
+    p->last_launches += 1;
+    return XC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int xc_plan(xc_plan_t** out, int N, int P, int F, int T, int layout) {
+    if (!out) return XC_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (N < 1 || F < 1 || T < 1) return XC_ERR_INVALID_ARG;
+    if (P != 2 || layout != XC_LAYOUT_TFSPC) return XC_ERR_UNSUPPORTED;
+    if (T > XC_MAX_T) return XC_ERR_OVERFLOW;
+    if (N > 32768) return XC_ERR_UNSUPPORTED;  // tile indices are 16-bit; 4N*F*T must also fit the address space
+    xc_plan_t* p = new (std::nothrow) xc_plan_s();
+    if (!p) return XC_ERR_INVALID_ARG;
+    p->N = N;
+    p->P = P;
+    p->F = F;
+    p->T = T;
+    p->NB = static_cast<long long>(N) * (N + 1) / 2;
+    p->Npad = (N + 3) & ~3;
+    // Tile width on the j side: 64 stations (UMMA_N = 256) unless the narrower 32-station tile
+    // wastes clearly less of the tensor pipe on the diagonal (small N).
+    const std::vector<uint32_t> t256 = build_tiles(N, 32, 64), t128 = build_tiles(N, 32, 32);
+    const double area256 = 256.0 * t256.size(), area128 = 128.0 * t128.size();
+    if (area128 < 0.8 * area256) {
+        p->umma_n = 128;
+        p->tiles_tc = t128;
+    } else {
+        p->umma_n = 256;
+        p->tiles_tc = t256;
+    }
+    p->tiles_f32 = build_tiles(N, xc::F32_SI, xc::F32_SJ);
+    memset(&p->tmap, 0, sizeof p->tmap);
+    *out = p;
+    return XC_OK;
+}
+
+void xc_destroy(xc_plan_t* p) {
+    if (!p) return;
+    if (p->d_tiles_tc) cudaFree(p->d_tiles_tc);
+    if (p->d_tiles_f32) cudaFree(p->d_tiles_f32);
+    if (p->ws && p->ws_owned) cudaFree(p->ws);
+    for (int k = 0; k < 2; ++k) {
+        if (p->ev_copied[k]) cudaEventDestroy(p->ev_copied[k]);
+        if (p->ev_free[k]) cudaEventDestroy(p->ev_free[k]);
+    }
+    if (p->ev_entry) cudaEventDestroy(p->ev_entry);
+    delete p;
+}
+
+size_t xc_in_bytes(const xc_plan_t* p) { return p ? static_cast<size_t>(4) * p->N * p->F * p->T : 0; }
+size_t xc_in_bytes_f32(const xc_plan_t* p) { return p ? static_cast<size_t>(16) * p->N * p->F * p->T : 0; }
+size_t xc_vis_bytes(const xc_plan_t* p) { return p ? static_cast<size_t>(32) * p->NB * p->F : 0; }
+size_t xc_n_baselines(const xc_plan_t* p) { return p ? static_cast<size_t>(p->NB) : 0; }
+size_t xc_workspace_bytes(const xc_plan_t* p) { return p ? static_cast<size_t>(4) * p->Npad * p->F * p->T : 0; }
+
+int xc_set_workspace(xc_plan_t* p, void* ws_dev, size_t bytes) {
+    if (!p) return XC_ERR_INVALID_ARG;
+    if (ws_dev && (reinterpret_cast<uintptr_t>(ws_dev) & 127u)) return XC_ERR_ALIGNMENT;
+    if (ws_dev && bytes < xc_workspace_bytes(p)) return XC_ERR_NO_WORKSPACE;
+    if (p->ws && p->ws_owned) cudaFree(p->ws);
+    p->ws = ws_dev;
+    p->ws_bytes = ws_dev ? bytes : 0;
+    p->ws_owned = false;
+    p->tmap_src = nullptr;
+    return XC_OK;
+}
+
+int xc_set_option(xc_plan_t* p, int option, int value) {
+    if (!p) return XC_ERR_INVALID_ARG;
+    switch (option) {
+        case XC_OPT_I8_KERNEL:
+            if (value < XC_I8_KERNEL_AUTO || value > XC_I8_KERNEL_SIMT) return XC_ERR_INVALID_ARG;
+            p->opt_kernel = value;
+            return XC_OK;
+        case XC_OPT_MAX_CTAS:
+            if (value < 0) return XC_ERR_INVALID_ARG;
+            p->opt_max_ctas = value;
+            return XC_OK;
+        case XC_OPT_FORCE_STAGE:
+            p->opt_force_stage = value ? 1 : 0;
+            return XC_OK;
+        default:
+            return XC_ERR_INVALID_ARG;
+    }
+}
+
+int xc_correlate(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* stream) {
+    return correlate_i8(p, in_dev, vis_dev, stream, 0);
+}
+int xc_correlate_acc(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* stream) {
+    return correlate_i8(p, in_dev, vis_dev, stream, 1);
+}
+
+int xc_correlate_f32(xc_plan_t* p, const float* in_dev, float* vis_dev, int accumulate, void* stream) {
+    if (!p || !in_dev || !vis_dev) return XC_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(in_dev) & 15u) || (reinterpret_cast<uintptr_t>(vis_dev) & 15u))
+        return XC_ERR_ALIGNMENT;
+    int rc = ensure_device(p);
+    if (rc != XC_OK) return rc;
+    p->last_launches = 0;
+    xc::F32Params fp;
+    fp.N = p->N;
+    fp.F = p->F;
+    fp.T = p->T;
+    fp.tiles_per_f = static_cast<int>(p->tiles_f32.size());
+    fp.NB = p->NB;
+    fp.tiles = p->d_tiles_f32;
+    fp.in = reinterpret_cast<const float4*>(in_dev);
+    fp.vis = vis_dev;
+    fp.accumulate = accumulate ? 1 : 0;
+    const long long total = static_cast<long long>(p->F) * fp.tiles_per_f;
+    if (total > 0x7FFFFFFFLL) return XC_ERR_UNSUPPORTED;
+    xc::xc_f32_kernel<<<static_cast<unsigned>(total), xc::F32_THREADS, xc::F32_SMEM_BYTES,
+                        static_cast<cudaStream_t>(stream)>>>(fp);
+    XC_CUDA(p, cudaGetLastError());
+    p->last_launches = 1;
+    return XC_OK;
+}
+
+int xc_correlate_pipelined(xc_plan_t* p, const int8_t* in_host, int n_blocks, int8_t* dev_buf2, int32_t* vis_dev,
+                           void* compute_stream, void* copy_stream) {
+    if (!p || !in_host || !dev_buf2 || !vis_dev || n_blocks < 1) return XC_ERR_INVALID_ARG;
+    if (reinterpret_cast<uintptr_t>(dev_buf2) & 127u) return XC_ERR_ALIGNMENT;
+    int rc = ensure_device(p);
+    if (rc != XC_OK) return rc;
+    cudaStream_t cs = static_cast<cudaStream_t>(compute_stream), xs = static_cast<cudaStream_t>(copy_stream);
+    for (int k = 0; k < 2; ++k) {
+        if (!p->ev_copied[k]) XC_CUDA(p, cudaEventCreateWithFlags(&p->ev_copied[k], cudaEventDisableTiming));
+        if (!p->ev_free[k]) XC_CUDA(p, cudaEventCreateWithFlags(&p->ev_free[k], cudaEventDisableTiming));
+    }
+    if (!p->ev_entry) XC_CUDA(p, cudaEventCreateWithFlags(&p->ev_entry, cudaEventDisableTiming));
+    const size_t blk = xc_in_bytes(p);
+    const size_t half = blk;  // a half that ends up not 16-byte aligned simply goes through staging (S0)
+    int launches = 0;
+    // Earlier work on the compute stream may still read dev_buf2: copies start after it.
+    XC_CUDA(p, cudaEventRecord(p->ev_entry, cs));
+    XC_CUDA(p, cudaStreamWaitEvent(xs, p->ev_entry, 0));
+    XC_CUDA(p, cudaMemcpyAsync(dev_buf2, in_host, blk, cudaMemcpyHostToDevice, xs));
+    XC_CUDA(p, cudaEventRecord(p->ev_copied[0], xs));
+    for (int b = 0; b < n_blocks; ++b) {
+        if (b + 1 < n_blocks) {
+            const int nb = (b + 1) & 1;
+            if (b >= 1) XC_CUDA(p, cudaStreamWaitEvent(xs, p->ev_free[nb], 0));  // X-engine on block b-1 is done with it
+            XC_CUDA(p, cudaMemcpyAsync(dev_buf2 + nb * half, in_host + static_cast<size_t>(b + 1) * blk, blk,
+                                       cudaMemcpyHostToDevice, xs));
+            XC_CUDA(p, cudaEventRecord(p->ev_copied[nb], xs));
+        }
+        XC_CUDA(p, cudaStreamWaitEvent(cs, p->ev_copied[b & 1], 0));
+        rc = correlate_i8(p, dev_buf2 + (b & 1) * half, vis_dev, compute_stream, b > 0 ? 1 : 0);
+        if (rc != XC_OK) return rc;
+        launches += p->last_launches;
+        XC_CUDA(p, cudaEventRecord(p->ev_free[b & 1], cs));
+    }
+    p->last_launches = launches;
+    return XC_OK;
+}
+
+int xc_correlate_host(xc_plan_t* p, const int8_t* in_host, int32_t* vis_host, int8_t* in_dev_scratch,
+                      int32_t* vis_dev_scratch, void* stream) {
+    if (!p || !in_host || !vis_host || !in_dev_scratch || !vis_dev_scratch) return XC_ERR_INVALID_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    XC_CUDA(p, cudaMemcpyAsync(in_dev_scratch, in_host, xc_in_bytes(p), cudaMemcpyHostToDevice, st));
+    int rc = correlate_i8(p, in_dev_scratch, vis_dev_scratch, stream, 0);
+    if (rc != XC_OK) return rc;
+    XC_CUDA(p, cudaMemcpyAsync(vis_host, vis_dev_scratch, xc_vis_bytes(p), cudaMemcpyDeviceToHost, st));
+    XC_CUDA(p, cudaStreamSynchronize(st));
+    return XC_OK;
+}
+
+int xc_tile_count(const xc_plan_t* p) { return p ? static_cast<int>(p->tiles_tc.size()) : 0; }
+
+int xc_tile_get(const xc_plan_t* p, int k, int* bi, int* bj, int* si, int* sj) {
+    if (!p || k < 0 || k >= static_cast<int>(p->tiles_tc.size())) return XC_ERR_INVALID_ARG;
+    if (bi) *bi = static_cast<int>(p->tiles_tc[k] & 0xFFFFu);
+    if (bj) *bj = static_cast<int>(p->tiles_tc[k] >> 16);
+    if (si) *si = 32;
+    if (sj) *sj = p->umma_n / 4;
+    return XC_OK;
+}
+
+int64_t xc_tri_index(int64_t bx, int64_t by) { return by * (by + 1) / 2 + bx; }
+
+void xc_tri_inverse(int64_t g, int64_t* bx, int64_t* by) {
+    long long x = 0, y = 0;
+    xc::tri_inverse(g, &x, &y);
+    if (bx) *bx = x;
+    if (by) *by = y;
+}
+
+int xc_last_launches(const xc_plan_t* p) { return p ? p->last_launches : 0; }
+
+const char* xc_status_string(int s) {
+    switch (s) {
+        case XC_OK: return "XC_OK";
+        case XC_ERR_INVALID_ARG: return "XC_ERR_INVALID_ARG";
+        case XC_ERR_UNSUPPORTED: return "XC_ERR_UNSUPPORTED";
+        case XC_ERR_OVERFLOW: return "XC_ERR_OVERFLOW";
+        case XC_ERR_ALIGNMENT: return "XC_ERR_ALIGNMENT";
+        case XC_ERR_CUDA: return "XC_ERR_CUDA";
+        case XC_ERR_NO_WORKSPACE: return "XC_ERR_NO_WORKSPACE";
+        default: return "XC_ERR_UNKNOWN";
+    }
+}
+
+const char* xc_last_cuda_error(const xc_plan_t* p) { return p ? p->last_err.c_str() : ""; }
+
+const char* xc_version(void) { return "xcorr-b200 0.1 (sm_100a, tcgen05 kind::i8)"; }
+
+}  // extern "C"

@@ -1,0 +1,143 @@
+// xc_f32.cuh -- the fp32-input X-engine on the CUDA cores.
+//
+// The paper's own arithmetic (a station pair costs 16 fp32 FMAs per sample) and its
+// own tiling idea: a register tile of station pairs per thread, fed
+// from a shared-memory tile of input vectors that the whole block loads cooperatively, filled in
+// only at the innermost level.  Re-sized for sm_100a: 2 x 4 station pairs per thread (64 fp32
+// accumulators; the paper's Fermi kernel 11 used 2 x 2), a 32 x 64 station tile per 256-thread
+// block, and a 3-stage cp.async ring in place of the paper's double-buffered texture loads.
+// Only tiles that intersect i <= j are launched; threads above the diagonal
+// compute but do not write (the paper's software-cache choice).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace xc {
+
+constexpr int F32_SI = 32;       // stations per tile on the i side
+constexpr int F32_SJ = 64;       // stations per tile on the j side
+constexpr int F32_BK = 16;       // samples per ring stage
+constexpr int F32_STAGES = 3;
+constexpr int F32_THREADS = 256;
+constexpr int F32_STAGE_F4 = F32_BK * (F32_SI + F32_SJ);             // float4 per stage
+constexpr int F32_SMEM_BYTES = F32_STAGES * F32_STAGE_F4 * 16;       // 72 KB
+
+struct F32Params {
+    int N, F, T;
+    int tiles_per_f;
+    long long NB;
+    const uint32_t* tiles;  // device: bi | (bj << 16), bi in 32-station blocks, bj in 64-station blocks
+    const float4* in;       // one float4 per (t, f, station): (p0.re, p0.im, p1.re, p1.im)
+    float* vis;
+    int accumulate;
+};
+
+__device__ __forceinline__ void cp_async16(uint32_t dst_smem, const void* src, int src_bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst_smem), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+
+// acc[(pi*2+pj)*2 + c] += a_{pi} * conj(b_{pj}): 16 FMAs.
+__device__ __forceinline__ void cmac4(float (&acc)[8], const float4& a, const float4& b) {
+    // pi = 0: (a.x, a.y); pi = 1: (a.z, a.w); pj = 0: (b.x, b.y); pj = 1: (b.z, b.w)
+    acc[0] = fmaf(a.x, b.x, acc[0]); acc[0] = fmaf(a.y, b.y, acc[0]);
+    acc[1] = fmaf(a.y, b.x, acc[1]); acc[1] = fmaf(-a.x, b.y, acc[1]);
+    acc[2] = fmaf(a.x, b.z, acc[2]); acc[2] = fmaf(a.y, b.w, acc[2]);
+    acc[3] = fmaf(a.y, b.z, acc[3]); acc[3] = fmaf(-a.x, b.w, acc[3]);
+    acc[4] = fmaf(a.z, b.x, acc[4]); acc[4] = fmaf(a.w, b.y, acc[4]);
+    acc[5] = fmaf(a.w, b.x, acc[5]); acc[5] = fmaf(-a.z, b.y, acc[5]);
+    acc[6] = fmaf(a.z, b.z, acc[6]); acc[6] = fmaf(a.w, b.w, acc[6]);
+    acc[7] = fmaf(a.w, b.z, acc[7]); acc[7] = fmaf(-a.z, b.w, acc[7]);
+}
+
+__global__ void __launch_bounds__(F32_THREADS, 2) xc_f32_kernel(const F32Params p) {
+    extern __shared__ __align__(16) float4 smem_f4[];
+    const int tid = threadIdx.x;
+    const int ti = tid & 15;   // stations i0 + ti, i0 + ti + 16
+    const int tj = tid >> 4;   // stations j0 + tj + 16 n, n = 0..3
+
+    const long long w = blockIdx.x;
+    const int f = static_cast<int>(w / p.tiles_per_f);
+    const uint32_t tb = __ldg(p.tiles + static_cast<int>(w % p.tiles_per_f));
+    const int i0 = static_cast<int>(tb & 0xFFFFu) * F32_SI;
+    const int j0 = static_cast<int>(tb >> 16) * F32_SJ;
+
+    const uint32_t smem0 = static_cast<uint32_t>(__cvta_generic_to_shared(smem_f4));
+    const int KB = (p.T + F32_BK - 1) / F32_BK;
+
+    // Cooperative load of one stage: F32_BK rows of (32 + 64) float4; zero fill outside [0,T) x [0,N).
+    auto load_stage = [&](int kb, int stage) {
+        const uint32_t sbase = smem0 + static_cast<uint32_t>(stage * F32_STAGE_F4 * 16);
+#pragma unroll
+        for (int r = 0; r < F32_STAGE_F4 / F32_THREADS; ++r) {
+            const int idx = tid + r * F32_THREADS;
+            const int k = idx / (F32_SI + F32_SJ);
+            const int c = idx - k * (F32_SI + F32_SJ);
+            const int s = (c < F32_SI) ? (i0 + c) : (j0 + c - F32_SI);
+            const int t = kb * F32_BK + k;
+            const bool ok = (t < p.T) && (s < p.N) && (kb < KB);
+            const float4* src = ok ? (p.in + (static_cast<long long>(t) * p.F + f) * p.N + s) : p.in;
+            cp_async16(sbase + static_cast<uint32_t>(idx * 16), src, ok ? 16 : 0);
+        }
+    };
+
+    float acc[2][4][8];
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b)
+#pragma unroll
+            for (int c = 0; c < 8; ++c) acc[a][b][c] = 0.f;
+
+#pragma unroll
+    for (int s = 0; s < F32_STAGES - 1; ++s) {
+        load_stage(s, s);
+        cp_async_commit();
+    }
+
+    for (int kb = 0; kb < KB; ++kb) {
+        cp_async_wait<F32_STAGES - 2>();
+        __syncthreads();
+        load_stage(kb + F32_STAGES - 1, (kb + F32_STAGES - 1) % F32_STAGES);
+        cp_async_commit();
+        const float4* sA = smem_f4 + (kb % F32_STAGES) * F32_STAGE_F4;
+#pragma unroll
+        for (int k = 0; k < F32_BK; ++k) {
+            const float4* row = sA + k * (F32_SI + F32_SJ);
+            const float4 a0 = row[ti], a1 = row[ti + 16];
+            const float4 b0 = row[F32_SI + tj], b1 = row[F32_SI + tj + 16];
+            const float4 b2 = row[F32_SI + tj + 32], b3 = row[F32_SI + tj + 48];
+            cmac4(acc[0][0], a0, b0); cmac4(acc[0][1], a0, b1); cmac4(acc[0][2], a0, b2); cmac4(acc[0][3], a0, b3);
+            cmac4(acc[1][0], a1, b0); cmac4(acc[1][1], a1, b1); cmac4(acc[1][2], a1, b2); cmac4(acc[1][3], a1, b3);
+        }
+    }
+    cp_async_wait<0>();
+
+    float* visf = p.vis + static_cast<long long>(f) * p.NB * 8;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        const int j = j0 + tj + 16 * b;
+#pragma unroll
+        for (int a = 0; a < 2; ++a) {
+            const int i = i0 + ti + 16 * a;
+            if (i <= j && j < p.N) {
+                float4* dst = reinterpret_cast<float4*>(visf + (static_cast<long long>(j) * (j + 1) / 2 + i) * 8);
+                float4 lo = make_float4(acc[a][b][0], acc[a][b][1], acc[a][b][2], acc[a][b][3]);
+                float4 hi = make_float4(acc[a][b][4], acc[a][b][5], acc[a][b][6], acc[a][b][7]);
+                if (p.accumulate) {
+                    const float4 o0 = dst[0], o1 = dst[1];
+                    lo.x += o0.x; lo.y += o0.y; lo.z += o0.z; lo.w += o0.w;
+                    hi.x += o1.x; hi.y += o1.y; hi.z += o1.z; hi.w += o1.w;
+                }
+                dst[0] = lo;
+                dst[1] = hi;
+            }
+        }
+    }
+}
+
+}  // namespace xc

@@ -1,0 +1,84 @@
+// xc_simt.cuh -- (a) a plain CUDA-core int8 X-engine, one thread per station pair, kept as a
+// debugging aid for the tensor-core kernel (XC_I8_KERNEL_SIMT; never chosen by AUTO), and
+// (b) the staging kernel of SURVEY 8(a) S0 that pads the station axis for TMA.
+//
+// (a) is the paper's simplest mapping, R = (1,1): each thread owns one
+// station pair and its four polarisation products, reads both stations' samples straight from
+// global memory (hardware-managed cache), and the thread-block grid covers the lower triangle
+// through the closed-form map of PAPER.md:157-163.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace xc {
+
+constexpr int SIMT_B = 16;  // stations per block edge
+
+struct SimtParams {
+    int N, F, T;
+    long long NB;
+    const int8_t* in;
+    int32_t* vis;
+    int accumulate;
+};
+
+// by = floor(-1/2 + sqrt(1/4 + 2g)), bx = g - by(by+1)/2, with an integer
+// fix-up because the floating square root is exact only for small g (SURVEY 8(c) reading 12).
+__host__ __device__ inline void tri_inverse(long long g, long long* bx, long long* by) {
+    long long y = static_cast<long long>(-0.5 + sqrt(0.25 + 2.0 * static_cast<double>(g)));
+    if (y < 0) y = 0;
+    while (y * (y + 1) / 2 > g) --y;
+    while ((y + 1) * (y + 2) / 2 <= g) ++y;
+    *by = y;
+    *bx = g - y * (y + 1) / 2;
+}
+
+__global__ void __launch_bounds__(SIMT_B* SIMT_B) xc_i8_simt_kernel(const SimtParams p) {
+    long long bx, by;
+    tri_inverse(blockIdx.x, &bx, &by);  // bx <= by: block column (i side), block row (j side)
+    const int f = blockIdx.y;
+    const int i = static_cast<int>(bx) * SIMT_B + threadIdx.x;
+    const int j = static_cast<int>(by) * SIMT_B + threadIdx.y;
+    if (i > j || j >= p.N) return;  // super-diagonal threads exit
+    int acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (int t = 0; t < p.T; ++t) {
+        const int8_t* x = p.in + (static_cast<long long>(t) * p.F + f) * p.N * 4;
+        int a[4], b[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            a[k] = x[i * 4 + k];
+            b[k] = x[j * 4 + k];
+        }
+#pragma unroll
+        for (int pi = 0; pi < 2; ++pi)
+#pragma unroll
+            for (int pj = 0; pj < 2; ++pj) {
+                acc[(pi * 2 + pj) * 2 + 0] += a[2 * pi] * b[2 * pj] + a[2 * pi + 1] * b[2 * pj + 1];
+                acc[(pi * 2 + pj) * 2 + 1] += a[2 * pi + 1] * b[2 * pj] - a[2 * pi] * b[2 * pj + 1];
+            }
+    }
+    int32_t* dst = p.vis + (static_cast<long long>(f) * p.NB + static_cast<long long>(j) * (j + 1) / 2 + i) * 8;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) dst[k] = p.accumulate ? dst[k] + acc[k] : acc[k];
+}
+
+// (b) Staging: rows of 4N bytes -> rows of 4*Npad bytes (Npad = N rounded up to 4), zero padded,
+// written to a 128-byte-aligned workspace.  One thread per destination station (4 bytes).
+__global__ void xc_stage_pad_kernel(const int8_t* __restrict__ in, uint32_t* __restrict__ out, long long rows, int N,
+                                    int Npad) {
+    const long long total = rows * Npad;
+    for (long long k = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; k < total;
+         k += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long r = k / Npad;
+        const int s = static_cast<int>(k - r * Npad);
+        uint32_t v = 0;
+        if (s < N) {
+            const uint8_t* src = reinterpret_cast<const uint8_t*>(in) + (r * N + s) * 4;
+            v = static_cast<uint32_t>(src[0]) | (static_cast<uint32_t>(src[1]) << 8) |
+                (static_cast<uint32_t>(src[2]) << 16) | (static_cast<uint32_t>(src[3]) << 24);
+        }
+        out[k] = v;
+    }
+}
+
+}  // namespace xc

@@ -1,0 +1,125 @@
+"""CPU-side checks of the C-ABI library (no compute calls): it loads, exports every symbol
+include/xc.h declares, validates arguments, and its triangular tile schedule
+covers every stored station pair exactly once."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_1107_4264_b200 as xcb
+from paper_1107_4264_b200 import build as xc_build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    xc_build.build()
+    xcb.load_library()
+
+
+def test_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "xc.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(xc_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(xcb.EXPORTED_SYMBOLS)
+    L = ctypes.CDLL(xcb.binding.LIB_PATH)
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_no_oracle_or_cpu_path_in_product():
+    """The product package never imports the oracle (or numpy compute) -- parity would be void."""
+    pkg = os.path.join(ROOT, "paper_1107_4264_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, fn)).read()
+                assert "oracle" not in src.replace("no oracle", ""), fn
+                assert "xo_" not in src, fn
+
+
+def test_plan_argument_validation():
+    L = xcb.lib()
+    h = ctypes.c_void_p()
+    assert L.xc_plan(ctypes.byref(h), 16, 2, 4, 256, 0) == 0 and h.value
+    assert L.xc_in_bytes(h) == 4 * 16 * 4 * 256
+    assert L.xc_in_bytes_f32(h) == 16 * 16 * 4 * 256
+    assert L.xc_n_baselines(h) == 136                      # BASELINE.json configs[0]
+    assert L.xc_vis_bytes(h) == 32 * 136 * 4
+    L.xc_destroy(h)
+    for args, code in [((0, 2, 4, 8, 0), -1), ((4, 2, 0, 8, 0), -1), ((4, 2, 4, 0, 0), -1),
+                       ((4, 1, 4, 8, 0), -2), ((4, 2, 4, 8, 7), -2), ((4, 2, 4, 65536, 0), -3)]:
+        h = ctypes.c_void_p()
+        assert L.xc_plan(ctypes.byref(h), *args) == code, args
+        assert not h.value
+    assert L.xc_plan(None, 4, 2, 4, 8, 0) == -1
+    assert L.xc_status_string(-3) == b"XC_ERR_OVERFLOW"
+    L.xc_destroy(None)
+    # 2 * 128^2 * XC_MAX_T still fits int32, one more sample does not (PAPER.md:96 reading 7)
+    assert 2 * 128 * 128 * xcb.MAX_T < 2 ** 31 <= 2 * 128 * 128 * (xcb.MAX_T + 1)
+
+
+def test_compute_without_gpu_fails_loudly():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("has a GPU")
+    p = xcb.Plan(8, 2, 16)
+    fake = ctypes.c_void_p(0x1000)
+    rc = xcb.lib().xc_correlate(p._h, fake, fake, None)
+    assert rc in (-5, -2)                                  # XC_ERR_CUDA / UNSUPPORTED: never a CPU fallback
+    rc = xcb.lib().xc_correlate_f32(p._h, fake, fake, 0, None)
+    assert rc in (-5, -2)
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 5, 16, 31, 32, 33, 64, 65, 100, 128, 129, 256, 500, 512, 1024])
+def test_tile_schedule_covers_triangle_exactly_once(N):
+    p = xcb.Plan(N, 1, 8)
+    tiles = p.tiles()
+    cover = np.zeros((N, N), np.int32)
+    for bi, bj, si, sj in tiles:
+        i0, j0 = bi * si, bj * sj
+        assert i0 < N and j0 < N
+        ii = np.arange(i0, min(i0 + si, N))[:, None]
+        jj = np.arange(j0, min(j0 + sj, N))[None, :]
+        assert (ii <= jj).any(), "a scheduled tile holds no stored pair"
+        cover[i0:i0 + si, j0:j0 + sj] += 1
+    iu = np.triu_indices(N)                                # i <= j
+    assert (cover[iu] == 1).all()
+    assert len(set((t[0], t[1]) for t in tiles)) == len(tiles)
+    # raw/useful area as in the paper's wasted-work model: never worse than 3x at N >= 64
+    if N >= 64:
+        raw = sum(si * sj for _, _, si, sj in tiles)
+        assert raw <= 3.0 * (N * (N + 1) // 2)
+
+
+def test_tile_counts_match_survey_table():
+    """S1: 128x256 tiles per channel."""
+    for N, n in [(128, 6), (256, 20), (512, 72), (1024, 272)]:
+        assert len(xcb.Plan(N, 1, 8).tiles()) == n
+
+
+def test_triangular_map_round_trip():
+    """g = by(by+1)/2 + bx and its inverse."""
+    g = 0
+    for by in range(0, 300):
+        for bx in range(0, by + 1):
+            assert xcb.tri_index(bx, by) == g
+            assert xcb.tri_inverse(g) == (bx, by)
+            g += 1
+    for by in [10 ** 6, 94906265, 94906266, 2 ** 31 - 1, 3 * 10 ** 9]:   # around 2g ~ 2^53: float sqrt is inexact
+        for bx in (0, 1, by // 2, by - 1, by):
+            g = by * (by + 1) // 2 + bx
+            assert xcb.tri_inverse(g) == (bx, by)
+
+
+def test_shard_channels_partition():
+    for F in (1, 7, 64, 1024):
+        for ws in (1, 2, 3, 8):
+            parts = [xcb.shard_channels(F, ws, r) for r in range(ws)]
+            assert parts[0][0] == 0 and parts[-1][1] == F
+            assert all(parts[k][1] == parts[k + 1][0] for k in range(ws - 1))
+            sizes = [hi - lo for lo, hi in parts]
+            assert max(sizes) - min(sizes) <= 1

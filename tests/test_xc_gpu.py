@@ -1,0 +1,308 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+int8 path: bit-exact.  fp32 path: |V - V64| <= 1e-5 * sqrt(V64_ii * V64_jj) (north_star; SURVEY 8(c)
+reading 13), and exactly equal to the int8 result for integer-valued input whose sums stay below 2^24.
+At BASELINE.json's full sizes the oracle covers a sample of channels (always f = 0 and F-1, all
+baselines) and an independent exact fp64 matmul on the GPU (torch, no code shared with the kernels:
+every partial sum is < 2^53) covers every output.
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_1107_4264_b200 as xcb
+import xc_workloads as wl
+from oracle import xo
+from paper_1107_4264_b200 import build as xc_build
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    xc_build.build()
+    xcb.load_library()
+    assert torch.cuda.is_available()
+
+
+def run_i8(x_np, kernel=xcb.I8_KERNEL_AUTO, force_stage=False, max_ctas=0):
+    T, F, N = x_np.shape[:3]
+    p = xcb.Plan(N, F, T)
+    p.set_option(xcb.OPT_I8_KERNEL, kernel)
+    p.set_option(xcb.OPT_FORCE_STAGE, int(force_stage))
+    p.set_option(xcb.OPT_MAX_CTAS, max_ctas)
+    x = torch.from_numpy(x_np).cuda()
+    vis = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32, device="cuda")  # poison: every entry must be written
+    p.correlate(x, vis)
+    torch.cuda.synchronize()
+    out = vis.cpu().numpy()
+    p.close()
+    return out
+
+
+def gram_check_fp64(x_gpu, vis_gpu, f_chunk=8):
+    """Independent exact check of EVERY output: fp64 matmul of the real 4N x T matrix per channel."""
+    T, F, N = x_gpu.shape[:3]
+    iu = torch.triu_indices(N, N, device="cuda")            # (i, j) with i <= j
+    order = torch.argsort(iu[1] * (iu[1] + 1) // 2 + iu[0])
+    ii, jj = iu[0][order], iu[1][order]
+    for f0 in range(0, F, f_chunk):
+        f1 = min(F, f0 + f_chunk)
+        z = x_gpu[:, f0:f1].reshape(T, f1 - f0, 2 * N, 2).to(torch.float64)
+        zc = torch.complex(z[..., 0], z[..., 1]).permute(1, 2, 0)            # [f][2N][T]
+        full = zc @ zc.conj().transpose(1, 2)                                  # x x^H, [f][2N][2N]
+        full = full.reshape(f1 - f0, N, 2, N, 2)
+        ref = full[:, ii, :, jj, :]                                            # [nb][f][pi][pj] (advanced idx first)
+        ref = ref.permute(1, 0, 2, 3)
+        ref = torch.stack([ref.real, ref.imag], dim=-1).round().to(torch.int64)
+        got = vis_gpu[f0:f1].to(torch.int64)
+        if not torch.equal(ref, got):
+            bad = (ref != got).nonzero()[0].tolist()
+            raise AssertionError(f"mismatch at f={f0 + bad[0]} b={bad[1]} idx={bad[2:]}: "
+                                 f"ref={ref[tuple(bad)].item()} got={got[tuple(bad)].item()}")
+
+
+# ---------------------------------------------------------------------------------------------
+# config 1 in full, both kernels
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("kernel", [xcb.I8_KERNEL_TC, xcb.I8_KERNEL_SIMT])
+def test_config1_full(kernel):
+    w = wl.CONFIGS["cfg1"]
+    x = wl.make_input(w)
+    ref = xo.correlate_i8(x)
+    got = run_i8(x, kernel)
+    assert got.shape == (4, 136, 2, 2, 2)
+    assert np.array_equal(got, ref)
+
+
+# ---------------------------------------------------------------------------------------------
+# small shapes: several tiles, ragged tails in N and T, degenerate sizes
+# ---------------------------------------------------------------------------------------------
+
+SMALL = [(1, 1, 1), (2, 3, 5), (3, 2, 31), (5, 2, 33), (16, 3, 64), (31, 2, 65), (32, 2, 100), (33, 2, 129),
+         (40, 3, 1000), (64, 2, 200), (65, 2, 96), (100, 2, 257), (128, 2, 300), (132, 1, 130), (200, 1, 70),
+         (257, 1, 64), (300, 1, 33)]
+
+
+@pytest.mark.parametrize("N,F,T", SMALL)
+def test_small_shapes_tc(N, F, T):
+    x = wl.full_range(N, F, T, seed=N * 1000 + T)            # whole int8 range incl. -128 (reading 6)
+    ref = xo.correlate_i8(x)
+    assert np.array_equal(run_i8(x, xcb.I8_KERNEL_TC), ref)
+
+
+@pytest.mark.parametrize("N,F,T", [(1, 1, 1), (5, 2, 33), (33, 2, 129), (100, 2, 57)])
+def test_small_shapes_simt(N, F, T):
+    x = wl.full_range(N, F, T, seed=7 + N)
+    assert np.array_equal(run_i8(x, xcb.I8_KERNEL_SIMT), xo.correlate_i8(x))
+
+
+def test_all_minus_128():
+    """Worst case magnitude: every component -128; V = 2 * 128^2 * T on every real part."""
+    N, F, T = 36, 2, 96
+    x = np.full((T, F, N, 2, 2), -128, np.int8)
+    got = run_i8(x)
+    assert np.array_equal(got, xo.correlate_i8(x))
+    assert (got[..., 0] == 2 * 128 * 128 * T).all() and (got[..., 1] == 0).all()
+
+
+def test_max_T_no_overflow():
+    """T = XC_MAX_T with all -128: 2 * 128^2 * 65535 = 2147450880 < 2^31 (reading 7)."""
+    N, F, T = 4, 1, xcb.MAX_T
+    x = np.full((T, F, N, 2, 2), -128, np.int8)
+    got = run_i8(x)
+    assert (got[..., 0] == 2 * 128 * 128 * T).all() and (got[..., 1] == 0).all()
+
+
+def test_forced_staging_and_unaligned_pointer():
+    N, F, T = 64, 3, 150
+    x = wl.full_range(N, F, T, seed=5)
+    ref = xo.correlate_i8(x)
+    assert np.array_equal(run_i8(x, force_stage=True), ref)
+    # input pointer off by 4 bytes: not 16-byte aligned -> S0 staging path is taken by the library itself
+    p = xcb.Plan(N, F, T)
+    buf = torch.zeros(x.size + 64, dtype=torch.int8, device="cuda")
+    xs = buf[4:4 + x.size].view(T, F, N, 2, 2)
+    assert xs.data_ptr() % 16 == 4
+    xs.copy_(torch.from_numpy(x))
+    ws = torch.empty(p.workspace_bytes, dtype=torch.int8, device="cuda")
+    p.set_workspace(ws)
+    vis = p.correlate(xs)
+    assert p.last_launches == 2
+    torch.cuda.synchronize()
+    assert np.array_equal(vis.cpu().numpy(), ref)
+
+
+def test_persistent_schedule_independent_of_cta_count():
+    N, F, T = 100, 5, 200
+    x = wl.gaussian(N, F, T, seed=11, sigma=30.0)
+    ref = xo.correlate_i8(x)
+    for ctas in (1, 2, 7, 0):
+        assert np.array_equal(run_i8(x, max_ctas=ctas), ref)
+
+
+def test_accumulate_is_linear_in_time():
+    """I = N_p * I': three blocks accumulated == one long integration, exactly."""
+    N, F, T = 48, 4, 96
+    blocks = [wl.gaussian(N, F, T, seed=20 + k, sigma=20.0) for k in range(3)]
+    ref = xo.correlate_i8(np.concatenate(blocks, axis=0))
+    p = xcb.Plan(N, F, T)
+    vis = p.correlate(torch.from_numpy(blocks[0]).cuda())
+    for b in blocks[1:]:
+        p.correlate_acc(torch.from_numpy(b).cuda(), vis)
+    torch.cuda.synchronize()
+    assert np.array_equal(vis.cpu().numpy(), ref)
+
+
+def test_common_tone_phases_on_gpu():
+    """Rank-1 input: V_ij = T A^2 w_i conj(w_j) (fixes which factor is conjugated, reading 1)."""
+    N, F, T, A = 40, 2, 64, 3
+    x, wq = wl.common_tone(N, F, T, seed=3, A=A)
+    got = run_i8(x)
+    w = np.exp(1j * np.pi / 2 * wq)                          # [f][s][p]
+    for f in range(F):
+        for (i, j) in [(0, 0), (0, 1), (3, 17), (39, 39), (12, 38)]:
+            b = j * (j + 1) // 2 + i
+            v = got[f, b, ..., 0] + 1j * got[f, b, ..., 1]
+            exp = T * A * A * w[f, i][:, None] * np.conj(w[f, j])[None, :]
+            assert np.allclose(v, exp)
+
+
+# ---------------------------------------------------------------------------------------------
+# two-stream pipeline (Algorithm 1) and the host end-to-end call
+# ---------------------------------------------------------------------------------------------
+
+def test_pipelined_matches_long_integration():
+    N, F, T, nblk = 64, 8, 128, 5
+    w = wl.Workload("pipe", N, F, T, "gauss", 8.0, 0)
+    blocks = wl.make_blocks(w, nblk)
+    ref = xo.correlate_i8(np.concatenate(blocks, axis=0))
+    p = xcb.Plan(N, F, T)
+    host = torch.from_numpy(np.stack(blocks)).pin_memory()
+    dev2 = torch.empty(2 * p.in_bytes, dtype=torch.int8, device="cuda")
+    vis = torch.full(p.vis_shape(), -1, dtype=torch.int32, device="cuda")
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    p.correlate_pipelined(host, dev2, vis, s1, s2)
+    s1.synchronize()
+    assert p.last_launches == nblk
+    assert np.array_equal(vis.cpu().numpy(), ref)
+    # again into the same buffers: entry ordering against earlier work on the compute stream
+    p.correlate_pipelined(host, dev2, vis, s1, s2)
+    s1.synchronize()
+    assert np.array_equal(vis.cpu().numpy(), ref)
+
+
+def test_host_end_to_end_call():
+    w = wl.CONFIGS["cfg1"]
+    x = wl.make_input(w)
+    p = xcb.Plan(w.N, w.F, w.T)
+    xh = torch.from_numpy(x).pin_memory()
+    vh = torch.empty(p.vis_shape(), dtype=torch.int32).pin_memory()
+    xd = torch.empty(p.in_shape(), dtype=torch.int8, device="cuda")
+    vd = p.new_vis()
+    p.correlate_host(xh, vh, xd, vd)
+    assert np.array_equal(vh.numpy(), xo.correlate_i8(x))
+
+
+# ---------------------------------------------------------------------------------------------
+# fp32 path
+# ---------------------------------------------------------------------------------------------
+
+def f32_tolerance_check(got, ref64, N):
+    """|V - V64| <= 1e-5 sqrt(V64[(i,pi),(i,pi)] V64[(j,pj),(j,pj)]) per complex entry."""
+    F = ref64.shape[0]
+    diag = np.array([j * (j + 1) // 2 + j for j in range(N)])
+    auto = np.stack([ref64[:, diag, 0, 0, 0], ref64[:, diag, 1, 1, 0]], axis=-1)     # [f][s][p]
+    jj, ii = np.array([(j, i) for j in range(N) for i in range(j + 1)]).T
+    norm = np.sqrt(auto[:, ii][:, :, :, None] * auto[:, jj][:, :, None, :])           # [f][b][pi][pj]
+    err = np.abs((got[..., 0] - ref64[..., 0]) + 1j * (got[..., 1] - ref64[..., 1]))
+    ratio = err / np.maximum(norm, 1e-30)
+    assert ratio.max() <= 1e-5, ratio.max()
+    return ratio.max()
+
+
+@pytest.mark.parametrize("N,F,T", [(1, 1, 1), (3, 2, 17), (33, 2, 100), (64, 3, 257), (100, 2, 130), (130, 1, 1000)])
+def test_f32_against_fp64_oracle(N, F, T):
+    rng = np.random.default_rng(N + T)
+    x = rng.standard_normal((T, F, N, 2, 2)).astype(np.float32) * 4.0
+    p = xcb.Plan(N, F, T)
+    vis = torch.full(p.vis_shape(), float("nan"), dtype=torch.float32, device="cuda")
+    p.correlate_f32(torch.from_numpy(x).cuda(), vis)
+    torch.cuda.synchronize()
+    got = vis.cpu().numpy().astype(np.float64)
+    assert np.isfinite(got).all()
+    f32_tolerance_check(got, xo.channels_f64(x), N)
+
+
+def test_f32_equals_int8_for_integer_input():
+    """Config 3's values as float: all products and sums are exact in fp32 -> identical results."""
+    w = wl.Workload("cfg3small", 256, 4, 1000, "gauss_tone", 4.0, 1003)
+    x = wl.make_input(w)
+    p = xcb.Plan(w.N, w.F, w.T)
+    xd = torch.from_numpy(x).cuda()
+    vi = p.correlate(xd)
+    vf = p.correlate_f32(xd.to(torch.float32))
+    torch.cuda.synchronize()
+    ref = xo.correlate_i8(x)
+    assert np.array_equal(vi.cpu().numpy(), ref)
+    assert np.array_equal(vf.cpu().numpy(), ref.astype(np.float32))
+    # accumulate flag
+    p.correlate_f32(xd.to(torch.float32), vf, accumulate=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(vf.cpu().numpy(), 2 * ref.astype(np.float32))
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes, in the launch configuration bench.py times
+# ---------------------------------------------------------------------------------------------
+
+FULL = ["cfg2", "cfg3", "cfg4", "cfg5_N32", "cfg5_N64", "cfg5_N100", "cfg5_N500", "cfg5_N1024"]
+
+
+@pytest.mark.parametrize("name", FULL)
+def test_full_size_configs(name):
+    w = wl.CONFIGS[name]
+    x = wl.make_input(w)
+    p = xcb.Plan(w.N, w.F, w.T)
+    xd = torch.from_numpy(x).cuda()
+    vis = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+    p.correlate(xd, vis)
+    torch.cuda.synchronize()
+    # (a) oracle on sampled channels, all baselines
+    nsel = 2 if w.N >= 1000 else (3 if w.N >= 500 else 4)
+    rng = np.random.default_rng(w.seed)
+    fsel = sorted({0, w.F - 1, *rng.integers(0, w.F, size=nsel - 2).tolist()})
+    ref = xo.channels_i8(x, fsel)
+    got = vis[torch.tensor(fsel, device="cuda")].cpu().numpy()
+    assert np.array_equal(got, ref), name
+    # (b) every output against an exact fp64 matmul (independent of the kernels)
+    gram_check_fp64(xd, vis, f_chunk=max(1, 2048 // w.N))
+    # (c) invariants that hold at any size: autocorrelations real, same-station cross-pols conjugate
+    diag = torch.tensor([j * (j + 1) // 2 + j for j in range(w.N)], device="cuda")
+    a = vis[:, diag]
+    assert (a[:, :, 0, 0, 1] == 0).all() and (a[:, :, 1, 1, 1] == 0).all()
+    assert torch.equal(a[:, :, 0, 1, 0], a[:, :, 1, 0, 0]) and torch.equal(a[:, :, 0, 1, 1], -a[:, :, 1, 0, 1])
+    if name == "cfg3":
+        # the same values through the fp32 path (BASELINE.json configs[2]): exact for these magnitudes
+        vf = p.correlate_f32(xd.to(torch.float32))
+        torch.cuda.synchronize()
+        assert torch.equal(vf, vis.to(torch.float32))
+
+
+def test_cfg5_two_stream_eight_blocks():
+    """Config 5's pipelined run: 8 host blocks accumulated (total integration 16384 samples)."""
+    w = wl.CONFIGS["cfg5_N100"]
+    blocks = wl.make_blocks(w, 8)
+    p = xcb.Plan(w.N, w.F, w.T)
+    host = torch.from_numpy(np.stack(blocks)).pin_memory()
+    dev2 = torch.empty(2 * p.in_bytes, dtype=torch.int8, device="cuda")
+    vis = p.new_vis()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    p.correlate_pipelined(host, dev2, vis, s1, s2)
+    s1.synchronize()
+    fsel = [0, 31, 63]
+    ref = xo.channels_i8(np.concatenate(blocks, axis=0), fsel)
+    assert np.array_equal(vis[torch.tensor(fsel, device="cuda")].cpu().numpy(), ref)
