@@ -45,48 +45,58 @@ def load_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons sampled through NVML (pynvml) every ~1 ms by a thread, DURING the
+    timed region (the recipe's clocks line, without nvidia-smi's start-up latency)."""
+    REASONS = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
 
     def __init__(self, index: int):
-        self.rows, self.proc = [], None
+        self.rows, self.ok, self._stop = [], False, False
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.thr = threading.Thread(target=self._read, daemon=True)
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and vis.split(",")[index].isdigit() else index
+            self.nv, self.h = pynvml, pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_sm = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+            self.thr = threading.Thread(target=self._run, daemon=True)
             self.thr.start()
-        except OSError:
-            self.proc = None
+        except Exception as e:  # noqa: BLE001 -- report, never fail the bench for a missing NVML
+            self.err = repr(e)
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append((time.perf_counter(), line.strip()))
+    def _run(self):
+        nv, h = self.nv, self.h
+        while not self._stop:
+            try:
+                sm = nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)
+                try:
+                    rs = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                except AttributeError:
+                    rs = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                pw = nv.nvmlDeviceGetPowerUsage(h) / 1000.0
+                self.rows.append((time.perf_counter(), float(sm), int(rs), pw))
+            except Exception:  # noqa: BLE001
+                pass
+            time.sleep(0.001)
 
     def window(self, t0, t1):
-        sm, mx, reasons = [], 0.0, set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ts, line in self.rows:
-            if ts < t0 - 0.05 or ts > t1 + 0.15:
-                continue
-            tok = [t.strip() for t in line.split(",")]
-            try:
-                sm.append(float(tok[0]))
-                mx = max(mx, float(tok[1]))
-            except (ValueError, IndexError):
-                continue
-            for n, v in zip(names, tok[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(n)
-        sm.sort()
-        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx or None, "samples": len(sm),
-                "reasons": sorted(reasons)}
+        if not self.ok:
+            return {"sm_mhz": None, "sm_max_mhz": None, "samples": 0, "reasons": [], "error": getattr(self, "err", "")}
+        rows = [r for r in self.rows if t0 <= r[0] <= t1]
+        where = "timed region"
+        if not rows:  # region shorter than one sampling period: take the samples right after it
+            rows = [r for r in self.rows if t1 < r[0] <= t1 + 0.02][:3]
+            where = "first samples after the timed region (region shorter than the sampling period)"
+        sm = sorted(r[1] for r in rows)
+        bits = 0
+        for r in rows:
+            bits |= r[2]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": self.max_sm, "samples": len(sm),
+                "power_w_max": max((r[3] for r in rows), default=None),
+                "reasons": sorted(n for n, b in self.REASONS.items() if bits & b), "window": where}
 
     def stop(self):
-        if self.proc:
-            self.proc.terminate()
+        self._stop = True
 
 
 def workload_desc(w):
@@ -163,7 +173,7 @@ def time_kernel(p, xd, vis, stream, steps, warmup):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
@@ -239,7 +249,7 @@ def main():
     tops = world * w.ops / (ms_step * 1e-3) / 1e12
 
     # ---- per-launch duration of the dominant kernel (events around each launch) -------------
-    per = time_kernel(p, xd, vis, stream, args.steps, 1)
+    per = time_kernel(p, xd, vis, stream, min(args.steps, 50), 1)
     k_ms = sum(per) / len(per)
     alg_bytes = w.in_bytes + w.vis_bytes                      # input once + output once
     i8_peak = peaks["bf16_burst"] * NOMINAL_I8_OVER_BF16      # Tops/s: measured bf16 x nominal int8/bf16 ratio

@@ -70,10 +70,20 @@ enum {
     XC_I8_KERNEL_SIMT = 2  /* plain CUDA-core kernel, one thread per baseline: a debugging    */
                            /* aid that shares no device code with the tensor-core kernel     */
 };
+/* Tensor-core tile shapes (Gram rows x Gram columns; 4 Gram rows = 1 station), xc_set_option(XC_OPT_TILE, ...). */
+enum {
+    XC_TILE_AUTO = 0,         /* chosen from N at plan time                                        */
+    XC_TILE_1CTA_128x128 = 1, /* 32 x 32 stations on one CTA (small N)                             */
+    XC_TILE_1CTA_128x256 = 2, /* 32 x 64 stations on one CTA                                       */
+    XC_TILE_2CTA_256x256 = 3  /* 64 x 64 stations on a CTA pair (tcgen05 cta_group::2)             */
+};
 typedef enum {
     XC_OPT_I8_KERNEL = 0, /* one of XC_I8_KERNEL_*                                            */
     XC_OPT_MAX_CTAS = 1,  /* cap on persistent CTAs of the tensor-core kernel (0 = SM count)  */
-    XC_OPT_FORCE_STAGE = 2 /* 1 = always run the staging (pad/copy) kernel, for testing S0     */
+    XC_OPT_FORCE_STAGE = 2, /* 1 = always run the staging (pad/copy) kernel, for testing S0    */
+    XC_OPT_TILE = 4,       /* one of XC_TILE_*; rebuilds the tile schedule (synchronising on next call) */
+    XC_OPT_DEBUG_SKIP = 3  /* PROFILING ONLY, results become meaningless: bit 0 = no TMA loads  */
+                           /* after the first ring fill, bit 1 = no MMAs, bit 2 = no stores     */
 } xc_option;
 
 /* xc_plan -- north_star's xc_plan(N, P=2, F, T, layout).
@@ -108,7 +118,7 @@ int xc_set_option(xc_plan_t* plan, int option, int value);
 
 /* xc_correlate -- vis = X-engine(in)  (Eq. 4).  Overwrites all F*NB*8 int32 of vis_dev; old
  *   contents are not read.  in_dev: int8 [T][F][N][2][2]; vis_dev: int32 [F][NB][2][2][2],
- *   4-byte aligned at least (32-byte alignment gives full-sector stores).  Exact for the whole
+ *   16-byte aligned (32-byte alignment gives full-sector stores).  Exact for the whole
  *   int8 range including -128.  Bit-exact to the definition; independent of tile schedule.
  * xc_correlate_acc -- vis += X-engine(in)  ("matrix_d <- X-engine(matrix_d, buffer_d)",
  *   PAPER.md:244; I = N_p * I').  int32 two's-complement addition. */
@@ -141,6 +151,11 @@ int xc_correlate_pipelined(xc_plan_t* plan, const int8_t* in_host_pinned, int n_
  *   in_dev_scratch / vis_dev_scratch are caller-owned device buffers of the plan's sizes. */
 int xc_correlate_host(xc_plan_t* plan, const int8_t* in_host, int32_t* vis_host, int8_t* in_dev_scratch,
                       int32_t* vis_dev_scratch, void* cuda_stream);
+
+/* PROFILING ONLY: trace_dev = device buffer of 3*256*4 int64 (or NULL to switch off); CTA 0 of the
+ * tensor-core kernel writes clock64() stamps of its first 256 pipeline iterations per warp role
+ * (0 = TMA producer, 1 = MMA issuer, 2 = epilogue) into it. */
+int xc_debug_set_trace(xc_plan_t* plan, void* trace_dev);
 
 /* Tile schedule introspection (for tests of the triangular map).
  *   xc_tile_count: number of scheduled tiles per channel for the integer path.

@@ -13,14 +13,15 @@ LIB_PATH = os.path.join(HERE, "libxc.so")
 
 MAX_T = 65535
 I8_KERNEL_AUTO, I8_KERNEL_TC, I8_KERNEL_SIMT = 0, 1, 2
-OPT_I8_KERNEL, OPT_MAX_CTAS, OPT_FORCE_STAGE = 0, 1, 2
+OPT_I8_KERNEL, OPT_MAX_CTAS, OPT_FORCE_STAGE, OPT_DEBUG_SKIP, OPT_TILE = 0, 1, 2, 3, 4
+TILE_AUTO, TILE_1CTA_128x128, TILE_1CTA_128x256, TILE_2CTA_256x256 = 0, 1, 2, 3
 
 # every symbol include/xc.h declares
 EXPORTED_SYMBOLS = (
     "xc_plan", "xc_destroy", "xc_in_bytes", "xc_in_bytes_f32", "xc_vis_bytes", "xc_n_baselines",
     "xc_workspace_bytes", "xc_set_workspace", "xc_set_option", "xc_correlate", "xc_correlate_acc",
     "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_tile_count", "xc_tile_get",
-    "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error",
+    "xc_debug_set_trace", "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error",
     "xc_version",
 )
 
@@ -57,6 +58,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_correlate_f32": (i, [p, p, p, i, p]),
         "xc_correlate_pipelined": (i, [p, p, i, p, p, p, p]),
         "xc_correlate_host": (i, [p, p, p, p, p, p]),
+        "xc_debug_set_trace": (i, [p, p]),
         "xc_tile_count": (i, [p]),
         "xc_tile_get": (i, [p, i, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i)]),
         "xc_tri_index": (i64, [i64, i64]),

@@ -45,10 +45,10 @@ struct xc_plan_s {
     int N = 0, P = 0, F = 0, T = 0;
     long long NB = 0;
     int Npad = 0;
-    int umma_n = 256;
+    int tile_mode = 0;  // XC_TILE_*: shape of the tensor-core tile actually in use
     std::vector<uint32_t> tiles_tc, tiles_f32;
     // device state (created lazily on the device current at first compute call)
-    bool dev_ready = false;
+    bool dev_ready = false, tiles_uploaded = false;
     int device = -1, sm_count = 0;
     uint32_t* d_tiles_tc = nullptr;
     uint32_t* d_tiles_f32 = nullptr;
@@ -56,7 +56,8 @@ struct xc_plan_s {
     void* ws = nullptr;
     size_t ws_bytes = 0;
     bool ws_owned = false;
-    int opt_kernel = XC_I8_KERNEL_AUTO, opt_max_ctas = 0, opt_force_stage = 0;
+    int opt_kernel = XC_I8_KERNEL_AUTO, opt_max_ctas = 0, opt_force_stage = 0, opt_debug_skip = 0;
+    long long* trace = nullptr;
     CUtensorMap tmap;
     const void* tmap_src = nullptr;
     int tmap_nrow = 0;
@@ -78,6 +79,64 @@ int cuda_fail(xc_plan_t* p, cudaError_t e, const char* where) {
         if (e__ != cudaSuccess) return cuda_fail((p), e__, #call);    \
     } while (0)
 
+void tile_shape(int mode, int* si, int* sj) {
+    *si = (mode == XC_TILE_2CTA_256x256) ? 64 : 32;
+    *sj = (mode == XC_TILE_1CTA_128x128) ? 32 : 64;
+}
+
+// S1: pick the tensor-core tile and build its per-channel schedule.
+void set_tile_mode(xc_plan_t* p, int mode) {
+    if (mode == XC_TILE_AUTO) {
+        // CTA-pair 256x256 tiles halve the shared-memory traffic per MMA and are the default; the
+        // narrow single-CTA tile only wins when it wastes clearly less of the tensor pipe on the
+        // diagonal (small N).
+        const double a2 = 65536.0 * build_tiles(p->N, 64, 64).size();
+        const double a1 = 16384.0 * build_tiles(p->N, 32, 32).size();
+        mode = (a1 < 0.6 * a2) ? XC_TILE_1CTA_128x128 : XC_TILE_2CTA_256x256;
+    }
+    int si, sj;
+    tile_shape(mode, &si, &sj);
+    p->tile_mode = mode;
+    p->tiles_tc = build_tiles(p->N, si, sj);
+    p->tiles_uploaded = false;
+}
+
+int upload_tiles(xc_plan_t* p) {
+    if (p->tiles_uploaded) return XC_OK;
+    if (p->d_tiles_tc) XC_CUDA(p, cudaFree(p->d_tiles_tc));   // synchronising; only after xc_set_option(XC_OPT_TILE)
+    p->d_tiles_tc = nullptr;
+    XC_CUDA(p, cudaMalloc(&p->d_tiles_tc, p->tiles_tc.size() * sizeof(uint32_t)));
+    XC_CUDA(p, cudaMemcpy(p->d_tiles_tc, p->tiles_tc.data(), p->tiles_tc.size() * sizeof(uint32_t),
+                          cudaMemcpyHostToDevice));
+    p->tiles_uploaded = true;
+    return XC_OK;
+}
+
+template <int UMMA_N, int CG>
+int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
+    long long units = (p->opt_max_ctas > 0 ? p->opt_max_ctas : p->sm_count) / CG;
+    if (units < 1) units = 1;
+    if (units > tp.total_tiles) units = tp.total_tiles;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(units * CG));
+    cfg.blockDim = dim3(xc::TC_THREADS);
+    cfg.dynamicSmemBytes = xc::TcCfg<UMMA_N, CG>::SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CG;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (CG == 2 && UMMA_N == 256 && tp.trace) {
+        XC_CUDA(p, cudaLaunchKernelEx(&cfg, xc::xc_i8_tc_kernel<256, 2, true>, p->tmap, tp));
+    } else {
+        XC_CUDA(p, cudaLaunchKernelEx(&cfg, xc::xc_i8_tc_kernel<UMMA_N, CG, false>, p->tmap, tp));
+    }
+    return XC_OK;
+}
+
 int ensure_device(xc_plan_t* p) {
     if (p->dev_ready) return XC_OK;
     int dev = 0;
@@ -94,6 +153,7 @@ int ensure_device(xc_plan_t* p) {
     XC_CUDA(p, cudaMalloc(&p->d_tiles_tc, p->tiles_tc.size() * sizeof(uint32_t)));
     XC_CUDA(p, cudaMemcpy(p->d_tiles_tc, p->tiles_tc.data(), p->tiles_tc.size() * sizeof(uint32_t),
                           cudaMemcpyHostToDevice));
+    p->tiles_uploaded = true;
     XC_CUDA(p, cudaMalloc(&p->d_tiles_f32, p->tiles_f32.size() * sizeof(uint32_t)));
     XC_CUDA(p, cudaMemcpy(p->d_tiles_f32, p->tiles_f32.data(), p->tiles_f32.size() * sizeof(uint32_t),
                           cudaMemcpyHostToDevice));
@@ -105,10 +165,14 @@ int ensure_device(xc_plan_t* p) {
         return XC_ERR_CUDA;
     }
     p->encode = reinterpret_cast<PFN_encodeTiled>(fn);
-    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    xc::TcCfg<256>::SMEM_BYTES));
-    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    xc::TcCfg<128>::SMEM_BYTES));
+    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_kernel<128, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    xc::TcCfg<128, 1>::SMEM_BYTES));
+    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_kernel<256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    xc::TcCfg<256, 1>::SMEM_BYTES));
+    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_kernel<256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    xc::TcCfg<256, 2>::SMEM_BYTES));
+    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_kernel<256, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    xc::TcCfg<256, 2>::SMEM_BYTES));
     XC_CUDA(p, cudaFuncSetAttribute(xc::xc_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     xc::F32_SMEM_BYTES));
     p->dev_ready = true;
@@ -168,7 +232,7 @@ int encode_tmap(xc_plan_t* p, const void* src, int nrow) {
 
 int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* stream, int accumulate) {
     if (!p || !in_dev || !vis_dev) return XC_ERR_INVALID_ARG;
-    if (reinterpret_cast<uintptr_t>(vis_dev) & 7u) return XC_ERR_ALIGNMENT;
+    if (reinterpret_cast<uintptr_t>(vis_dev) & 15u) return XC_ERR_ALIGNMENT;
     int rc = ensure_device(p);
     if (rc != XC_OK) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -192,24 +256,25 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     rc = encode_tmap(p, src, nrow);
     if (rc != XC_OK) return rc;
 
+    rc = upload_tiles(p);
+    if (rc != XC_OK) return rc;
     xc::TcParams tp;
     tp.N = p->N;
     tp.F = p->F;
     tp.T = p->T;
     tp.tiles_per_f = static_cast<int>(p->tiles_tc.size());
-    tp.total_tiles = static_cast<long long>(p->F) * tp.tiles_per_f;
+    if (static_cast<long long>(p->F) * tp.tiles_per_f > 0x7FFFFFFFLL) return XC_ERR_UNSUPPORTED;
+    tp.total_tiles = p->F * tp.tiles_per_f;
     tp.NB = p->NB;
     tp.tiles = p->d_tiles_tc;
     tp.vis = vis_dev;
     tp.accumulate = accumulate;
-    long long ctas = p->opt_max_ctas > 0 ? p->opt_max_ctas : p->sm_count;
-    if (ctas > tp.total_tiles) ctas = tp.total_tiles;
-    if (p->umma_n == 256) {
-        xc::xc_i8_tc_kernel<256><<<static_cast<unsigned>(ctas), xc::TC_THREADS, xc::TcCfg<256>::SMEM_BYTES, st>>>(p->tmap, tp);
-    } else {
-        xc::xc_i8_tc_kernel<128><<<static_cast<unsigned>(ctas), xc::TC_THREADS, xc::TcCfg<128>::SMEM_BYTES, st>>>(p->tmap, tp);
-    }
-    XC_CUDA(p, cudaGetLastError());
+    tp.debug_skip = p->opt_debug_skip;
+    tp.trace = p->trace;
+    if (p->tile_mode == XC_TILE_2CTA_256x256) rc = launch_tc<256, 2>(p, tp, st);
+    else if (p->tile_mode == XC_TILE_1CTA_128x256) rc = launch_tc<256, 1>(p, tp, st);
+    else rc = launch_tc<128, 1>(p, tp, st);
+    if (rc != XC_OK) return rc;
     p->last_launches += 1;
     return XC_OK;
 }
@@ -233,17 +298,7 @@ int xc_plan(xc_plan_t** out, int N, int P, int F, int T, int layout) {
     p->T = T;
     p->NB = static_cast<long long>(N) * (N + 1) / 2;
     p->Npad = (N + 3) & ~3;
-    // Tile width on the j side: 64 stations (UMMA_N = 256) unless the narrower 32-station tile
-    // wastes clearly less of the tensor pipe on the diagonal (small N).
-    const std::vector<uint32_t> t256 = build_tiles(N, 32, 64), t128 = build_tiles(N, 32, 32);
-    const double area256 = 256.0 * t256.size(), area128 = 128.0 * t128.size();
-    if (area128 < 0.8 * area256) {
-        p->umma_n = 128;
-        p->tiles_tc = t128;
-    } else {
-        p->umma_n = 256;
-        p->tiles_tc = t256;
-    }
+    set_tile_mode(p, XC_TILE_AUTO);
     p->tiles_f32 = build_tiles(N, xc::F32_SI, xc::F32_SJ);
     memset(&p->tmap, 0, sizeof p->tmap);
     *out = p;
@@ -294,6 +349,13 @@ int xc_set_option(xc_plan_t* p, int option, int value) {
             return XC_OK;
         case XC_OPT_FORCE_STAGE:
             p->opt_force_stage = value ? 1 : 0;
+            return XC_OK;
+        case XC_OPT_TILE:
+            if (value < XC_TILE_AUTO || value > XC_TILE_2CTA_256x256) return XC_ERR_INVALID_ARG;
+            set_tile_mode(p, value);
+            return XC_OK;
+        case XC_OPT_DEBUG_SKIP:
+            p->opt_debug_skip = value & 7;
             return XC_OK;
         default:
             return XC_ERR_INVALID_ARG;
@@ -383,14 +445,22 @@ int xc_correlate_host(xc_plan_t* p, const int8_t* in_host, int32_t* vis_host, in
     return XC_OK;
 }
 
+int xc_debug_set_trace(xc_plan_t* p, void* trace_dev) {
+    if (!p) return XC_ERR_INVALID_ARG;
+    p->trace = static_cast<long long*>(trace_dev);
+    return XC_OK;
+}
+
 int xc_tile_count(const xc_plan_t* p) { return p ? static_cast<int>(p->tiles_tc.size()) : 0; }
 
 int xc_tile_get(const xc_plan_t* p, int k, int* bi, int* bj, int* si, int* sj) {
     if (!p || k < 0 || k >= static_cast<int>(p->tiles_tc.size())) return XC_ERR_INVALID_ARG;
     if (bi) *bi = static_cast<int>(p->tiles_tc[k] & 0xFFFFu);
     if (bj) *bj = static_cast<int>(p->tiles_tc[k] >> 16);
-    if (si) *si = 32;
-    if (sj) *sj = p->umma_n / 4;
+    int a, b;
+    tile_shape(p->tile_mode, &a, &b);
+    if (si) *si = a;
+    if (sj) *sj = b;
     return XC_OK;
 }
 

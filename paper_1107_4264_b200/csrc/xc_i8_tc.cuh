@@ -11,219 +11,296 @@
 // level, outer levels hold input vectors) maps to: TMEM accumulator tile (innermost) <- smem
 // operand ring filled by TMA <- L2 (a channel's input, <= 8 MB, is shared by all its tiles).
 // The triangular thread-block map becomes a per-channel tile table walked by
-// persistent CTAs; only tiles that intersect i <= j are scheduled.
+// persistent CTAs (or CTA pairs); only tiles that intersect i <= j are scheduled.
 //
-// One CTA = 6 warps: warp 0 TMA producer, warp 1 MMA issuer (+ TMEM owner), warps 2-5 epilogue.
-// Tile = 128 Gram rows (32 stations, i side) x UMMA_N Gram columns (UMMA_N/4 stations, j side).
+// One CTA = 10 warps: warp 0 TMA producer, warp 1 MMA issuer (+ TMEM owner), warps 2-9 epilogue.
+// CG = 1: tile = 128 Gram rows (32 stations, i side) x UMMA_N Gram columns, one CTA.
+// CG = 2: tile = 256 Gram rows (64 stations) x 256 columns (64 stations) on a CTA pair
+//         (tcgen05 cta_group::2): each CTA holds its own 128 A rows and half of B, so every
+//         operand byte is fetched from L2 and written to shared memory once per pair.
 // K (= time) advances BK samples per ring stage, 32 per tcgen05.mma.  Time is the slowest input
 // index, so both operands are MN-major in shared memory: a TMA box
 // [BK t][1 f][128 B of m] lands as BK rows of 128 bytes, which is exactly the SWIZZLE_128B
 // MN-major canonical layout (8-row atoms of 1024 B).  Two TMEM accumulators (2 x UMMA_N columns)
-// let the epilogue of tile k overlap the MMAs of tile k+1.
+// let the epilogue of tile k overlap the MMAs of tile k+1.  On tiles that touch the diagonal the
+// A rows are a sub-block of the B rows: they are loaded once and both descriptors point at them.
+//
+// Producer and MMA loops run warp-uniformly (all 32 lanes walk the loop, one elected lane issues)
+// so that addresses, coordinates and descriptors stay in uniform registers: a single-lane branch
+// costs ~80 cycles per TMA / MMA issue in register->uniform-register waterfalls, which at 128
+// tensor cycles per MMA starves the pipe (measured).
 #pragma once
 #include "xc_ptx.cuh"
 
 namespace xc {
 
-constexpr int TC_BK = 64;          // samples per pipeline stage
+constexpr int TC_BK = 128;         // samples per pipeline stage
 constexpr int TC_UMMA_K = 32;      // samples per tcgen05.mma (kind::i8)
-constexpr int TC_M = 128;          // Gram rows per tile = 32 stations
-constexpr int TC_THREADS = 192;    // 6 warps
+constexpr int TC_EPI_WARPS = 8;     // 2 per TMEM lane quarter, each owning half of the tile's columns
+constexpr int TC_THREADS = 64 + 32 * TC_EPI_WARPS;   // + TMA producer warp + MMA issuer warp
 constexpr int TC_SMEM_LIMIT = 232448;  // 227 KB
+constexpr int TC_BOX_BYTES = TC_BK * 128;   // one TMA box: BK rows of 128 bytes
 
-template <int UMMA_N>
+template <int UMMA_N, int CG>
 struct TcCfg {
-    static constexpr int A_BYTES = TC_BK * 128;
-    static constexpr int B_BYTES = TC_BK * UMMA_N;
+    static constexpr int M = 128 * CG;                    // Gram rows per tile
+    static constexpr int B_BOXES = UMMA_N / 128 / CG;     // 128-row B boxes held by one CTA
+    static constexpr int A_BYTES = TC_BOX_BYTES;
+    static constexpr int B_BYTES = B_BOXES * TC_BOX_BYTES;
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-    static constexpr int STAGES = (UMMA_N == 256) ? 8 : 12;
-    static constexpr int BAR_BYTES = 1024;  // barriers + tmem slot, kept in the first KB
+    static constexpr int STAGES = 196608 / STAGE_BYTES;   // 4 x 48 KB or 6 x 32 KB
+    static constexpr int BAR_BYTES = 1024;                // barriers + tmem slot, kept in the first KB
     static constexpr int SMEM_BYTES = BAR_BYTES + STAGES * STAGE_BYTES + 1024;  // + slack for 1024-B alignment
-    static constexpr int SJ = UMMA_N / 4;   // stations per tile on the j side
+    static constexpr int SI = 32 * CG;                    // stations per tile on the i side
+    static constexpr int SJ = UMMA_N / 4;                 // stations per tile on the j side
+    static_assert(B_BOXES >= 1, "a CTA holds at least one 128-row B box");
     static_assert(SMEM_BYTES <= TC_SMEM_LIMIT, "smem");
 };
 
 struct TcParams {
     int N, F, T;
     int tiles_per_f;          // entries of `tiles` per channel
-    long long total_tiles;    // F * tiles_per_f
+    int total_tiles;          // F * tiles_per_f
     long long NB;             // N(N+1)/2
-    const uint32_t* tiles;    // device: bi | (bj << 16)
+    const uint32_t* tiles;    // device: bi | (bj << 16), in units of (SI, SJ) stations
     int32_t* vis;
     int accumulate;
+    int debug_skip;           // profiling only (XC_OPT_DEBUG_SKIP): 1 = no TMA after the first ring fill,
+                              // 2 = no MMA, 4 = no global stores; results are then meaningless
+    long long* trace;         // profiling only: CTA 0 writes clock64() stamps here (see TC_TRACE_*), or null
 };
+constexpr int TC_TRACE_ITERS = 256;   // k-blocks traced; layout: [3 roles][TC_TRACE_ITERS][4] long long
 
 // Epilogue for one 32-column chunk (8 stations j) held in v[]: complex combine, mask, store.
-// Thread <-> Gram row r = (i, pi, ci): lanes 4s..4s+3 of a warp are one station i.
-//   ci = 0 holds G[(i,pi,re), (j,pj,cj)], ci = 1 holds G[(i,pi,im), (j,pj,cj)]; the pair swaps
-//   two values so that lane ci=0 ends with (Re,Im) of [pi][pj=0] and lane ci=1 with [pi][pj=1]:
-//   every lane then stores 8 contiguous bytes and four lanes one 32-byte record.
-template <bool MASKED, bool ACC>
+// Thread <-> Gram row r = (i, pi, ci): lanes 4s..4s+3 of a warp are one station i; ci = 0 holds
+// G[(i,pi,re), (j,pj,cj)] and ci = 1 holds G[(i,pi,im), (j,pj,cj)] for the chunk's columns (j,pj,cj).
+// Stations j are taken two at a time: the ci = 0 lane finishes the even one, the ci = 1 lane the odd
+// one, after swapping the four values the other needs (4 shuffles per station pair).  Each lane then
+// owns [pi][pj=0,1][re,im] of its (i, j) = 16 contiguous bytes, two lanes one 32-byte record, and a
+// warp store instruction writes two 256-byte runs (8 consecutive i for each of the two j).
+template <bool MASKED, bool ACC, bool NOSTORE = false>
 __device__ __forceinline__ void epi_chunk(const uint32_t (&v)[32], int32_t* __restrict__ visf, int i, int jbase, int N,
                                           int lane) {
     const int ci = lane & 1;
-    const int slot = (lane & 3) * 2;  // int32 offset inside the 8-int record: pi*4 + pj*2, pj := ci
+    const int slot = ((lane >> 1) & 1) * 4;  // int32 offset of [pi] inside the 8-int record
 #pragma unroll
-    for (int js = 0; js < 8; ++js) {
-        const int a0 = static_cast<int>(v[4 * js + 0]);  // column (j, pj=0, re)
-        const int a1 = static_cast<int>(v[4 * js + 1]);  // column (j, pj=0, im)
-        const int a2 = static_cast<int>(v[4 * js + 2]);  // column (j, pj=1, re)
-        const int a3 = static_cast<int>(v[4 * js + 3]);  // column (j, pj=1, im)
-        const int sx = ci ? a0 : a2;
-        const int sy = ci ? a1 : a3;
-        const int rx = __shfl_xor_sync(0xffffffffu, sx, 1);
-        const int ry = __shfl_xor_sync(0xffffffffu, sy, 1);
-        // ci=0: Re = G[re,re] + G[im,im] = a0 + ry ; Im = G[im,re] - G[re,im] = rx - a1   (pj = 0)
-        // ci=1: Re = G[re,re] + G[im,im] = rx + a3 ; Im = G[im,re] - G[re,im] = a2 - ry   (pj = 1)
-        int re = ci ? (rx + a3) : (a0 + ry);
-        int im = ci ? (a2 - ry) : (rx - a1);
-        const int j = jbase + js;
-        if (!MASKED || (i <= j && j < N)) {
-            int2* dst = reinterpret_cast<int2*>(visf + ((static_cast<long long>(j) * (j + 1) / 2 + i) * 8 + slot));
+    for (int jp = 0; jp < 4; ++jp) {
+        int own[4], got[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int e = static_cast<int>(v[8 * jp + k]);      // even station of the pair, column (pj, cj) = k
+            const int o = static_cast<int>(v[8 * jp + 4 + k]);  // odd station of the pair
+            own[k] = ci ? o : e;
+            got[k] = __shfl_xor_sync(0xffffffffu, ci ? e : o, 1);
+        }
+        // R[k] = G[(i,pi,re),(j,k)], I[k] = G[(i,pi,im),(j,k)] for this lane's station j; k = 2*pj + cj
+        const int R0 = ci ? got[0] : own[0], R1 = ci ? got[1] : own[1], R2 = ci ? got[2] : own[2], R3 = ci ? got[3] : own[3];
+        const int I0 = ci ? own[0] : got[0], I1 = ci ? own[1] : got[1], I2 = ci ? own[2] : got[2], I3 = ci ? own[3] : got[3];
+        int4 out;
+        out.x = R0 + I1;   // Re [pi][0] = G[re,re] + G[im,im]
+        out.y = I0 - R1;   // Im [pi][0] = G[im,re] - G[re,im]
+        out.z = R2 + I3;   // Re [pi][1]
+        out.w = I2 - R3;   // Im [pi][1]
+        const int j = jbase + 2 * jp + ci;
+        if ((!MASKED || (i <= j && j < N)) && !NOSTORE) {
+            int4* dst = reinterpret_cast<int4*>(visf + ((static_cast<long long>(j) * (j + 1) / 2 + i) * 8 + slot));
             if (ACC) {
-                const int2 old = *dst;
-                re += old.x;
-                im += old.y;
+                const int4 old = __ldcs(dst);
+                out.x += old.x;
+                out.y += old.y;
+                out.z += old.z;
+                out.w += old.w;
             }
-            *dst = make_int2(re, im);
+            __stcs(dst, out);   // streaming: written once, never re-read by this kernel
         }
     }
 }
 
-template <int UMMA_N>
+template <int UMMA_N, int CG, bool TRACE = false>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
-    using Cfg = TcCfg<UMMA_N>;
+    using Cfg = TcCfg<UMMA_N, CG>;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // Barriers first, operand ring after, on a 1024-byte boundary (SWIZZLE_128B atoms).
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw);
-    const uint32_t bar0 = smem_u32(bars);
-    auto full_bar = [&](int s) { return bar0 + 8u * s; };
-    auto empty_bar = [&](int s) { return bar0 + 8u * (Cfg::STAGES + s); };
-    auto tfull_bar = [&](int b) { return bar0 + 8u * (2 * Cfg::STAGES + b); };
-    auto tempty_bar = [&](int b) { return bar0 + 8u * (2 * Cfg::STAGES + 2 + b); };
+    const uint32_t bar0 = smem_u32(smem_raw);
+    auto full_bar = [&](uint32_t s) { return bar0 + 8u * s; };
+    auto empty_bar = [&](uint32_t s) { return bar0 + 8u * (Cfg::STAGES + s); };
+    auto tfull_bar = [&](uint32_t b) { return bar0 + 8u * (2 * Cfg::STAGES + b); };
+    auto tempty_bar = [&](uint32_t b) { return bar0 + 8u * (2 * Cfg::STAGES + 2 + b); };
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem_raw + 8 * (2 * Cfg::STAGES + 4));
-    const uint32_t ring0 = (smem_u32(smem_raw) + Cfg::BAR_BYTES + 1023u) & ~1023u;
+    const uint32_t ring0 = (bar0 + Cfg::BAR_BYTES + 1023u) & ~1023u;
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    constexpr uint32_t TMEM_COLS = 2 * UMMA_N;  // 512 or 256: a power of two >= 32
+    const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;         // 0 = leader of the CTA pair
+    const int unit = (CG == 2) ? static_cast<int>(blockIdx.x >> 1) : static_cast<int>(blockIdx.x);
+    const int nunits = static_cast<int>(gridDim.x) / CG;              // persistent CTAs (pairs)
+    constexpr uint32_t TMEM_COLS = 2 * UMMA_N;                         // 512 or 256: a power of two >= 32
 
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&tmap);
         for (int s = 0; s < Cfg::STAGES; ++s) {
-            mbar_init(full_bar(s), 1);
-            mbar_init(empty_bar(s), 1);
+            mbar_init(full_bar(s), 1);     // producer's arrive.expect_tx (+ TMA bytes of the whole pair)
+            mbar_init(empty_bar(s), 1);    // tcgen05.commit (multicast to both CTAs when CG = 2)
         }
         for (int b = 0; b < 2; ++b) {
-            mbar_init(tfull_bar(b), 1);
-            mbar_init(tempty_bar(b), 4);  // one arrival per epilogue warp
+            mbar_init(tfull_bar(b), 1);            // tcgen05.commit
+            mbar_init(tempty_bar(b), TC_EPI_WARPS * CG);   // one arrival per epilogue warp of the pair (on the leader)
         }
         fence_barrier_init();
     }
     if (warp == 1) {
-        tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
-        tmem_relinquish();
+        tmem_alloc<CG>(smem_u32(tmem_slot), TMEM_COLS);
+        tmem_relinquish<CG>();
     }
     tc_fence_before();
-    __syncthreads();
+    if (CG == 2) cluster_sync_all(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
     const int KB = (p.T + TC_BK - 1) / TC_BK;
 
     if (warp == 0) {
-        // ===== TMA producer (one lane) =====
-        if (lane == 0) {
-            int stage = 0;
-            uint32_t phase = 0;
-            for (long long w = blockIdx.x; w < p.total_tiles; w += gridDim.x) {
-                const int f = static_cast<int>(w / p.tiles_per_f);
-                const uint32_t tb = __ldg(p.tiles + static_cast<int>(w % p.tiles_per_f));
-                const int m_a = static_cast<int>(tb & 0xFFFFu) * TC_M;
-                const int m_b = static_cast<int>(tb >> 16) * UMMA_N;
-                for (int kb = 0; kb < KB; ++kb) {
-                    mbar_wait(empty_bar(stage), phase ^ 1u);
+        // ===== TMA producer: the whole warp walks the loop, one elected lane issues =====
+        const uint32_t elected = elect_one();
+        uint32_t stage = 0, phase = 0;
+        int it = 0;
+        uint32_t tb_next = (unit < p.total_tiles) ? __ldg(p.tiles + unit % p.tiles_per_f) : 0u;
+        for (int w = unit; w < p.total_tiles; w += nunits) {
+            const int f = w / p.tiles_per_f;
+            const uint32_t tb = __shfl_sync(0xffffffffu, tb_next, 0);
+            // the next tile's table entry is fetched now so that its latency hides behind this tile's k loop
+            if (w + nunits < p.total_tiles) tb_next = __ldg(p.tiles + (w + nunits) % p.tiles_per_f);
+            const int m_a = static_cast<int>(tb & 0xFFFFu) * Cfg::M + 128 * static_cast<int>(rank);
+            const int m_b = static_cast<int>(tb >> 16) * UMMA_N + Cfg::B_BOXES * 128 * static_cast<int>(rank);
+            const bool a_in_b = (m_a >= m_b) && (m_a < m_b + Cfg::B_BOXES * 128);   // diagonal: A rows are B rows
+            const uint32_t my_bytes = a_in_b ? Cfg::B_BYTES : Cfg::STAGE_BYTES;
+            for (int kb = 0; kb < KB; ++kb) {
+                const bool tr = TRACE && p.trace && blockIdx.x == 0 && it < TC_TRACE_ITERS && elected;
+                if (tr) p.trace[(0 * TC_TRACE_ITERS + it) * 4 + 0] = clock64();
+                mbar_wait(empty_bar(stage), phase ^ 1u);
+                if (tr) p.trace[(0 * TC_TRACE_ITERS + it) * 4 + 1] = clock64();
+                if (elected) {
                     const uint32_t sa = ring0 + stage * Cfg::STAGE_BYTES;
                     const uint32_t sb = sa + Cfg::A_BYTES;
-                    mbar_arrive_expect_tx(full_bar(stage), Cfg::STAGE_BYTES);
                     const int t0 = kb * TC_BK;
-                    tma_load_3d(sa, &tmap, full_bar(stage), m_a, f, t0);
+                    if ((p.debug_skip & 1) && (w != unit || kb >= Cfg::STAGES)) {
+                        if (rank == 0) mbar_arrive(full_bar(stage));
+                    } else if (CG == 1) {
+                        mbar_arrive_expect_tx(full_bar(stage), my_bytes);
+                        if (!a_in_b) tma_load_3d(sa, &tmap, full_bar(stage), m_a, f, t0);
 #pragma unroll
-                    for (int h = 0; h < UMMA_N / 128; ++h)
-                        tma_load_3d(sb + h * (TC_BK * 128), &tmap, full_bar(stage), m_b + 128 * h, f, t0);
-                    if (++stage == Cfg::STAGES) {
-                        stage = 0;
-                        phase ^= 1u;
+                        for (int h = 0; h < Cfg::B_BOXES; ++h)
+                            tma_load_3d(sb + h * TC_BOX_BYTES, &tmap, full_bar(stage), m_b + 128 * h, f, t0);
+                    } else {
+                        // both CTAs' bytes are counted on the LEADER's barrier (a_in_b is the same in both)
+                        const uint32_t lead_full = mapa_u32(full_bar(stage), 0);
+                        if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * my_bytes);
+                        if (!a_in_b) tma_load_3d_2sm(sa, &tmap, lead_full, m_a, f, t0);
+#pragma unroll
+                        for (int h = 0; h < Cfg::B_BOXES; ++h)
+                            tma_load_3d_2sm(sb + h * TC_BOX_BYTES, &tmap, lead_full, m_b + 128 * h, f, t0);
                     }
+                }
+                __syncwarp();
+                if (tr) p.trace[(0 * TC_TRACE_ITERS + it) * 4 + 2] = clock64();
+                ++it;
+                if (++stage == Cfg::STAGES) {
+                    stage = 0;
+                    phase ^= 1u;
                 }
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer (one lane) =====
-        if (lane == 0) {
-            constexpr uint32_t idesc = make_idesc_i8_mn(TC_M, UMMA_N);
-            int stage = 0;
-            uint32_t phase = 0;
-            int buf = 0;
-            uint32_t tphase = 0u;  // bit b = phase of accumulator b
-            for (long long w = blockIdx.x; w < p.total_tiles; w += gridDim.x) {
-                mbar_wait(tempty_bar(buf), ((tphase >> buf) & 1u) ^ 1u);  // epilogue has drained this accumulator
+        // ===== MMA issuer: leader CTA only; warp-uniform loop, one elected lane issues =====
+        if (rank == 0) {
+            const uint32_t elected = elect_one();
+            constexpr uint32_t idesc = make_idesc_i8_mn(Cfg::M, UMMA_N);
+            uint32_t stage = 0, phase = 0, buf = 0, tphase = 0;   // tphase bit b = phase of accumulator b
+            int it = 0;
+            uint32_t tb_next = (unit < p.total_tiles) ? __ldg(p.tiles + unit % p.tiles_per_f) : 0u;
+            for (int w = unit; w < p.total_tiles; w += nunits) {
+                const uint32_t tb = __shfl_sync(0xffffffffu, tb_next, 0);
+                if (w + nunits < p.total_tiles) tb_next = __ldg(p.tiles + (w + nunits) % p.tiles_per_f);
+                const int m_a = static_cast<int>(tb & 0xFFFFu) * Cfg::M;
+                const int m_b = static_cast<int>(tb >> 16) * UMMA_N;
+                const bool a_in_b = (m_a >= m_b) && (m_a < m_b + Cfg::B_BOXES * 128);
+                // byte offset of the A operand inside a stage: its own box, or the B box holding the same rows
+                const uint32_t a_off = a_in_b ? static_cast<uint32_t>(Cfg::A_BYTES + ((m_a - m_b) >> 7) * TC_BOX_BYTES) : 0u;
+                mbar_wait(tempty_bar(buf), ((tphase >> buf) & 1u) ^ 1u);  // epilogues have drained this accumulator
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(buf * UMMA_N);
+                const uint32_t d_tmem = tmem_base + buf * UMMA_N;
                 for (int kb = 0; kb < KB; ++kb) {
+                    const bool tr = TRACE && p.trace && blockIdx.x == 0 && it < TC_TRACE_ITERS && elected;
+                    if (tr) p.trace[(1 * TC_TRACE_ITERS + it) * 4 + 0] = clock64();
                     mbar_wait(full_bar(stage), phase);
                     tc_fence_after();
-                    const uint32_t sa = ring0 + stage * Cfg::STAGE_BYTES;
-                    const uint32_t sb = sa + Cfg::A_BYTES;
-                    const uint64_t adesc = make_smem_desc_mn_sw128(sa, TC_BK * 128, 1024);
-                    const uint64_t bdesc = make_smem_desc_mn_sw128(sb, TC_BK * 128, 1024);
-                    const int rows = min(TC_BK, p.T - kb * TC_BK);           // valid samples in this stage
-                    const int nk = (rows + TC_UMMA_K - 1) / TC_UMMA_K;       // rows beyond T are TMA zero fill
+                    if (tr) p.trace[(1 * TC_TRACE_ITERS + it) * 4 + 1] = clock64();
+                    if (elected) {
+                        const uint32_t sa = ring0 + stage * Cfg::STAGE_BYTES;
+                        const uint64_t adesc = make_smem_desc_mn_sw128(sa + a_off, TC_BOX_BYTES, 1024);
+                        const uint64_t bdesc = make_smem_desc_mn_sw128(sa + Cfg::A_BYTES, TC_BOX_BYTES, 1024);
+                        const int rows = min(TC_BK, p.T - kb * TC_BK);           // valid samples in this stage
+                        const int nk = (rows + TC_UMMA_K - 1) / TC_UMMA_K;       // rows beyond T are TMA zero fill
 #pragma unroll
-                    for (int ks = 0; ks < TC_BK / TC_UMMA_K; ++ks) {
-                        if (ks < nk) {
-                            // K advance: 32 samples = 4 swizzle atoms = 4096 B -> +256 in the address field
-                            umma_i8(d_tmem, adesc + static_cast<uint64_t>(ks * 256), bdesc + static_cast<uint64_t>(ks * 256),
-                                    idesc, (kb | ks) ? 1u : 0u);
+                        for (int ks = 0; ks < TC_BK / TC_UMMA_K; ++ks) {
+                            if (ks < nk && !(p.debug_skip & 2)) {
+                                // K advance: 32 samples = 4 swizzle atoms = 4096 B -> +256 in the address field
+                                umma_i8<CG>(d_tmem, adesc + static_cast<uint64_t>(ks * 256),
+                                            bdesc + static_cast<uint64_t>(ks * 256), idesc, (kb | ks) ? 1u : 0u);
+                            }
                         }
+                        if (tr) p.trace[(1 * TC_TRACE_ITERS + it) * 4 + 2] = clock64();
+                        umma_commit<CG>(empty_bar(stage));  // frees the ring slot (in both CTAs) when these MMAs retire
+                        if (kb == KB - 1) umma_commit<CG>(tfull_bar(buf));  // accumulator complete -> epilogues
                     }
-                    umma_commit(empty_bar(stage));  // frees the ring slot when these MMAs retire
+                    __syncwarp();
+                    if (tr) p.trace[(1 * TC_TRACE_ITERS + it) * 4 + 3] = clock64();
+                    ++it;
                     if (++stage == Cfg::STAGES) {
                         stage = 0;
                         phase ^= 1u;
                     }
                 }
-                umma_commit(tfull_bar(buf));  // accumulator complete -> epilogue
                 tphase ^= 1u << buf;
-                buf ^= 1;
+                buf ^= 1u;
             }
         }
     } else {
-        // ===== epilogue: warps 2..5, TMEM lane quarter = warp % 4 =====
+        // ===== epilogue: warps 2..9; TMEM lane quarter = warp % 4, column half = (warp - 2) / 4 =====
         const int q = warp & 3;
-        int buf = 0;
-        uint32_t tphase = 0u;
-        for (long long w = blockIdx.x; w < p.total_tiles; w += gridDim.x) {
-            const int f = static_cast<int>(w / p.tiles_per_f);
-            const uint32_t tb = __ldg(p.tiles + static_cast<int>(w % p.tiles_per_f));
-            const int i0 = static_cast<int>(tb & 0xFFFFu) * 32 + 8 * q;  // first station of this warp's rows
-            const int j0 = static_cast<int>(tb >> 16) * Cfg::SJ;
-            const int i = i0 + (lane >> 2);
+        const int half = (warp - 2) >> 2;
+        constexpr int CHUNKS = UMMA_N / 32 / 2;   // 32-column chunks per warp
+        uint32_t buf = 0, tphase = 0;
+        int it = 0;
+        const uint32_t lead_tempty0 = (CG == 2) ? mapa_u32(tempty_bar(0), 0) : tempty_bar(0);
+        uint32_t tb_next = (unit < p.total_tiles) ? __ldg(p.tiles + unit % p.tiles_per_f) : 0u;
+        for (int w = unit; w < p.total_tiles; w += nunits) {
+            const bool tr = TRACE && p.trace && blockIdx.x == 0 && it < TC_TRACE_ITERS && warp == 2 && lane == 0;
+            if (tr) p.trace[(2 * TC_TRACE_ITERS + it) * 4 + 0] = clock64();
+            const int f = w / p.tiles_per_f;
+            const uint32_t tb = tb_next;
+            if (w + nunits < p.total_tiles) tb_next = __ldg(p.tiles + (w + nunits) % p.tiles_per_f);
+            const int i0 = static_cast<int>(tb & 0xFFFFu) * Cfg::SI + 32 * static_cast<int>(rank) + 8 * q;
+            const int j0 = static_cast<int>(tb >> 16) * Cfg::SJ + 8 * CHUNKS * half;   // first station of this warp's columns
+            const int i = i0 + (lane >> 2);                     // i0 = first station of this warp's rows
             int32_t* visf = p.vis + static_cast<long long>(f) * p.NB * 8;
 
             mbar_wait(tfull_bar(buf), (tphase >> buf) & 1u);
             tc_fence_after();
-            const uint32_t taddr0 = tmem_base + (static_cast<uint32_t>(32 * q) << 16) + static_cast<uint32_t>(buf * UMMA_N);
+            if (tr) p.trace[(2 * TC_TRACE_ITERS + it) * 4 + 1] = clock64();
+            const uint32_t taddr0 = tmem_base + (static_cast<uint32_t>(32 * q) << 16) + buf * UMMA_N + 32 * CHUNKS * half;
 #pragma unroll 1
-            for (int cc = 0; cc < UMMA_N / 32; ++cc) {
+            for (int cc = 0; cc < CHUNKS; ++cc) {
                 const int jbase = j0 + 8 * cc;
                 if (jbase >= p.N || jbase + 7 < i0) continue;  // warp-uniform: nothing of this chunk is stored
                 uint32_t v[32];
                 tmem_ld_32x32(taddr0 + static_cast<uint32_t>(32 * cc), v);
                 tmem_ld_wait();
                 const bool full = (i0 + 7 <= jbase) && (jbase + 7 < p.N);  // warp-uniform: no masking needed
-                if (p.accumulate) {
+                if (p.debug_skip & 4) {
+                    epi_chunk<true, false, true>(v, visf, i, jbase, p.N, lane);
+                } else if (p.accumulate) {
                     if (full) epi_chunk<false, true>(v, visf, i, jbase, p.N, lane);
                     else epi_chunk<true, true>(v, visf, i, jbase, p.N, lane);
                 } else {
@@ -233,18 +310,24 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
             }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(tempty_bar(buf));
+            if (lane == 0) {
+                if (CG == 2) mbar_arrive_cluster(lead_tempty0 + 8u * buf);
+                else mbar_arrive(tempty_bar(buf));
+            }
+            if (tr) p.trace[(2 * TC_TRACE_ITERS + it) * 4 + 2] = clock64();
+            ++it;
             tphase ^= 1u << buf;
-            buf ^= 1;
+            buf ^= 1u;
         }
     }
 
+    // Teardown: nobody leaves (or frees TMEM) while the peer may still signal into this CTA.
     tc_fence_before();
-    __syncthreads();
+    if (CG == 2) cluster_sync_all(); else __syncthreads();
     if (warp == 1) {
         __syncwarp();
         tc_fence_after();
-        tmem_dealloc(tmem_base, TMEM_COLS);
+        tmem_dealloc<CG>(tmem_base, TMEM_COLS);
     }
 }
 
