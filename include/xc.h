@@ -77,11 +77,18 @@ enum {
     XC_TILE_1CTA_128x256 = 2, /* 32 x 64 stations on one CTA                                       */
     XC_TILE_2CTA_256x256 = 3  /* 64 x 64 stations on a CTA pair (tcgen05 cta_group::2)             */
 };
+/* Epilogue store path of the tensor-core kernel, xc_set_option(XC_OPT_EPILOGUE, ...). */
+enum {
+    XC_EPI_AUTO = 0,
+    XC_EPI_DIRECT = 1, /* registers -> 16-byte streaming global stores                                   */
+    XC_EPI_STAGED = 2  /* registers -> packed tile in shared memory -> bulk (TMA) stores / reduce-adds   */
+};
 typedef enum {
     XC_OPT_I8_KERNEL = 0, /* one of XC_I8_KERNEL_*                                            */
     XC_OPT_MAX_CTAS = 1,  /* cap on persistent CTAs of the tensor-core kernel (0 = SM count)  */
     XC_OPT_FORCE_STAGE = 2, /* 1 = always run the staging (pad/copy) kernel, for testing S0    */
     XC_OPT_TILE = 4,       /* one of XC_TILE_*; rebuilds the tile schedule (synchronising on next call) */
+    XC_OPT_EPILOGUE = 5,   /* one of XC_EPI_*                                                  */
     XC_OPT_DEBUG_SKIP = 3  /* PROFILING ONLY, results become meaningless: bit 0 = no TMA loads  */
                            /* after the first ring fill, bit 1 = no MMAs, bit 2 = no stores     */
 } xc_option;

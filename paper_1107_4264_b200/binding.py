@@ -13,7 +13,8 @@ LIB_PATH = os.path.join(HERE, "libxc.so")
 
 MAX_T = 65535
 I8_KERNEL_AUTO, I8_KERNEL_TC, I8_KERNEL_SIMT = 0, 1, 2
-OPT_I8_KERNEL, OPT_MAX_CTAS, OPT_FORCE_STAGE, OPT_DEBUG_SKIP, OPT_TILE = 0, 1, 2, 3, 4
+OPT_I8_KERNEL, OPT_MAX_CTAS, OPT_FORCE_STAGE, OPT_DEBUG_SKIP, OPT_TILE, OPT_EPILOGUE = 0, 1, 2, 3, 4, 5
+EPI_AUTO, EPI_DIRECT, EPI_STAGED = 0, 1, 2
 TILE_AUTO, TILE_1CTA_128x128, TILE_1CTA_128x256, TILE_2CTA_256x256 = 0, 1, 2, 3
 
 # every symbol include/xc.h declares

@@ -56,11 +56,11 @@ struct xc_plan_s {
     void* ws = nullptr;
     size_t ws_bytes = 0;
     bool ws_owned = false;
-    int opt_kernel = XC_I8_KERNEL_AUTO, opt_max_ctas = 0, opt_force_stage = 0, opt_debug_skip = 0;
+    int opt_kernel = XC_I8_KERNEL_AUTO, opt_max_ctas = 0, opt_force_stage = 0, opt_debug_skip = 0, opt_epilogue = 0;
     long long* trace = nullptr;
     CUtensorMap tmap;
     const void* tmap_src = nullptr;
-    int tmap_nrow = 0;
+    int tmap_nrow = 0, tmap_bk = 0;
     cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_entry = nullptr;
     int last_launches = 0;
     std::string last_err;
@@ -112,7 +112,7 @@ int upload_tiles(xc_plan_t* p) {
     return XC_OK;
 }
 
-template <int UMMA_N, int CG>
+template <int UMMA_N, int CG, bool STAGED>
 int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
     long long units = (p->opt_max_ctas > 0 ? p->opt_max_ctas : p->sm_count) / CG;
     if (units < 1) units = 1;
@@ -120,7 +120,7 @@ int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(units * CG));
     cfg.blockDim = dim3(xc::TC_THREADS);
-    cfg.dynamicSmemBytes = xc::TcCfg<UMMA_N, CG>::SMEM_BYTES;
+    cfg.dynamicSmemBytes = xc::TcCfg<UMMA_N, CG, STAGED>::SMEM_BYTES;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -129,11 +129,11 @@ int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (CG == 2 && UMMA_N == 256 && tp.trace) {
-        XC_CUDA(p, cudaLaunchKernelEx(&cfg, xc::xc_i8_tc_kernel<256, 2, true>, p->tmap, tp));
-    } else {
-        XC_CUDA(p, cudaLaunchKernelEx(&cfg, xc::xc_i8_tc_kernel<UMMA_N, CG, false>, p->tmap, tp));
-    }
+    auto kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, false>;
+    if (CG == 2 && UMMA_N == 256 && tp.trace) kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, (CG == 2 && UMMA_N == 256)>;
+    XC_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    xc::TcCfg<UMMA_N, CG, STAGED>::SMEM_BYTES));
+    XC_CUDA(p, cudaLaunchKernelEx(&cfg, kern, p->tmap, tp));
     return XC_OK;
 }
 
@@ -165,14 +165,6 @@ int ensure_device(xc_plan_t* p) {
         return XC_ERR_CUDA;
     }
     p->encode = reinterpret_cast<PFN_encodeTiled>(fn);
-    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_kernel<128, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    xc::TcCfg<128, 1>::SMEM_BYTES));
-    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_kernel<256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    xc::TcCfg<256, 1>::SMEM_BYTES));
-    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_kernel<256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    xc::TcCfg<256, 2>::SMEM_BYTES));
-    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_kernel<256, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    xc::TcCfg<256, 2>::SMEM_BYTES));
     XC_CUDA(p, cudaFuncSetAttribute(xc::xc_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     xc::F32_SMEM_BYTES));
     p->dev_ready = true;
@@ -207,13 +199,13 @@ int stage_if_needed(xc_plan_t* p, const int8_t* in_dev, cudaStream_t st, const v
     return XC_OK;
 }
 
-int encode_tmap(xc_plan_t* p, const void* src, int nrow) {
-    if (p->tmap_src == src && p->tmap_nrow == nrow) return XC_OK;
+int encode_tmap(xc_plan_t* p, const void* src, int nrow, int bk) {
+    if (p->tmap_src == src && p->tmap_nrow == nrow && p->tmap_bk == bk) return XC_OK;
     const cuuint64_t gdim[3] = {static_cast<cuuint64_t>(4) * nrow, static_cast<cuuint64_t>(p->F),
                                 static_cast<cuuint64_t>(p->T)};
     const cuuint64_t gstride[2] = {static_cast<cuuint64_t>(4) * nrow,
                                    static_cast<cuuint64_t>(4) * nrow * static_cast<cuuint64_t>(p->F)};
-    const cuuint32_t box[3] = {128, 1, static_cast<cuuint32_t>(xc::TC_BK)};
+    const cuuint32_t box[3] = {128, 1, static_cast<cuuint32_t>(bk)};
     const cuuint32_t estr[3] = {1, 1, 1};
     CUresult r = p->encode(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(src), gdim, gstride, box, estr,
                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -227,6 +219,7 @@ int encode_tmap(xc_plan_t* p, const void* src, int nrow) {
     }
     p->tmap_src = src;
     p->tmap_nrow = nrow;
+    p->tmap_bk = bk;
     return XC_OK;
 }
 
@@ -253,7 +246,10 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     int nrow = 0;
     rc = stage_if_needed(p, in_dev, st, &src, &nrow);
     if (rc != XC_OK) return rc;
-    rc = encode_tmap(p, src, nrow);
+    const int bk = p->tile_mode == XC_TILE_2CTA_256x256   ? xc::TcCfg<256, 2, false>::BK
+                   : p->tile_mode == XC_TILE_1CTA_128x256 ? xc::TcCfg<256, 1, false>::BK
+                                                          : xc::TcCfg<128, 1, false>::BK;
+    rc = encode_tmap(p, src, nrow, bk);
     if (rc != XC_OK) return rc;
 
     rc = upload_tiles(p);
@@ -271,9 +267,13 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     tp.accumulate = accumulate;
     tp.debug_skip = p->opt_debug_skip;
     tp.trace = p->trace;
-    if (p->tile_mode == XC_TILE_2CTA_256x256) rc = launch_tc<256, 2>(p, tp, st);
-    else if (p->tile_mode == XC_TILE_1CTA_128x256) rc = launch_tc<256, 1>(p, tp, st);
-    else rc = launch_tc<128, 1>(p, tp, st);
+    const bool staged = p->opt_epilogue == XC_EPI_STAGED;   // AUTO = direct stores (measured faster)
+    if (p->tile_mode == XC_TILE_2CTA_256x256)
+        rc = staged ? launch_tc<256, 2, true>(p, tp, st) : launch_tc<256, 2, false>(p, tp, st);
+    else if (p->tile_mode == XC_TILE_1CTA_128x256)
+        rc = staged ? launch_tc<256, 1, true>(p, tp, st) : launch_tc<256, 1, false>(p, tp, st);
+    else
+        rc = staged ? launch_tc<128, 1, true>(p, tp, st) : launch_tc<128, 1, false>(p, tp, st);
     if (rc != XC_OK) return rc;
     p->last_launches += 1;
     return XC_OK;
@@ -354,8 +354,12 @@ int xc_set_option(xc_plan_t* p, int option, int value) {
             if (value < XC_TILE_AUTO || value > XC_TILE_2CTA_256x256) return XC_ERR_INVALID_ARG;
             set_tile_mode(p, value);
             return XC_OK;
+        case XC_OPT_EPILOGUE:
+            if (value < XC_EPI_AUTO || value > XC_EPI_STAGED) return XC_ERR_INVALID_ARG;
+            p->opt_epilogue = value;
+            return XC_OK;
         case XC_OPT_DEBUG_SKIP:
-            p->opt_debug_skip = value & 7;
+            p->opt_debug_skip = value & 15;
             return XC_OK;
         default:
             return XC_ERR_INVALID_ARG;

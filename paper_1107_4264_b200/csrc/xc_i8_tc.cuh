@@ -34,27 +34,34 @@
 
 namespace xc {
 
-constexpr int TC_BK = 128;         // samples per pipeline stage
 constexpr int TC_UMMA_K = 32;      // samples per tcgen05.mma (kind::i8)
 constexpr int TC_EPI_WARPS = 8;     // 2 per TMEM lane quarter, each owning half of the tile's columns
 constexpr int TC_THREADS = 64 + 32 * TC_EPI_WARPS;   // + TMA producer warp + MMA issuer warp
 constexpr int TC_SMEM_LIMIT = 232448;  // 227 KB
-constexpr int TC_BOX_BYTES = TC_BK * 128;   // one TMA box: BK rows of 128 bytes
 
-template <int UMMA_N, int CG>
+template <int UMMA_N, int CG, bool STAGED>
 struct TcCfg {
     static constexpr int M = 128 * CG;                    // Gram rows per tile
     static constexpr int B_BOXES = UMMA_N / 128 / CG;     // 128-row B boxes held by one CTA
-    static constexpr int A_BYTES = TC_BOX_BYTES;
-    static constexpr int B_BYTES = B_BOXES * TC_BOX_BYTES;
+    // Samples per pipeline stage.  Every stage costs the producer and the MMA issuer some hundred cycles of
+    // barrier round trips and instruction issue (measured), so a stage must hold clearly more than that in
+    // tensor work (128 cycles per 32 samples).  192-sample stages (4 of them) measured slower than 128 x 7.
+    static constexpr int BK = 128;
+    static constexpr int BOX_BYTES = BK * 128;            // one TMA box: BK rows of 128 bytes
+    static constexpr int A_BYTES = BOX_BYTES;
+    static constexpr int B_BYTES = B_BOXES * BOX_BYTES;
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-    static constexpr int STAGES = 196608 / STAGE_BYTES;   // 4 x 48 KB or 6 x 32 KB
-    static constexpr int BAR_BYTES = 1024;                // barriers + tmem slot, kept in the first KB
-    static constexpr int SMEM_BYTES = BAR_BYTES + STAGES * STAGE_BYTES + 1024;  // + slack for 1024-B alignment
     static constexpr int SI = 32 * CG;                    // stations per tile on the i side
     static constexpr int SJ = UMMA_N / 4;                 // stations per tile on the j side
+    // STAGED: the epilogue packs the tile's visibilities into shared memory ([SJ rows j][32 stations i][32 B]) and
+    // the TMA store engine writes each row's contiguous run to global memory (bulk copy / bulk reduce-add).
+    static constexpr int OUT_BYTES = STAGED ? SJ * 1024 : 0;
+    static constexpr int STAGES = (229376 - OUT_BYTES) / STAGE_BYTES;   // 224 KB for ring + staging tile
+    static constexpr int BAR_BYTES = 1024;                // barriers + tmem slot, kept in the first KB
+    static constexpr int SMEM_BYTES = BAR_BYTES + STAGES * STAGE_BYTES + OUT_BYTES + 1024;  // + slack for 1024-B alignment
     static_assert(B_BOXES >= 1, "a CTA holds at least one 128-row B box");
     static_assert(SMEM_BYTES <= TC_SMEM_LIMIT, "smem");
+    static_assert(STAGES >= 3, "ring too shallow");
 };
 
 struct TcParams {
@@ -78,7 +85,7 @@ constexpr int TC_TRACE_ITERS = 256;   // k-blocks traced; layout: [3 roles][TC_T
 // one, after swapping the four values the other needs (4 shuffles per station pair).  Each lane then
 // owns [pi][pj=0,1][re,im] of its (i, j) = 16 contiguous bytes, two lanes one 32-byte record, and a
 // warp store instruction writes two 256-byte runs (8 consecutive i for each of the two j).
-template <bool MASKED, bool ACC, bool NOSTORE = false>
+template <bool MASKED, bool ACC, bool NOSTORE = false, bool WRAP = false>
 __device__ __forceinline__ void epi_chunk(const uint32_t (&v)[32], int32_t* __restrict__ visf, int i, int jbase, int N,
                                           int lane) {
     const int ci = lane & 1;
@@ -103,7 +110,9 @@ __device__ __forceinline__ void epi_chunk(const uint32_t (&v)[32], int32_t* __re
         out.w = I2 - R3;   // Im [pi][1]
         const int j = jbase + 2 * jp + ci;
         if ((!MASKED || (i <= j && j < N)) && !NOSTORE) {
-            int4* dst = reinterpret_cast<int4*>(visf + ((static_cast<long long>(j) * (j + 1) / 2 + i) * 8 + slot));
+            long long off = (static_cast<long long>(j) * (j + 1) / 2 + i) * 8 + slot;
+            if (WRAP) off &= (1 << 21) - 1;   // profiling: keep all stores inside an 8 MB window (L2 resident)
+            int4* dst = reinterpret_cast<int4*>(visf + off);
             if (ACC) {
                 const int4 old = __ldcs(dst);
                 out.x += old.x;
@@ -116,10 +125,29 @@ __device__ __forceinline__ void epi_chunk(const uint32_t (&v)[32], int32_t* __re
     }
 }
 
-template <int UMMA_N, int CG, bool TRACE = false>
+// Same combine, but the 16 bytes go to the packed staging tile in shared memory (row pitch 1024 B per j).
+__device__ __forceinline__ void epi_chunk_smem(const uint32_t (&v)[32], uint32_t dst, int lane) {
+    const int ci = lane & 1;
+#pragma unroll
+    for (int jp = 0; jp < 4; ++jp) {
+        int own[4], got[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int e = static_cast<int>(v[8 * jp + k]);
+            const int o = static_cast<int>(v[8 * jp + 4 + k]);
+            own[k] = ci ? o : e;
+            got[k] = __shfl_xor_sync(0xffffffffu, ci ? e : o, 1);
+        }
+        const int R0 = ci ? got[0] : own[0], R1 = ci ? got[1] : own[1], R2 = ci ? got[2] : own[2], R3 = ci ? got[3] : own[3];
+        const int I0 = ci ? own[0] : got[0], I1 = ci ? own[1] : got[1], I2 = ci ? own[2] : got[2], I3 = ci ? own[3] : got[3];
+        st_shared_v4(dst + static_cast<uint32_t>((2 * jp + ci) * 1024), make_int4(R0 + I1, I0 - R1, R2 + I3, I2 - R3));
+    }
+}
+
+template <int UMMA_N, int CG, bool STAGED, bool TRACE = false>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
-    using Cfg = TcCfg<UMMA_N, CG>;
+    using Cfg = TcCfg<UMMA_N, CG, STAGED>;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // Barriers first, operand ring after, on a 1024-byte boundary (SWIZZLE_128B atoms).
     const uint32_t bar0 = smem_u32(smem_raw);
@@ -129,6 +157,7 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
     auto tempty_bar = [&](uint32_t b) { return bar0 + 8u * (2 * Cfg::STAGES + 2 + b); };
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem_raw + 8 * (2 * Cfg::STAGES + 4));
     const uint32_t ring0 = (bar0 + Cfg::BAR_BYTES + 1023u) & ~1023u;
+    const uint32_t out0 = ring0 + Cfg::STAGES * Cfg::STAGE_BYTES;    // STAGED: packed output tile
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -158,7 +187,7 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    const int KB = (p.T + TC_BK - 1) / TC_BK;
+    const int KB = (p.T + Cfg::BK - 1) / Cfg::BK;
 
     if (warp == 0) {
         // ===== TMA producer: the whole warp walks the loop, one elected lane issues =====
@@ -183,7 +212,7 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
                 if (elected) {
                     const uint32_t sa = ring0 + stage * Cfg::STAGE_BYTES;
                     const uint32_t sb = sa + Cfg::A_BYTES;
-                    const int t0 = kb * TC_BK;
+                    const int t0 = kb * Cfg::BK;
                     if ((p.debug_skip & 1) && (w != unit || kb >= Cfg::STAGES)) {
                         if (rank == 0) mbar_arrive(full_bar(stage));
                     } else if (CG == 1) {
@@ -191,7 +220,7 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
                         if (!a_in_b) tma_load_3d(sa, &tmap, full_bar(stage), m_a, f, t0);
 #pragma unroll
                         for (int h = 0; h < Cfg::B_BOXES; ++h)
-                            tma_load_3d(sb + h * TC_BOX_BYTES, &tmap, full_bar(stage), m_b + 128 * h, f, t0);
+                            tma_load_3d(sb + h * Cfg::BOX_BYTES, &tmap, full_bar(stage), m_b + 128 * h, f, t0);
                     } else {
                         // both CTAs' bytes are counted on the LEADER's barrier (a_in_b is the same in both)
                         const uint32_t lead_full = mapa_u32(full_bar(stage), 0);
@@ -199,7 +228,7 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
                         if (!a_in_b) tma_load_3d_2sm(sa, &tmap, lead_full, m_a, f, t0);
 #pragma unroll
                         for (int h = 0; h < Cfg::B_BOXES; ++h)
-                            tma_load_3d_2sm(sb + h * TC_BOX_BYTES, &tmap, lead_full, m_b + 128 * h, f, t0);
+                            tma_load_3d_2sm(sb + h * Cfg::BOX_BYTES, &tmap, lead_full, m_b + 128 * h, f, t0);
                     }
                 }
                 __syncwarp();
@@ -226,7 +255,7 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
                 const int m_b = static_cast<int>(tb >> 16) * UMMA_N;
                 const bool a_in_b = (m_a >= m_b) && (m_a < m_b + Cfg::B_BOXES * 128);
                 // byte offset of the A operand inside a stage: its own box, or the B box holding the same rows
-                const uint32_t a_off = a_in_b ? static_cast<uint32_t>(Cfg::A_BYTES + ((m_a - m_b) >> 7) * TC_BOX_BYTES) : 0u;
+                const uint32_t a_off = a_in_b ? static_cast<uint32_t>(Cfg::A_BYTES + ((m_a - m_b) >> 7) * Cfg::BOX_BYTES) : 0u;
                 mbar_wait(tempty_bar(buf), ((tphase >> buf) & 1u) ^ 1u);  // epilogues have drained this accumulator
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + buf * UMMA_N;
@@ -238,12 +267,12 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
                     if (tr) p.trace[(1 * TC_TRACE_ITERS + it) * 4 + 1] = clock64();
                     if (elected) {
                         const uint32_t sa = ring0 + stage * Cfg::STAGE_BYTES;
-                        const uint64_t adesc = make_smem_desc_mn_sw128(sa + a_off, TC_BOX_BYTES, 1024);
-                        const uint64_t bdesc = make_smem_desc_mn_sw128(sa + Cfg::A_BYTES, TC_BOX_BYTES, 1024);
-                        const int rows = min(TC_BK, p.T - kb * TC_BK);           // valid samples in this stage
+                        const uint64_t adesc = make_smem_desc_mn_sw128(sa + a_off, Cfg::BOX_BYTES, 1024);
+                        const uint64_t bdesc = make_smem_desc_mn_sw128(sa + Cfg::A_BYTES, Cfg::BOX_BYTES, 1024);
+                        const int rows = min(Cfg::BK, p.T - kb * Cfg::BK);           // valid samples in this stage
                         const int nk = (rows + TC_UMMA_K - 1) / TC_UMMA_K;       // rows beyond T are TMA zero fill
 #pragma unroll
-                        for (int ks = 0; ks < TC_BK / TC_UMMA_K; ++ks) {
+                        for (int ks = 0; ks < Cfg::BK / TC_UMMA_K; ++ks) {
                             if (ks < nk && !(p.debug_skip & 2)) {
                                 // K advance: 32 samples = 4 swizzle atoms = 4096 B -> +256 in the address field
                                 umma_i8<CG>(d_tmem, adesc + static_cast<uint64_t>(ks * 256),
@@ -290,6 +319,11 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
             tc_fence_after();
             if (tr) p.trace[(2 * TC_TRACE_ITERS + it) * 4 + 1] = clock64();
             const uint32_t taddr0 = tmem_base + (static_cast<uint32_t>(32 * q) << 16) + buf * UMMA_N + 32 * CHUNKS * half;
+            if (STAGED) {
+                // the previous tile's bulk stores must have finished reading the staging buffer
+                if (warp < 4) bulk_wait_read0();            // warps 2-3 issue the bulk stores
+                named_bar_sync(1, 32 * TC_EPI_WARPS);
+            }
 #pragma unroll 1
             for (int cc = 0; cc < CHUNKS; ++cc) {
                 const int jbase = j0 + 8 * cc;
@@ -298,8 +332,15 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
                 tmem_ld_32x32(taddr0 + static_cast<uint32_t>(32 * cc), v);
                 tmem_ld_wait();
                 const bool full = (i0 + 7 <= jbase) && (jbase + 7 < p.N);  // warp-uniform: no masking needed
-                if (p.debug_skip & 4) {
+                if (STAGED) {
+                    // row (j - tile's first j) of the staging buffer, 32 bytes per station i of this CTA, 16 per pol_i
+                    const uint32_t dst = out0 + static_cast<uint32_t>((8 * (CHUNKS * half + cc)) * 1024 +
+                                                                       (8 * q + (lane >> 2)) * 32 + ((lane >> 1) & 1) * 16);
+                    epi_chunk_smem(v, dst, lane);
+                } else if (p.debug_skip & 4) {
                     epi_chunk<true, false, true>(v, visf, i, jbase, p.N, lane);
+                } else if (p.debug_skip & 8) {
+                    epi_chunk<true, false, false, true>(v, p.vis, i, jbase, p.N, lane);
                 } else if (p.accumulate) {
                     if (full) epi_chunk<false, true>(v, visf, i, jbase, p.N, lane);
                     else epi_chunk<true, true>(v, visf, i, jbase, p.N, lane);
@@ -314,6 +355,23 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
                 if (CG == 2) mbar_arrive_cluster(lead_tempty0 + 8u * buf);
                 else mbar_arrive(tempty_bar(buf));
             }
+            if (STAGED) {
+                fence_proxy_async();                         // my st.shared -> visible to the bulk-copy engine
+                named_bar_sync(1, 32 * TC_EPI_WARPS);        // the whole tile is packed
+                const int e = static_cast<int>(threadIdx.x) - 64;   // epilogue thread index; thread e stores row e
+                if (e < Cfg::SJ && !(p.debug_skip & 4)) {
+                    const int ic = i0 - 8 * q;                       // first station of this CTA's 32 rows
+                    const int j = static_cast<int>(tb >> 16) * Cfg::SJ + e;
+                    const int last = min(min(ic + 31, j), p.N - 1);  // stored pairs of row j: ic <= i <= last (a prefix)
+                    if (j < p.N && last >= ic) {
+                        int32_t* g = visf + (static_cast<long long>(j) * (j + 1) / 2 + ic) * 8;
+                        const uint32_t bytes = static_cast<uint32_t>(last - ic + 1) * 32u;
+                        if (p.accumulate) bulk_reduce_add_s32(g, out0 + e * 1024, bytes);
+                        else bulk_store(g, out0 + e * 1024, bytes);
+                    }
+                    bulk_commit();
+                }
+            }
             if (tr) p.trace[(2 * TC_TRACE_ITERS + it) * 4 + 2] = clock64();
             ++it;
             tphase ^= 1u << buf;
@@ -321,6 +379,7 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
         }
     }
 
+    if (STAGED && warp >= 2 && warp < 4) bulk_wait0();   // the CTA's shared memory must outlive its bulk stores
     // Teardown: nobody leaves (or frees TMEM) while the peer may still signal into this CTA.
     tc_fence_before();
     if (CG == 2) cluster_sync_all(); else __syncthreads();

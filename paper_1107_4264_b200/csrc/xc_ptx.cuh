@@ -8,7 +8,7 @@
 namespace xc {
 
 #ifndef XC_SPIN_LIMIT
-#define XC_SPIN_LIMIT (1u << 26)   // mbarrier.try_wait retries before __trap(): a broken pipeline
+#define XC_SPIN_LIMIT 67108864   // mbarrier.try_wait retries before __trap(): a broken pipeline
 #endif                             // aborts the kernel instead of hanging the GPU
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -26,7 +26,7 @@ __device__ __forceinline__ void fence_proxy_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+    asm volatile("mbarrier.arrive.relaxed.cta.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
@@ -42,11 +42,27 @@ __device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t parity)
         : "memory");
     return ok;
 }
+// Spin until the phase with the given parity has completed.  The loop lives inside ONE asm statement so
+// that the compiler sees straight-line, convergent code around it (a C++ loop on a per-thread predicate
+// makes everything after it "possibly divergent" and pushes addresses out of the uniform registers).
+// A bounded retry count turns a broken pipeline into a trap instead of a hung GPU.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    uint32_t spins = 0;
-    while (!mbar_try_wait(bar, parity)) {
-        if (++spins > XC_SPIN_LIMIT) __trap();
-    }
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p, q;\n\t"
+        ".reg .u32 n;\n\t"
+        "mov.u32 n, 0;\n\t"
+        "XC_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra XC_DONE;\n\t"
+        "add.u32 n, n, 1;\n\t"
+        "setp.gt.u32 q, n, %2;\n\t"
+        "@q trap;\n\t"
+        "bra XC_WAIT;\n\t"
+        "XC_DONE:\n\t"
+        "}" ::"r"(bar),
+        "r"(parity), "n"(XC_SPIN_LIMIT)
+        : "memory");
 }
 
 // ---- clusters / CTA pairs ------------------------------------------------------------------------
@@ -64,9 +80,13 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
     return r;
 }
-// arrive on an mbarrier anywhere in the cluster (address from mapa_u32)
+// Arrive on an mbarrier anywhere in the cluster (address from mapa_u32).  RELAXED on purpose: the signal
+// ("this TMEM accumulator has been read out") orders nothing in memory -- tcgen05.wait::ld has already
+// completed the reads.  A .release.cluster arrive compiles to MEMBAR.ALL.GPU, which makes every epilogue
+// warp wait for all of its outstanding global stores before freeing the accumulator (measured: 36 % of
+// all stall samples of the kernel).
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
 }
 __device__ __forceinline__ uint32_t elect_one() {
     uint32_t pred;
@@ -100,6 +120,29 @@ __device__ __forceinline__ void tma_load_3d_2sm(uint32_t dst_smem, const CUtenso
         "%5}], [%2];" ::"r"(dst_smem),
         "l"(reinterpret_cast<uint64_t>(tmap)), "r"(cluster_bar), "r"(c0), "r"(c1), "r"(c2)
         : "memory");
+}
+
+// ---- bulk stores shared -> global (TMA store engine, no tensor map) ------------------------------
+// Generic-proxy writes to shared memory must be made visible to the async proxy before it reads them.
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void bulk_store(void* gdst, uint32_t ssrc, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(ssrc), "r"(bytes) : "memory");
+}
+// global[i] += shared[i] (int32), element-wise, performed in L2
+__device__ __forceinline__ void bulk_reduce_add_s32(void* gdst, uint32_t ssrc, uint32_t bytes) {
+    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.s32 [%0], [%1], %2;" ::"l"(gdst), "r"(ssrc),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// all bulk groups of this thread have finished READING shared memory (the source may be overwritten)
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, int4 v) {
+    asm volatile("st.shared.v4.s32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
 // ---- tcgen05 / TMEM -------------------------------------------------------------------------

@@ -28,10 +28,14 @@ def _built():
 TILE_MODES = [xcb.TILE_1CTA_128x128, xcb.TILE_1CTA_128x256, xcb.TILE_2CTA_256x256]
 
 
-def run_i8(x_np, kernel=xcb.I8_KERNEL_AUTO, force_stage=False, max_ctas=0, tile=xcb.TILE_AUTO):
+EPI_MODES = [xcb.EPI_DIRECT, xcb.EPI_STAGED]
+
+
+def run_i8(x_np, kernel=xcb.I8_KERNEL_AUTO, force_stage=False, max_ctas=0, tile=xcb.TILE_AUTO, epi=xcb.EPI_AUTO):
     T, F, N = x_np.shape[:3]
     p = xcb.Plan(N, F, T)
     p.set_option(xcb.OPT_TILE, tile)
+    p.set_option(xcb.OPT_EPILOGUE, epi)
     p.set_option(xcb.OPT_I8_KERNEL, kernel)
     p.set_option(xcb.OPT_FORCE_STAGE, int(force_stage))
     p.set_option(xcb.OPT_MAX_CTAS, max_ctas)
@@ -89,12 +93,13 @@ SMALL = [(1, 1, 1), (2, 3, 5), (3, 2, 31), (5, 2, 33), (16, 3, 64), (31, 2, 65),
          (257, 1, 64), (300, 1, 33)]
 
 
+@pytest.mark.parametrize("epi", EPI_MODES)
 @pytest.mark.parametrize("tile", TILE_MODES)
 @pytest.mark.parametrize("N,F,T", SMALL)
-def test_small_shapes_tc(N, F, T, tile):
+def test_small_shapes_tc(N, F, T, tile, epi):
     x = wl.full_range(N, F, T, seed=N * 1000 + T)            # whole int8 range incl. -128 (reading 6)
     ref = xo.correlate_i8(x)
-    assert np.array_equal(run_i8(x, xcb.I8_KERNEL_TC, tile=tile), ref)
+    assert np.array_equal(run_i8(x, xcb.I8_KERNEL_TC, tile=tile, epi=epi), ref)
 
 
 @pytest.mark.parametrize("N,F,T", [(1, 1, 1), (5, 2, 33), (33, 2, 129), (100, 2, 57)])
@@ -144,8 +149,9 @@ def test_persistent_schedule_independent_of_cta_count():
     x = wl.gaussian(N, F, T, seed=11, sigma=30.0)
     ref = xo.correlate_i8(x)
     for tile in TILE_MODES:
-        for ctas in (1, 2, 7, 0):
-            assert np.array_equal(run_i8(x, max_ctas=ctas, tile=tile), ref)
+        for epi in EPI_MODES:
+            for ctas in (1, 2, 7, 0):
+                assert np.array_equal(run_i8(x, max_ctas=ctas, tile=tile, epi=epi), ref)
 
 
 def test_accumulate_is_linear_in_time():
@@ -154,13 +160,15 @@ def test_accumulate_is_linear_in_time():
     blocks = [wl.gaussian(N, F, T, seed=20 + k, sigma=20.0) for k in range(3)]
     ref = xo.correlate_i8(np.concatenate(blocks, axis=0))
     for tile in TILE_MODES:
-        p = xcb.Plan(N, F, T)
-        p.set_option(xcb.OPT_TILE, tile)
-        vis = p.correlate(torch.from_numpy(blocks[0]).cuda())
-        for b in blocks[1:]:
-            p.correlate_acc(torch.from_numpy(b).cuda(), vis)
-        torch.cuda.synchronize()
-        assert np.array_equal(vis.cpu().numpy(), ref)
+        for epi in EPI_MODES:
+            p = xcb.Plan(N, F, T)
+            p.set_option(xcb.OPT_TILE, tile)
+            p.set_option(xcb.OPT_EPILOGUE, epi)
+            vis = p.correlate(torch.from_numpy(blocks[0]).cuda())
+            for b in blocks[1:]:
+                p.correlate_acc(torch.from_numpy(b).cuda(), vis)
+            torch.cuda.synchronize()
+            assert np.array_equal(vis.cpu().numpy(), ref), (tile, epi)
 
 
 def test_common_tone_phases_on_gpu():
@@ -277,15 +285,19 @@ def test_full_size_configs(name):
     xd = torch.from_numpy(x).cuda()
     vis = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
     # the other tile shapes must give the very same bits (tile-schedule independence)
+    first = None
     for tile in TILE_MODES:
-        p.set_option(xcb.OPT_TILE, tile)
-        v2 = p.correlate(xd)
-        if tile == TILE_MODES[0]:
-            first = v2
-        else:
-            assert torch.equal(first, v2), (name, tile)
+        for epi in EPI_MODES:
+            p.set_option(xcb.OPT_TILE, tile)
+            p.set_option(xcb.OPT_EPILOGUE, epi)
+            v2 = p.correlate(xd)
+            if first is None:
+                first = v2
+            else:
+                assert torch.equal(first, v2), (name, tile, epi)
     del first, v2
     p.set_option(xcb.OPT_TILE, xcb.TILE_AUTO)           # the launch configuration bench.py times
+    p.set_option(xcb.OPT_EPILOGUE, xcb.EPI_AUTO)
     p.correlate(xd, vis)
     torch.cuda.synchronize()
     # (a) oracle on sampled channels, all baselines
