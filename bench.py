@@ -312,6 +312,65 @@ def main():
             del xx, vv
             torch.cuda.empty_cache()
 
+    # ---- S5 / S6 of the scope table: fp32 variant and two-stream pipeline (rank 0, N=1) -------------
+    extras = {}
+    if rank == 0 and world == 1 and not args.no_sweep:
+        # fp32-input variant on config 3's values (BASELINE.json configs[2]); ALU-bound: peak = SMs x 128 FMA x 2 x f_max
+        w3 = wl.CONFIGS["cfg3"]
+        x3 = torch.from_numpy(wl.make_input(w3)).cuda().to(torch.float32)
+        p3 = xcb.Plan(w3.N, w3.F, w3.T)
+        v3 = p3.new_vis(torch.float32)
+        for _ in range(3):
+            p3.correlate_f32(x3, v3, stream=stream)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        stream.synchronize()
+        ev[0].record(stream)
+        for _ in range(5):
+            p3.correlate_f32(x3, v3, stream=stream)
+        ev[1].record(stream)
+        stream.synchronize()
+        ms = ev[0].elapsed_time(ev[1]) / 5
+        sms = torch.cuda.get_device_properties(0).multi_processor_count
+        fp32_peak = sms * 128 * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+        extras["f32"] = {"workload": "cfg3 values as float32 through xc_correlate_f32", "kernel_ms": ms,
+                         "tflops": w3.ops / (ms * 1e-3) / 1e12, "bound": "alu", "peak_tflops": fp32_peak,
+                         "frac": w3.ops / (ms * 1e-3) / 1e12 / fp32_peak,
+                         "peak_source": "SMs x 128 FMA/clk x 2 x clocks.max.sm (derived, DESIGN.md 5.2)"}
+        p3.close()
+        del x3, v3
+        torch.cuda.empty_cache()
+        # two-stream run of config 5: 8 host blocks (the same seeded block 8 times: only the timing matters here;
+        # parity of the 8-distinct-block run is tests/test_xc_gpu.py::test_cfg5_two_stream_eight_blocks)
+        w5 = wl.CONFIGS["cfg5_N1024"]
+        blk = torch.from_numpy(wl.make_input(w5))
+        host = torch.empty((8,) + tuple(blk.shape), dtype=torch.int8).pin_memory()
+        for k in range(8):
+            host[k].copy_(blk)
+        p5 = xcb.Plan(w5.N, w5.F, w5.T)
+        dev2 = torch.empty(2 * p5.in_bytes, dtype=torch.int8, device="cuda")
+        v5 = p5.new_vis()
+        s2 = torch.cuda.Stream()
+        p5.correlate_pipelined(host, dev2, v5, stream, s2)
+        stream.synchronize()
+        t0 = time.perf_counter()
+        p5.correlate_pipelined(host, dev2, v5, stream, s2)
+        stream.synchronize()
+        tot = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        for k in range(8):
+            dev2[:p5.in_bytes].view(torch.int8).copy_(host[k].view(-1), non_blocking=True)
+        torch.cuda.synchronize()
+        t_copy = time.perf_counter() - t0
+        xk = dev2[:p5.in_bytes].view(w5.T, w5.F, w5.N, 2, 2)
+        t_comp = 8e-3 * sorted(time_kernel(p5, xk, v5, stream, 5, 2))[2]
+        extras["two_stream"] = {"workload": "cfg5_N1024 x 8 pinned host blocks, xc_correlate_pipelined (Algorithm 1)",
+                                "total_ms": 1e3 * tot, "copy_alone_ms": 1e3 * t_copy, "compute_alone_ms": 1e3 * t_comp,
+                                "h2d_gbs": 8 * w5.in_bytes / tot / 1e9, "tops": 8 * w5.ops / tot / 1e12,
+                                "overlap_efficiency": max(t_copy, t_comp) / tot}
+        p5.close()
+        del host, dev2, v5
+        torch.cuda.empty_cache()
+
     # ---- CPU baseline: the oracle on a bounded sample (rank 0 at N=1 only) --------------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
@@ -329,7 +388,7 @@ def main():
                        "l2": "input block (%.0f MB) + output (%.0f MB) exceed the 126 MB L2: every step is cold"
                              % (w.in_bytes / 1e6, w.vis_bytes / 1e6)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * launches_per_step,
-            "roofline": roof, "cpu_baseline": cpu, "by_config": by_config,
+            "roofline": roof, "cpu_baseline": cpu, "by_config": by_config, "extras": extras,
             "frac_of_int8_peak": tops / world / i8_peak, "int8_peak_tops": i8_peak,
             "paper_context": "1058 GFLOPS = 79% of fp32 peak on a GeForce GTX 480 (PAPER.md:267); other hardware",
         }

@@ -113,7 +113,8 @@ size_t xc_vis_bytes(const xc_plan_t* plan);     /* 32*NB*F (int32 and float alik
 size_t xc_n_baselines(const xc_plan_t* plan);
 
 /* Staging.  The tensor-core kernel reads the input through TMA, which
- * needs a 16-byte-aligned base and 16-byte-multiple row pitch (4N bytes -> N % 4 == 0).
+ * needs a 16-byte-aligned base and 16-byte-multiple row pitch (4N bytes -> N % 4 == 0); for N >= 192 the
+ * library also re-pitches rows to a multiple of 128 bytes (N % 32 == 0) because that doubles the fill rate.
  * Otherwise the input is first copied by a padding kernel into a workspace of
  * xc_workspace_bytes() bytes (0 when never needed).  The caller may hand one in (device
  * memory, 128-byte aligned, kept until xc_destroy or replaced); if none was set the

@@ -173,7 +173,7 @@ int ensure_device(xc_plan_t* p) {
 
 // S0: decide whether the padding kernel is needed and run it; *src / *nrow describe what TMA reads.
 int stage_if_needed(xc_plan_t* p, const int8_t* in_dev, cudaStream_t st, const void** src, int* nrow) {
-    const bool need = p->opt_force_stage || (p->N % 4 != 0) || (reinterpret_cast<uintptr_t>(in_dev) & 15u);
+    const bool need = p->opt_force_stage || (p->Npad != p->N) || (reinterpret_cast<uintptr_t>(in_dev) & 15u);
     if (!need) {
         *src = in_dev;
         *nrow = p->N;
@@ -190,8 +190,13 @@ int stage_if_needed(xc_plan_t* p, const int8_t* in_dev, cudaStream_t st, const v
     const long long total = rows * p->Npad;
     long long blocks = (total + 255) / 256;
     if (blocks > 148LL * 32) blocks = 148LL * 32;
-    xc::xc_stage_pad_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in_dev, static_cast<uint32_t*>(p->ws), rows,
-                                                                             p->N, p->Npad);
+    if (p->N % 4 == 0 && !(reinterpret_cast<uintptr_t>(in_dev) & 15u)) {
+        xc::xc_stage_pad16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(
+            reinterpret_cast<const uint4*>(in_dev), static_cast<uint4*>(p->ws), rows, p->N / 4, p->Npad / 4);
+    } else {
+        xc::xc_stage_pad_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in_dev, static_cast<uint32_t*>(p->ws), rows,
+                                                                                 p->N, p->Npad);
+    }
     XC_CUDA(p, cudaGetLastError());
     p->last_launches += 1;
     *src = p->ws;
@@ -297,7 +302,9 @@ int xc_plan(xc_plan_t** out, int N, int P, int F, int T, int layout) {
     p->F = F;
     p->T = T;
     p->NB = static_cast<long long>(N) * (N + 1) / 2;
-    p->Npad = (N + 3) & ~3;
+    // Row pitch seen by TMA: a multiple of 16 bytes is mandatory (N % 4 == 0); for large N a multiple of 128 bytes
+    // (N % 32 == 0) is worth a staging pass, because a box row that straddles two 128-byte lines halves the fill rate.
+    p->Npad = (N >= 192 && N % 32 != 0) ? ((N + 31) & ~31) : ((N + 3) & ~3);
     set_tile_mode(p, XC_TILE_AUTO);
     p->tiles_f32 = build_tiles(N, xc::F32_SI, xc::F32_SJ);
     memset(&p->tmap, 0, sizeof p->tmap);
