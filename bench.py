@@ -270,6 +270,25 @@ def main():
                  "other_roof_frac": (w.ops / (k_ms * 1e-3) / 1e12 / i8_peak) if roof["bound"] == "hbm"
                  else (alg_bytes / (k_ms * 1e-3) / 1e9 / peaks["hbm_gbs"])})
 
+    # ---- the SM clock the kernel REALLY ran at: CTA 0 stamps (clock64, globaltimer) at start and end ----------
+    # (NVML keeps reporting clocks.max.sm while the chip's power management already runs the tensor-heavy kernel
+    # slower; measured 1.2-1.6 GHz.  Reported beside the NVML figures, which stay in the contract's keys.)
+    probe = torch.zeros(xcb.TRACE_WORDS, dtype=torch.int64, device="cuda")
+    p.set_trace(probe)
+    mhz = []
+    with torch.cuda.stream(stream):
+        for _ in range(20):
+            p.correlate(xd, vis, stream=stream)
+            stream.synchronize()
+            t4 = probe[-4:].tolist()
+            if t4[3] > t4[1]:
+                mhz.append((t4[2] - t4[0]) / (t4[3] - t4[1]) * 1e3)
+    p.set_trace(None)
+    mhz.sort()
+    clocks["sm_mhz_in_kernel"] = mhz[len(mhz) // 2] if mhz else None
+    clocks["sm_mhz_in_kernel_how"] = ("clock64 / globaltimer stamped by CTA 0 of xc_i8_tc_kernel at its start and end, "
+                                      "median of 20 back-to-back launches after the timed region")
+
     # ---- end to end through the C ABI with HOST buffers ---------------------------------------
     vh = torch.empty(p.vis_shape(), dtype=torch.int32).pin_memory()
     e2e_steps = max(3, min(args.steps, 10))

@@ -89,6 +89,7 @@ typedef enum {
     XC_OPT_FORCE_STAGE = 2, /* 1 = always run the staging (pad/copy) kernel, for testing S0    */
     XC_OPT_TILE = 4,       /* one of XC_TILE_*; rebuilds the tile schedule (synchronising on next call) */
     XC_OPT_EPILOGUE = 5,   /* one of XC_EPI_*                                                  */
+    XC_OPT_BK = 6,         /* samples per pipeline stage of the CTA-pair kernel: 0 (auto), 128 or 256 */
     XC_OPT_DEBUG_SKIP = 3  /* PROFILING ONLY, results become meaningless: bit 0 = no TMA loads  */
                            /* after the first ring fill, bit 1 = no MMAs, bit 2 = no stores     */
 } xc_option;
@@ -160,9 +161,10 @@ int xc_correlate_pipelined(xc_plan_t* plan, const int8_t* in_host_pinned, int n_
 int xc_correlate_host(xc_plan_t* plan, const int8_t* in_host, int32_t* vis_host, int8_t* in_dev_scratch,
                       int32_t* vis_dev_scratch, void* cuda_stream);
 
-/* PROFILING ONLY: trace_dev = device buffer of 3*256*4 int64 (or NULL to switch off); CTA 0 of the
+/* PROFILING ONLY: trace_dev = device buffer of 3*256*4 + 4 int64 (or NULL to switch off); CTA 0 of the
  * tensor-core kernel writes clock64() stamps of its first 256 pipeline iterations per warp role
- * (0 = TMA producer, 1 = MMA issuer, 2 = epilogue) into it. */
+ * (0 = TMA producer, 1 = MMA issuer, 2 = epilogue) into it (CTA-pair kernel only), and every tensor-core kernel
+ * writes {clock64, globaltimer} at its start and end into the last 4 words (effective SM clock of the launch). */
 int xc_debug_set_trace(xc_plan_t* plan, void* trace_dev);
 
 /* Tile schedule introspection (for tests of the triangular map).

@@ -12,8 +12,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libxc.so")
 
 MAX_T = 65535
+TRACE_WORDS = 3 * 256 * 4 + 4
 I8_KERNEL_AUTO, I8_KERNEL_TC, I8_KERNEL_SIMT = 0, 1, 2
-OPT_I8_KERNEL, OPT_MAX_CTAS, OPT_FORCE_STAGE, OPT_DEBUG_SKIP, OPT_TILE, OPT_EPILOGUE = 0, 1, 2, 3, 4, 5
+OPT_I8_KERNEL, OPT_MAX_CTAS, OPT_FORCE_STAGE, OPT_DEBUG_SKIP, OPT_TILE, OPT_EPILOGUE, OPT_BK = 0, 1, 2, 3, 4, 5, 6
 EPI_AUTO, EPI_DIRECT, EPI_STAGED = 0, 1, 2
 TILE_AUTO, TILE_1CTA_128x128, TILE_1CTA_128x256, TILE_2CTA_256x256 = 0, 1, 2, 3
 
@@ -182,6 +183,12 @@ class Plan:
                                           ctypes.byref(sj)), "xc_tile_get")
             out.append((bi.value, bj.value, si.value, sj.value))
         return out
+
+    def set_trace(self, buf) -> None:
+        """PROFILING ONLY: buf = int64 CUDA tensor of TRACE_WORDS elements (or None): see xc_debug_set_trace."""
+        self._check(lib().xc_debug_set_trace(self._h, ctypes.c_void_p(buf.data_ptr() if buf is not None else 0)),
+                    "xc_debug_set_trace")
+        self._trace = buf
 
     # compute -------------------------------------------------------------------------------
     def _chk_in(self, x, dtype):

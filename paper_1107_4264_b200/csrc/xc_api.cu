@@ -56,7 +56,7 @@ struct xc_plan_s {
     void* ws = nullptr;
     size_t ws_bytes = 0;
     bool ws_owned = false;
-    int opt_kernel = XC_I8_KERNEL_AUTO, opt_max_ctas = 0, opt_force_stage = 0, opt_debug_skip = 0, opt_epilogue = 0;
+    int opt_kernel = XC_I8_KERNEL_AUTO, opt_max_ctas = 0, opt_force_stage = 0, opt_debug_skip = 0, opt_epilogue = 0, opt_bk = 0;
     long long* trace = nullptr;
     CUtensorMap tmap;
     const void* tmap_src = nullptr;
@@ -112,7 +112,7 @@ int upload_tiles(xc_plan_t* p) {
     return XC_OK;
 }
 
-template <int UMMA_N, int CG, bool STAGED>
+template <int UMMA_N, int CG, bool STAGED, int BK = 128>
 int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
     long long units = (p->opt_max_ctas > 0 ? p->opt_max_ctas : p->sm_count) / CG;
     if (units < 1) units = 1;
@@ -120,7 +120,7 @@ int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(units * CG));
     cfg.blockDim = dim3(xc::TC_THREADS);
-    cfg.dynamicSmemBytes = xc::TcCfg<UMMA_N, CG, STAGED>::SMEM_BYTES;
+    cfg.dynamicSmemBytes = xc::TcCfg<UMMA_N, CG, STAGED, BK>::SMEM_BYTES;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -129,10 +129,11 @@ int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    auto kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, false>;
-    if (CG == 2 && UMMA_N == 256 && tp.trace) kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, (CG == 2 && UMMA_N == 256)>;
+    auto kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, false, BK>;
+    if (CG == 2 && UMMA_N == 256 && BK == 128 && tp.trace)
+        kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, (CG == 2 && UMMA_N == 256 && BK == 128), BK>;
     XC_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    xc::TcCfg<UMMA_N, CG, STAGED>::SMEM_BYTES));
+                                    xc::TcCfg<UMMA_N, CG, STAGED, BK>::SMEM_BYTES));
     XC_CUDA(p, cudaLaunchKernelEx(&cfg, kern, p->tmap, tp));
     return XC_OK;
 }
@@ -251,9 +252,9 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     int nrow = 0;
     rc = stage_if_needed(p, in_dev, st, &src, &nrow);
     if (rc != XC_OK) return rc;
-    const int bk = p->tile_mode == XC_TILE_2CTA_256x256   ? xc::TcCfg<256, 2, false>::BK
-                   : p->tile_mode == XC_TILE_1CTA_128x256 ? xc::TcCfg<256, 1, false>::BK
-                                                          : xc::TcCfg<128, 1, false>::BK;
+    const bool bkopt = p->tile_mode == XC_TILE_2CTA_256x256 && p->opt_epilogue != XC_EPI_STAGED;
+    const bool bk256 = bkopt && p->opt_bk == 256, bk64 = bkopt && p->opt_bk == 64;
+    const int bk = bk256 ? 256 : (bk64 ? 64 : 128);
     rc = encode_tmap(p, src, nrow, bk);
     if (rc != XC_OK) return rc;
 
@@ -274,7 +275,9 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     tp.trace = p->trace;
     const bool staged = p->opt_epilogue == XC_EPI_STAGED;   // AUTO = direct stores (measured faster)
     if (p->tile_mode == XC_TILE_2CTA_256x256)
-        rc = staged ? launch_tc<256, 2, true>(p, tp, st) : launch_tc<256, 2, false>(p, tp, st);
+        rc = staged ? launch_tc<256, 2, true>(p, tp, st)
+                    : (bk256 ? launch_tc<256, 2, false, 256>(p, tp, st)
+                             : (bk64 ? launch_tc<256, 2, false, 64>(p, tp, st) : launch_tc<256, 2, false>(p, tp, st)));
     else if (p->tile_mode == XC_TILE_1CTA_128x256)
         rc = staged ? launch_tc<256, 1, true>(p, tp, st) : launch_tc<256, 1, false>(p, tp, st);
     else
@@ -360,6 +363,10 @@ int xc_set_option(xc_plan_t* p, int option, int value) {
         case XC_OPT_TILE:
             if (value < XC_TILE_AUTO || value > XC_TILE_2CTA_256x256) return XC_ERR_INVALID_ARG;
             set_tile_mode(p, value);
+            return XC_OK;
+        case XC_OPT_BK:
+            if (value != 0 && value != 64 && value != 128 && value != 256) return XC_ERR_INVALID_ARG;
+            p->opt_bk = value;
             return XC_OK;
         case XC_OPT_EPILOGUE:
             if (value < XC_EPI_AUTO || value > XC_EPI_STAGED) return XC_ERR_INVALID_ARG;

@@ -39,14 +39,14 @@ constexpr int TC_EPI_WARPS = 8;     // 2 per TMEM lane quarter, each owning half
 constexpr int TC_THREADS = 64 + 32 * TC_EPI_WARPS;   // + TMA producer warp + MMA issuer warp
 constexpr int TC_SMEM_LIMIT = 232448;  // 227 KB
 
-template <int UMMA_N, int CG, bool STAGED>
+template <int UMMA_N, int CG, bool STAGED, int BK_ = 128>
 struct TcCfg {
     static constexpr int M = 128 * CG;                    // Gram rows per tile
     static constexpr int B_BOXES = UMMA_N / 128 / CG;     // 128-row B boxes held by one CTA
     // Samples per pipeline stage.  Every stage costs the producer and the MMA issuer some hundred cycles of
     // barrier round trips and instruction issue (measured), so a stage must hold clearly more than that in
     // tensor work (128 cycles per 32 samples).  192-sample stages (4 of them) measured slower than 128 x 7.
-    static constexpr int BK = 128;
+    static constexpr int BK = BK_;
     static constexpr int BOX_BYTES = BK * 128;            // one TMA box: BK rows of 128 bytes
     static constexpr int A_BYTES = BOX_BYTES;
     static constexpr int B_BYTES = B_BOXES * BOX_BYTES;
@@ -61,7 +61,7 @@ struct TcCfg {
     static constexpr int SMEM_BYTES = BAR_BYTES + STAGES * STAGE_BYTES + OUT_BYTES + 1024;  // + slack for 1024-B alignment
     static_assert(B_BOXES >= 1, "a CTA holds at least one 128-row B box");
     static_assert(SMEM_BYTES <= TC_SMEM_LIMIT, "smem");
-    static_assert(STAGES >= 3, "ring too shallow");
+    static_assert(STAGES >= 2, "ring too shallow");
 };
 
 struct TcParams {
@@ -76,7 +76,7 @@ struct TcParams {
                               // 2 = no MMA, 4 = no global stores; results are then meaningless
     long long* trace;         // profiling only: CTA 0 writes clock64() stamps here (see TC_TRACE_*), or null
 };
-constexpr int TC_TRACE_ITERS = 256;   // k-blocks traced; layout: [3 roles][TC_TRACE_ITERS][4] long long
+constexpr int TC_TRACE_ITERS = 256;   // k-blocks traced; layout: [3 roles][TC_TRACE_ITERS][4] long long + 4 clock words
 
 // Epilogue for one 32-column chunk (8 stations j) held in v[]: complex combine, mask, store.
 // Thread <-> Gram row r = (i, pi, ci): lanes 4s..4s+3 of a warp are one station i; ci = 0 holds
@@ -144,10 +144,10 @@ __device__ __forceinline__ void epi_chunk_smem(const uint32_t (&v)[32], uint32_t
     }
 }
 
-template <int UMMA_N, int CG, bool STAGED, bool TRACE = false>
+template <int UMMA_N, int CG, bool STAGED, bool TRACE = false, int BK_ = 128>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
-    using Cfg = TcCfg<UMMA_N, CG, STAGED>;
+    using Cfg = TcCfg<UMMA_N, CG, STAGED, BK_>;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // Barriers first, operand ring after, on a 1024-byte boundary (SWIZZLE_128B atoms).
     const uint32_t bar0 = smem_u32(smem_raw);
@@ -188,6 +188,14 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
     const uint32_t tmem_base = *tmem_slot;
 
     const int KB = (p.T + Cfg::BK - 1) / Cfg::BK;
+    // profiling only: CTA 0 records (SM cycle counter, global nanosecond timer) at start and end, from which the
+    // caller derives the SM clock the kernel really ran at (trace[3 * TC_TRACE_ITERS * 4 + 0..3])
+    if (p.trace && blockIdx.x == 0 && threadIdx.x == 0) {
+        unsigned long long gt;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+        p.trace[3 * TC_TRACE_ITERS * 4 + 0] = clock64();
+        p.trace[3 * TC_TRACE_ITERS * 4 + 1] = static_cast<long long>(gt);
+    }
 
     if (warp == 0) {
         // ===== TMA producer: the whole warp walks the loop, one elected lane issues =====
@@ -379,6 +387,12 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
         }
     }
 
+    if (p.trace && blockIdx.x == 0 && threadIdx.x == 64) {   // an epilogue thread: it finishes last
+        unsigned long long gt;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+        p.trace[3 * TC_TRACE_ITERS * 4 + 2] = clock64();
+        p.trace[3 * TC_TRACE_ITERS * 4 + 3] = static_cast<long long>(gt);
+    }
     if (STAGED && warp >= 2 && warp < 4) bulk_wait0();   // the CTA's shared memory must outlive its bulk stores
     // Teardown: nobody leaves (or frees TMEM) while the peer may still signal into this CTA.
     tc_fence_before();
