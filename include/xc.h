@@ -75,7 +75,13 @@ enum {
     XC_TILE_AUTO = 0,         /* chosen from N at plan time                                        */
     XC_TILE_1CTA_128x128 = 1, /* 32 x 32 stations on one CTA (small N)                             */
     XC_TILE_1CTA_128x256 = 2, /* 32 x 64 stations on one CTA                                       */
-    XC_TILE_2CTA_256x256 = 3  /* 64 x 64 stations on a CTA pair (tcgen05 cta_group::2)             */
+    XC_TILE_2CTA_256x256 = 3, /* 64 x 64 stations on a CTA pair (tcgen05 cta_group::2)             */
+    XC_TILE_SPLIT = 4,        /* two launches: every diagonal 64-station block on ONE CTA as two sub-tiles  */
+                              /* (32 x 64 stations, then 32 x 32: the block's i > j quarter is never      */
+                              /* computed), every off-diagonal 64 x 64 block on a CTA pair (reads the      */
+                              /* input from HBM twice: kept for testing)                                   */
+    XC_TILE_MIXED = 5         /* the same schedule in ONE launch: some clusters work as two single CTAs on  */
+                              /* diagonal blocks, the others as CTA pairs on off-diagonal blocks            */
 };
 /* Epilogue store path of the tensor-core kernel, xc_set_option(XC_OPT_EPILOGUE, ...). */
 enum {

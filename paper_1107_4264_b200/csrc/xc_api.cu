@@ -6,6 +6,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -39,6 +40,46 @@ std::vector<uint32_t> build_tiles(int N, int si, int sj) {
     return t;
 }
 
+// XC_TILE_SPLIT, diagonal part: per 64-station diagonal block k two single-CTA sub-tiles, rows 2k (32 stations)
+// against both 32-station column boxes of block k, and rows 2k+1 against the second box only (padding entry
+// 0xFFFFFFFF where that row block starts beyond N).  Always two entries per k: the kernel walks them as a group.
+std::vector<uint32_t> build_tiles_diag(int N) {
+    std::vector<uint32_t> t;
+    const int nb = (N + 63) / 64;
+    for (int k = 0; k < nb; ++k) {
+        t.push_back(static_cast<uint32_t>(2 * k) | (static_cast<uint32_t>(k) << 16));
+        t.push_back((2 * k + 1) * 32 < N ? (static_cast<uint32_t>(2 * k + 1) | (static_cast<uint32_t>(k) << 16)) : 0xFFFFFFFFu);
+    }
+    return t;
+}
+// XC_TILE_SPLIT, off-diagonal part: the 64 x 64-station blocks strictly below the diagonal (bi < bj), CTA pairs.
+std::vector<uint32_t> build_tiles_off(int N) {
+    std::vector<uint32_t> t;
+    const int nb = (N + 63) / 64;
+    for (int bj = 0; bj < nb; ++bj)
+        for (int bi = 0; bi < bj; ++bi) t.push_back(static_cast<uint32_t>(bi) | (static_cast<uint32_t>(bj) << 16));
+    return t;
+}
+
+// XC_TILE_MIXED: how many of the `clusters` 2-CTA clusters work as two single CTAs on diagonal blocks (3 time units
+// per block per CTA); the others work as pairs on off-diagonal tiles (2 units per tile).  Minimises the modelled
+// makespan; *t_out receives it.
+int mixed_split(int N, int F, int clusters, double* t_out) {
+    const double gd = static_cast<double>((N + 63) / 64) * F;
+    const double go = static_cast<double>(build_tiles_off(N).size()) * F;
+    int best_n = clusters;
+    double best_t = std::ceil(gd / (2.0 * clusters)) * 3.0;
+    if (go > 0) {
+        best_t = 1e300;
+        for (int n = 1; n < clusters; ++n) {
+            const double t = std::max(std::ceil(gd / (2.0 * n)) * 3.0, std::ceil(go / (clusters - n)) * 2.0);
+            if (t < best_t) { best_t = t; best_n = n; }
+        }
+    }
+    if (t_out) *t_out = best_t;
+    return best_n;
+}
+
 }  // namespace
 
 struct xc_plan_s {
@@ -47,10 +88,12 @@ struct xc_plan_s {
     int Npad = 0;
     int tile_mode = 0;  // XC_TILE_*: shape of the tensor-core tile actually in use
     std::vector<uint32_t> tiles_tc, tiles_f32;
+    std::vector<uint32_t> tiles_diag;   // XC_TILE_SPLIT: diagonal sub-tiles (tiles_tc then holds the off-diagonal pair tiles)
     // device state (created lazily on the device current at first compute call)
     bool dev_ready = false, tiles_uploaded = false;
     int device = -1, sm_count = 0;
     uint32_t* d_tiles_tc = nullptr;
+    uint32_t* d_tiles_diag = nullptr;
     uint32_t* d_tiles_f32 = nullptr;
     PFN_encodeTiled encode = nullptr;
     void* ws = nullptr;
@@ -80,47 +123,68 @@ int cuda_fail(xc_plan_t* p, cudaError_t e, const char* where) {
     } while (0)
 
 void tile_shape(int mode, int* si, int* sj) {
-    *si = (mode == XC_TILE_2CTA_256x256) ? 64 : 32;
+    *si = (mode == XC_TILE_2CTA_256x256 || mode == XC_TILE_SPLIT || mode == XC_TILE_MIXED) ? 64 : 32;
     *sj = (mode == XC_TILE_1CTA_128x128) ? 32 : 64;
 }
 
 // S1: pick the tensor-core tile and build its per-channel schedule.
 void set_tile_mode(xc_plan_t* p, int mode) {
     if (mode == XC_TILE_AUTO) {
-        // CTA-pair 256x256 tiles halve the shared-memory traffic per MMA and are the default; the
-        // narrow single-CTA tile only wins when it wastes clearly less of the tensor pipe on the
-        // diagonal (small N).
-        const double a2 = 65536.0 * build_tiles(p->N, 64, 64).size();
-        const double a1 = 16384.0 * build_tiles(p->N, 32, 32).size();
-        mode = (a1 < 0.6 * a2) ? XC_TILE_1CTA_128x128 : XC_TILE_2CTA_256x256;
+        // Modelled in units of "one 128 x 128 Gram block over the whole integration on one SM" (the paper's wasted-work
+        // model, per SM): a CTA-pair 256x256 tile is 4 blocks on 2 SMs = 2 time units; single-CTA
+        // 128x128 tiles are 1 unit each but fill-bound (measured ~1.25x slower per block), so they only serve tiny
+        // problems.  XC_TILE_MIXED / XC_TILE_SPLIT compute 5-17 % fewer blocks but measured 15-25 % SLOWER (their
+        // single-CTA workers are bound by the per-stage barrier round trip and the epilogue): never AUTO.
+        const double sms = 148.0;
+        const double n2 = static_cast<double>(build_tiles(p->N, 64, 64).size()) * p->F;
+        const double n1 = static_cast<double>(build_tiles(p->N, 32, 32).size()) * p->F;
+        const double t_pair = std::ceil(n2 / (sms / 2)) * 2.0;
+        const double t_solo = std::ceil(n1 / sms) * 1.25;
+        mode = (t_solo < 0.8 * t_pair) ? XC_TILE_1CTA_128x128 : XC_TILE_2CTA_256x256;
     }
     int si, sj;
     tile_shape(mode, &si, &sj);
     p->tile_mode = mode;
-    p->tiles_tc = build_tiles(p->N, si, sj);
+    if (mode == XC_TILE_SPLIT || mode == XC_TILE_MIXED) {
+        p->tiles_tc = build_tiles_off(p->N);
+        p->tiles_diag = build_tiles_diag(p->N);
+    } else {
+        p->tiles_tc = build_tiles(p->N, si, sj);
+        p->tiles_diag.clear();
+    }
     p->tiles_uploaded = false;
+}
+
+int upload_table(xc_plan_t* p, uint32_t** dst, const std::vector<uint32_t>& src) {
+    if (*dst) XC_CUDA(p, cudaFree(*dst));   // synchronising; only after xc_set_option(XC_OPT_TILE)
+    *dst = nullptr;
+    if (src.empty()) return XC_OK;
+    XC_CUDA(p, cudaMalloc(dst, src.size() * sizeof(uint32_t)));
+    XC_CUDA(p, cudaMemcpy(*dst, src.data(), src.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    return XC_OK;
 }
 
 int upload_tiles(xc_plan_t* p) {
     if (p->tiles_uploaded) return XC_OK;
-    if (p->d_tiles_tc) XC_CUDA(p, cudaFree(p->d_tiles_tc));   // synchronising; only after xc_set_option(XC_OPT_TILE)
-    p->d_tiles_tc = nullptr;
-    XC_CUDA(p, cudaMalloc(&p->d_tiles_tc, p->tiles_tc.size() * sizeof(uint32_t)));
-    XC_CUDA(p, cudaMemcpy(p->d_tiles_tc, p->tiles_tc.data(), p->tiles_tc.size() * sizeof(uint32_t),
-                          cudaMemcpyHostToDevice));
+    int rc = upload_table(p, &p->d_tiles_tc, p->tiles_tc);
+    if (rc != XC_OK) return rc;
+    rc = upload_table(p, &p->d_tiles_diag, p->tiles_diag);
+    if (rc != XC_OK) return rc;
     p->tiles_uploaded = true;
     return XC_OK;
 }
 
-template <int UMMA_N, int CG, bool STAGED, int BK = 128>
+template <int UMMA_N, int CG, bool STAGED, int BK = 128, bool DIAG = false>
 int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
+    using Cfg = xc::TcCfg<UMMA_N, CG, STAGED, BK, DIAG>;
     long long units = (p->opt_max_ctas > 0 ? p->opt_max_ctas : p->sm_count) / CG;
     if (units < 1) units = 1;
-    if (units > tp.total_tiles) units = tp.total_tiles;
+    const long long groups = tp.total_tiles >> tp.group_shift;
+    if (units > groups) units = groups;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(units * CG));
     cfg.blockDim = dim3(xc::TC_THREADS);
-    cfg.dynamicSmemBytes = xc::TcCfg<UMMA_N, CG, STAGED, BK>::SMEM_BYTES;
+    cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -129,12 +193,12 @@ int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    auto kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, false, BK>;
+    auto kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, false, BK, DIAG>;
     if (CG == 2 && UMMA_N == 256 && BK == 128 && tp.trace)
-        kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, (CG == 2 && UMMA_N == 256 && BK == 128), BK>;
-    XC_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    xc::TcCfg<UMMA_N, CG, STAGED, BK>::SMEM_BYTES));
+        kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, (CG == 2 && UMMA_N == 256 && BK == 128), BK, DIAG>;
+    XC_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
     XC_CUDA(p, cudaLaunchKernelEx(&cfg, kern, p->tmap, tp));
+    p->last_launches += 1;
     return XC_OK;
 }
 
@@ -151,10 +215,9 @@ int ensure_device(xc_plan_t* p) {
     }
     p->device = dev;
     p->sm_count = sms;
-    XC_CUDA(p, cudaMalloc(&p->d_tiles_tc, p->tiles_tc.size() * sizeof(uint32_t)));
-    XC_CUDA(p, cudaMemcpy(p->d_tiles_tc, p->tiles_tc.data(), p->tiles_tc.size() * sizeof(uint32_t),
-                          cudaMemcpyHostToDevice));
-    p->tiles_uploaded = true;
+    p->tiles_uploaded = false;
+    int rc_up = upload_tiles(p);
+    if (rc_up != XC_OK) return rc_up;
     XC_CUDA(p, cudaMalloc(&p->d_tiles_f32, p->tiles_f32.size() * sizeof(uint32_t)));
     XC_CUDA(p, cudaMemcpy(p->d_tiles_f32, p->tiles_f32.data(), p->tiles_f32.size() * sizeof(uint32_t),
                           cudaMemcpyHostToDevice));
@@ -264,16 +327,66 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     tp.N = p->N;
     tp.F = p->F;
     tp.T = p->T;
-    tp.tiles_per_f = static_cast<int>(p->tiles_tc.size());
-    if (static_cast<long long>(p->F) * tp.tiles_per_f > 0x7FFFFFFFLL) return XC_ERR_UNSUPPORTED;
-    tp.total_tiles = p->F * tp.tiles_per_f;
     tp.NB = p->NB;
-    tp.tiles = p->d_tiles_tc;
     tp.vis = vis_dev;
     tp.accumulate = accumulate;
     tp.debug_skip = p->opt_debug_skip;
     tp.trace = p->trace;
+    auto set_table = [&](const std::vector<uint32_t>& host, const uint32_t* dev, int group_shift) {
+        tp.tiles_per_f = static_cast<int>(host.size());
+        tp.tiles = dev;
+        tp.group_shift = group_shift;
+        if (static_cast<long long>(p->F) * tp.tiles_per_f > 0x7FFFFFFFLL) return false;
+        tp.total_tiles = p->F * tp.tiles_per_f;
+        return true;
+    };
     const bool staged = p->opt_epilogue == XC_EPI_STAGED;   // AUTO = direct stores (measured faster)
+    if (p->tile_mode == XC_TILE_MIXED) {
+        // one launch, clusters of 2: some clusters are two single-CTA diagonal workers, the others are CTA pairs
+        xc::TcParams td = tp;
+        if (!set_table(p->tiles_diag, p->d_tiles_diag, 1)) return XC_ERR_UNSUPPORTED;
+        td = tp;
+        xc::TcParams to = tp;
+        to.total_tiles = 0;
+        if (!p->tiles_tc.empty()) {
+            if (!set_table(p->tiles_tc, p->d_tiles_tc, 0)) return XC_ERR_UNSUPPORTED;
+            to = tp;
+        }
+        int clusters = (p->opt_max_ctas > 0 ? p->opt_max_ctas : p->sm_count) / 2;
+        if (clusters < 2) clusters = 2;
+        const int n_solo = p->tiles_tc.empty() ? clusters : mixed_split(p->N, p->F, clusters, nullptr);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(static_cast<unsigned>(2 * clusters));
+        cfg.blockDim = dim3(xc::TC_THREADS);
+        cfg.dynamicSmemBytes = xc::TcCfg<256, 2, false, 128, false>::SMEM_BYTES;
+        static_assert(xc::TcCfg<256, 2, false, 128, false>::SMEM_BYTES == xc::TcCfg<256, 1, false, 128, true>::SMEM_BYTES,
+                      "both worker kinds of the mixed kernel use the same ring");
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        XC_CUDA(p, cudaFuncSetAttribute(xc::xc_i8_tc_mixed_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        static_cast<int>(cfg.dynamicSmemBytes)));
+        XC_CUDA(p, cudaLaunchKernelEx(&cfg, xc::xc_i8_tc_mixed_kernel, p->tmap, td, to, n_solo));
+        p->last_launches += 1;
+        return XC_OK;
+    }
+    if (p->tile_mode == XC_TILE_SPLIT) {
+        // two launches with disjoint outputs: diagonal 64-station blocks on single CTAs, the rest on CTA pairs
+        if (!set_table(p->tiles_diag, p->d_tiles_diag, 1)) return XC_ERR_UNSUPPORTED;
+        rc = launch_tc<256, 1, false, 128, true>(p, tp, st);
+        if (rc != XC_OK) return rc;
+        if (!p->tiles_tc.empty()) {
+            if (!set_table(p->tiles_tc, p->d_tiles_tc, 0)) return XC_ERR_UNSUPPORTED;
+            rc = staged ? launch_tc<256, 2, true>(p, tp, st) : launch_tc<256, 2, false>(p, tp, st);
+        }
+        return rc;
+    }
+    if (!set_table(p->tiles_tc, p->d_tiles_tc, 0)) return XC_ERR_UNSUPPORTED;
     if (p->tile_mode == XC_TILE_2CTA_256x256)
         rc = staged ? launch_tc<256, 2, true>(p, tp, st)
                     : (bk256 ? launch_tc<256, 2, false, 256>(p, tp, st)
@@ -282,9 +395,7 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
         rc = staged ? launch_tc<256, 1, true>(p, tp, st) : launch_tc<256, 1, false>(p, tp, st);
     else
         rc = staged ? launch_tc<128, 1, true>(p, tp, st) : launch_tc<128, 1, false>(p, tp, st);
-    if (rc != XC_OK) return rc;
-    p->last_launches += 1;
-    return XC_OK;
+    return rc;
 }
 
 }  // namespace
@@ -318,6 +429,7 @@ int xc_plan(xc_plan_t** out, int N, int P, int F, int T, int layout) {
 void xc_destroy(xc_plan_t* p) {
     if (!p) return;
     if (p->d_tiles_tc) cudaFree(p->d_tiles_tc);
+    if (p->d_tiles_diag) cudaFree(p->d_tiles_diag);
     if (p->d_tiles_f32) cudaFree(p->d_tiles_f32);
     if (p->ws && p->ws_owned) cudaFree(p->ws);
     for (int k = 0; k < 2; ++k) {
@@ -361,7 +473,7 @@ int xc_set_option(xc_plan_t* p, int option, int value) {
             p->opt_force_stage = value ? 1 : 0;
             return XC_OK;
         case XC_OPT_TILE:
-            if (value < XC_TILE_AUTO || value > XC_TILE_2CTA_256x256) return XC_ERR_INVALID_ARG;
+            if (value < XC_TILE_AUTO || value > XC_TILE_MIXED) return XC_ERR_INVALID_ARG;
             set_tile_mode(p, value);
             return XC_OK;
         case XC_OPT_BK:
@@ -469,14 +581,29 @@ int xc_debug_set_trace(xc_plan_t* p, void* trace_dev) {
     return XC_OK;
 }
 
-int xc_tile_count(const xc_plan_t* p) { return p ? static_cast<int>(p->tiles_tc.size()) : 0; }
+int xc_tile_count(const xc_plan_t* p) {
+    if (!p) return 0;
+    int n = static_cast<int>(p->tiles_tc.size());
+    for (uint32_t e : p->tiles_diag) n += (e != 0xFFFFFFFFu);
+    return n;
+}
 
 int xc_tile_get(const xc_plan_t* p, int k, int* bi, int* bj, int* si, int* sj) {
-    if (!p || k < 0 || k >= static_cast<int>(p->tiles_tc.size())) return XC_ERR_INVALID_ARG;
-    if (bi) *bi = static_cast<int>(p->tiles_tc[k] & 0xFFFFu);
-    if (bj) *bj = static_cast<int>(p->tiles_tc[k] >> 16);
-    int a, b;
-    tile_shape(p->tile_mode, &a, &b);
+    if (!p || k < 0) return XC_ERR_INVALID_ARG;
+    uint32_t e = 0;
+    int a = 0, b = 0;
+    bool found = false;
+    for (uint32_t d : p->tiles_diag) {          // XC_TILE_SPLIT: diagonal sub-tiles first (32 x 64 stations each)
+        if (d == 0xFFFFFFFFu) continue;
+        if (k-- == 0) { e = d; a = 32; b = 64; found = true; break; }
+    }
+    if (!found) {
+        if (k >= static_cast<int>(p->tiles_tc.size())) return XC_ERR_INVALID_ARG;
+        e = p->tiles_tc[k];
+        tile_shape(p->tile_mode, &a, &b);
+    }
+    if (bi) *bi = static_cast<int>(e & 0xFFFFu);
+    if (bj) *bj = static_cast<int>(e >> 16);
     if (si) *si = a;
     if (sj) *sj = b;
     return XC_OK;

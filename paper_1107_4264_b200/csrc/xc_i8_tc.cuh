@@ -39,8 +39,11 @@ constexpr int TC_EPI_WARPS = 8;     // 2 per TMEM lane quarter, each owning half
 constexpr int TC_THREADS = 64 + 32 * TC_EPI_WARPS;   // + TMA producer warp + MMA issuer warp
 constexpr int TC_SMEM_LIMIT = 232448;  // 227 KB
 
-template <int UMMA_N, int CG, bool STAGED, int BK_ = 128>
+template <int UMMA_N, int CG, bool STAGED, int BK_ = 128, bool DIAG_ = false>
 struct TcCfg {
+    // DIAG: every tile of the launch sits on the diagonal (its A rows are one of its own B boxes), so the ring
+    // holds no separate A box -- the single-CTA 128x256 tile then has the same 32 KB stages as the CTA-pair tile.
+    static constexpr bool DIAG = DIAG_;
     static constexpr int M = 128 * CG;                    // Gram rows per tile
     static constexpr int B_BOXES = UMMA_N / 128 / CG;     // 128-row B boxes held by one CTA
     // Samples per pipeline stage.  Every stage costs the producer and the MMA issuer some hundred cycles of
@@ -48,7 +51,7 @@ struct TcCfg {
     // tensor work (128 cycles per 32 samples).  192-sample stages (4 of them) measured slower than 128 x 7.
     static constexpr int BK = BK_;
     static constexpr int BOX_BYTES = BK * 128;            // one TMA box: BK rows of 128 bytes
-    static constexpr int A_BYTES = BOX_BYTES;
+    static constexpr int A_BYTES = DIAG_ ? 0 : BOX_BYTES;
     static constexpr int B_BYTES = B_BOXES * BOX_BYTES;
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
     static constexpr int SI = 32 * CG;                    // stations per tile on the i side
@@ -60,23 +63,34 @@ struct TcCfg {
     static constexpr int BAR_BYTES = 1024;                // barriers + tmem slot, kept in the first KB
     static constexpr int SMEM_BYTES = BAR_BYTES + STAGES * STAGE_BYTES + OUT_BYTES + 1024;  // + slack for 1024-B alignment
     static_assert(B_BOXES >= 1, "a CTA holds at least one 128-row B box");
+    static_assert(!DIAG_ || (CG == 1 && UMMA_N == 256 && !STAGED), "DIAG is the single-CTA 128x256 direct-store variant");
     static_assert(SMEM_BYTES <= TC_SMEM_LIMIT, "smem");
     static_assert(STAGES >= 2, "ring too shallow");
 };
 
 struct TcParams {
     int N, F, T;
-    int tiles_per_f;          // entries of `tiles` per channel
+    int tiles_per_f;          // entries of `tiles` per channel (a multiple of 1 << group_shift)
     int total_tiles;          // F * tiles_per_f
+    int group_shift;          // a persistent CTA takes 2^group_shift consecutive table entries at a time (walk())
     long long NB;             // N(N+1)/2
-    const uint32_t* tiles;    // device: bi | (bj << 16), in units of (SI, SJ) stations
+    const uint32_t* tiles;    // device: bi | (bj << 16), in units of (SI, SJ) stations; TC_TILE_EMPTY = padding entry
     int32_t* vis;
     int accumulate;
     int debug_skip;           // profiling only (XC_OPT_DEBUG_SKIP): 1 = no TMA after the first ring fill,
                               // 2 = no MMA, 4 = no global stores; results are then meaningless
     long long* trace;         // profiling only: CTA 0 writes clock64() stamps here (see TC_TRACE_*), or null
 };
-constexpr int TC_TRACE_ITERS = 256;   // k-blocks traced; layout: [3 roles][TC_TRACE_ITERS][4] long long + 4 clock words
+constexpr uint32_t TC_TILE_EMPTY = 0xFFFFFFFFu;
+constexpr int TC_TRACE_ITERS = 256;
+
+// The persistent walk (S1): work unit `unit` of `nunits` takes groups unit, unit + nunits, ... of 2^gs consecutive
+// entries of the (channel-major) tile list; n counts the entries this unit has taken so far.  Returns the global
+// entry index, or -1 past the end.  Groups keep the two unequal sub-tiles of one diagonal block on one CTA.
+__device__ __forceinline__ int walk(int n, int unit, int nunits, int gs, int total) {
+    const long long w = ((static_cast<long long>(unit) + static_cast<long long>(n >> gs) * nunits) << gs) + (n & ((1 << gs) - 1));
+    return w < total ? static_cast<int>(w) : -1;
+}   // k-blocks traced; layout: [3 roles][TC_TRACE_ITERS][4] long long + 4 clock words
 
 // Epilogue for one 32-column chunk (8 stations j) held in v[]: complex combine, mask, store.
 // Thread <-> Gram row r = (i, pi, ci): lanes 4s..4s+3 of a warp are one station i; ci = 0 holds
@@ -144,10 +158,11 @@ __device__ __forceinline__ void epi_chunk_smem(const uint32_t (&v)[32], uint32_t
     }
 }
 
-template <int UMMA_N, int CG, bool STAGED, bool TRACE = false, int BK_ = 128>
-__global__ void __launch_bounds__(TC_THREADS, 1)
-xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
-    using Cfg = TcCfg<UMMA_N, CG, STAGED, BK_>;
+// The whole life of one persistent CTA (CG = 1) or of one CTA of a pair (CG = 2): work unit `unit` of `nunits`
+// walks the tile list of p.  `tmap` is the kernel's __grid_constant__ tensor map.
+template <int UMMA_N, int CG, bool STAGED, bool TRACE, int BK_, bool DIAG>
+__device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams& p, const int unit, const int nunits) {
+    using Cfg = TcCfg<UMMA_N, CG, STAGED, BK_, DIAG>;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     // Barriers first, operand ring after, on a 1024-byte boundary (SWIZZLE_128B atoms).
     const uint32_t bar0 = smem_u32(smem_raw);
@@ -162,8 +177,6 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;         // 0 = leader of the CTA pair
-    const int unit = (CG == 2) ? static_cast<int>(blockIdx.x >> 1) : static_cast<int>(blockIdx.x);
-    const int nunits = static_cast<int>(gridDim.x) / CG;              // persistent CTAs (pairs)
     constexpr uint32_t TMEM_COLS = 2 * UMMA_N;                         // 512 or 256: a power of two >= 32
 
     if (warp == 0 && lane == 0) {
@@ -202,16 +215,22 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
         const uint32_t elected = elect_one();
         uint32_t stage = 0, phase = 0;
         int it = 0;
-        uint32_t tb_next = (unit < p.total_tiles) ? __ldg(p.tiles + unit % p.tiles_per_f) : 0u;
-        for (int w = unit; w < p.total_tiles; w += nunits) {
-            const int f = w / p.tiles_per_f;
+        int w_next = walk(0, unit, nunits, p.group_shift, p.total_tiles);
+        uint32_t tb_next = (w_next >= 0) ? __ldg(p.tiles + w_next % p.tiles_per_f) : 0u;
+        for (int n = 0; w_next >= 0; ++n) {
+            const int f = w_next / p.tiles_per_f;
             const uint32_t tb = __shfl_sync(0xffffffffu, tb_next, 0);
             // the next tile's table entry is fetched now so that its latency hides behind this tile's k loop
-            if (w + nunits < p.total_tiles) tb_next = __ldg(p.tiles + (w + nunits) % p.tiles_per_f);
+            w_next = walk(n + 1, unit, nunits, p.group_shift, p.total_tiles);
+            if (w_next >= 0) tb_next = __ldg(p.tiles + w_next % p.tiles_per_f);
+            if (tb == TC_TILE_EMPTY) continue;
             const int m_a = static_cast<int>(tb & 0xFFFFu) * Cfg::M + 128 * static_cast<int>(rank);
             const int m_b = static_cast<int>(tb >> 16) * UMMA_N + Cfg::B_BOXES * 128 * static_cast<int>(rank);
-            const bool a_in_b = (m_a >= m_b) && (m_a < m_b + Cfg::B_BOXES * 128);   // diagonal: A rows are B rows
-            const uint32_t my_bytes = a_in_b ? Cfg::B_BYTES : Cfg::STAGE_BYTES;
+            const bool a_in_b = DIAG || ((m_a >= m_b) && (m_a < m_b + Cfg::B_BOXES * 128));   // diagonal: A rows are B rows
+            // DIAG: a row block that lies in the tile's second column box needs nothing of the first one (every pair
+            // there has i > j): only box 1 is loaded and the MMA shrinks to N = 128
+            const int h0 = (DIAG && m_a >= m_b + 128) ? 1 : 0;
+            const uint32_t my_bytes = a_in_b ? static_cast<uint32_t>(Cfg::B_BYTES - h0 * Cfg::BOX_BYTES) : Cfg::STAGE_BYTES;
             for (int kb = 0; kb < KB; ++kb) {
                 const bool tr = TRACE && p.trace && blockIdx.x == 0 && it < TC_TRACE_ITERS && elected;
                 if (tr) p.trace[(0 * TC_TRACE_ITERS + it) * 4 + 0] = clock64();
@@ -221,14 +240,14 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
                     const uint32_t sa = ring0 + stage * Cfg::STAGE_BYTES;
                     const uint32_t sb = sa + Cfg::A_BYTES;
                     const int t0 = kb * Cfg::BK;
-                    if ((p.debug_skip & 1) && (w != unit || kb >= Cfg::STAGES)) {
+                    if ((p.debug_skip & 1) && (n != 0 || kb >= Cfg::STAGES)) {
                         if (rank == 0) mbar_arrive(full_bar(stage));
                     } else if (CG == 1) {
                         mbar_arrive_expect_tx(full_bar(stage), my_bytes);
                         if (!a_in_b) tma_load_3d(sa, &tmap, full_bar(stage), m_a, f, t0);
 #pragma unroll
                         for (int h = 0; h < Cfg::B_BOXES; ++h)
-                            tma_load_3d(sb + h * Cfg::BOX_BYTES, &tmap, full_bar(stage), m_b + 128 * h, f, t0);
+                            if (h >= h0) tma_load_3d(sb + h * Cfg::BOX_BYTES, &tmap, full_bar(stage), m_b + 128 * h, f, t0);
                     } else {
                         // both CTAs' bytes are counted on the LEADER's barrier (a_in_b is the same in both)
                         const uint32_t lead_full = mapa_u32(full_bar(stage), 0);
@@ -255,18 +274,24 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
             constexpr uint32_t idesc = make_idesc_i8_mn(Cfg::M, UMMA_N);
             uint32_t stage = 0, phase = 0, buf = 0, tphase = 0;   // tphase bit b = phase of accumulator b
             int it = 0;
-            uint32_t tb_next = (unit < p.total_tiles) ? __ldg(p.tiles + unit % p.tiles_per_f) : 0u;
-            for (int w = unit; w < p.total_tiles; w += nunits) {
+            int w_next = walk(0, unit, nunits, p.group_shift, p.total_tiles);
+            uint32_t tb_next = (w_next >= 0) ? __ldg(p.tiles + w_next % p.tiles_per_f) : 0u;
+            for (int n = 0; w_next >= 0; ++n) {
                 const uint32_t tb = __shfl_sync(0xffffffffu, tb_next, 0);
-                if (w + nunits < p.total_tiles) tb_next = __ldg(p.tiles + (w + nunits) % p.tiles_per_f);
+                w_next = walk(n + 1, unit, nunits, p.group_shift, p.total_tiles);
+                if (w_next >= 0) tb_next = __ldg(p.tiles + w_next % p.tiles_per_f);
+                if (tb == TC_TILE_EMPTY) continue;
                 const int m_a = static_cast<int>(tb & 0xFFFFu) * Cfg::M;
                 const int m_b = static_cast<int>(tb >> 16) * UMMA_N;
-                const bool a_in_b = (m_a >= m_b) && (m_a < m_b + Cfg::B_BOXES * 128);
+                const bool a_in_b = DIAG || ((m_a >= m_b) && (m_a < m_b + Cfg::B_BOXES * 128));
                 // byte offset of the A operand inside a stage: its own box, or the B box holding the same rows
                 const uint32_t a_off = a_in_b ? static_cast<uint32_t>(Cfg::A_BYTES + ((m_a - m_b) >> 7) * Cfg::BOX_BYTES) : 0u;
+                // DIAG, row block in the second column box: N = 128 MMA on box 1 into the accumulator's upper 128 columns
+                const uint32_t h0 = (DIAG && m_a >= m_b + 128) ? 1u : 0u;
+                const uint32_t idesc_t = h0 ? make_idesc_i8_mn(Cfg::M, 128) : idesc;
                 mbar_wait(tempty_bar(buf), ((tphase >> buf) & 1u) ^ 1u);  // epilogues have drained this accumulator
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + buf * UMMA_N;
+                const uint32_t d_tmem = tmem_base + buf * UMMA_N + h0 * 128u;
                 for (int kb = 0; kb < KB; ++kb) {
                     const bool tr = TRACE && p.trace && blockIdx.x == 0 && it < TC_TRACE_ITERS && elected;
                     if (tr) p.trace[(1 * TC_TRACE_ITERS + it) * 4 + 0] = clock64();
@@ -276,7 +301,7 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
                     if (elected) {
                         const uint32_t sa = ring0 + stage * Cfg::STAGE_BYTES;
                         const uint64_t adesc = make_smem_desc_mn_sw128(sa + a_off, Cfg::BOX_BYTES, 1024);
-                        const uint64_t bdesc = make_smem_desc_mn_sw128(sa + Cfg::A_BYTES, Cfg::BOX_BYTES, 1024);
+                        const uint64_t bdesc = make_smem_desc_mn_sw128(sa + Cfg::A_BYTES + h0 * Cfg::BOX_BYTES, Cfg::BOX_BYTES, 1024);
                         const int rows = min(Cfg::BK, p.T - kb * Cfg::BK);           // valid samples in this stage
                         const int nk = (rows + TC_UMMA_K - 1) / TC_UMMA_K;       // rows beyond T are TMA zero fill
 #pragma unroll
@@ -284,7 +309,7 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
                             if (ks < nk && !(p.debug_skip & 2)) {
                                 // K advance: 32 samples = 4 swizzle atoms = 4096 B -> +256 in the address field
                                 umma_i8<CG>(d_tmem, adesc + static_cast<uint64_t>(ks * 256),
-                                            bdesc + static_cast<uint64_t>(ks * 256), idesc, (kb | ks) ? 1u : 0u);
+                                            bdesc + static_cast<uint64_t>(ks * 256), idesc_t, (kb | ks) ? 1u : 0u);
                             }
                         }
                         if (tr) p.trace[(1 * TC_TRACE_ITERS + it) * 4 + 2] = clock64();
@@ -311,13 +336,16 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
         uint32_t buf = 0, tphase = 0;
         int it = 0;
         const uint32_t lead_tempty0 = (CG == 2) ? mapa_u32(tempty_bar(0), 0) : tempty_bar(0);
-        uint32_t tb_next = (unit < p.total_tiles) ? __ldg(p.tiles + unit % p.tiles_per_f) : 0u;
-        for (int w = unit; w < p.total_tiles; w += nunits) {
+        int w_next = walk(0, unit, nunits, p.group_shift, p.total_tiles);
+        uint32_t tb_next = (w_next >= 0) ? __ldg(p.tiles + w_next % p.tiles_per_f) : 0u;
+        for (int n = 0; w_next >= 0; ++n) {
             const bool tr = TRACE && p.trace && blockIdx.x == 0 && it < TC_TRACE_ITERS && warp == 2 && lane == 0;
             if (tr) p.trace[(2 * TC_TRACE_ITERS + it) * 4 + 0] = clock64();
-            const int f = w / p.tiles_per_f;
+            const int f = w_next / p.tiles_per_f;
             const uint32_t tb = tb_next;
-            if (w + nunits < p.total_tiles) tb_next = __ldg(p.tiles + (w + nunits) % p.tiles_per_f);
+            w_next = walk(n + 1, unit, nunits, p.group_shift, p.total_tiles);
+            if (w_next >= 0) tb_next = __ldg(p.tiles + w_next % p.tiles_per_f);
+            if (tb == TC_TILE_EMPTY) continue;
             const int i0 = static_cast<int>(tb & 0xFFFFu) * Cfg::SI + 32 * static_cast<int>(rank) + 8 * q;
             const int j0 = static_cast<int>(tb >> 16) * Cfg::SJ + 8 * CHUNKS * half;   // first station of this warp's columns
             const int i = i0 + (lane >> 2);                     // i0 = first station of this warp's rows
@@ -402,6 +430,29 @@ xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
         tc_fence_after();
         tmem_dealloc<CG>(tmem_base, TMEM_COLS);
     }
+}
+
+// One tile shape per launch: every CTA (CG = 1) or CTA pair (CG = 2, cluster of 2) is one work unit.
+template <int UMMA_N, int CG, bool STAGED, bool TRACE = false, int BK_ = 128, bool DIAG = false>
+__global__ void __launch_bounds__(TC_THREADS, 1)
+xc_i8_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p) {
+    tc_body<UMMA_N, CG, STAGED, TRACE, BK_, DIAG>(tmap, p, static_cast<int>(blockIdx.x) / CG, static_cast<int>(gridDim.x) / CG);
+}
+
+// XC_TILE_MIXED: ONE launch in clusters of 2 in which the first n_solo_clusters clusters are two independent
+// single-CTA workers on the diagonal 64-station blocks (pd: DIAG sub-tiles, tcgen05 cta_group::1 only) and the other
+// clusters are CTA pairs on the off-diagonal 256x256 tiles (po: cta_group::2 only).  A given CTA executes
+// tcgen05 instructions of one cta_group only, for its whole life.  Both kinds of worker walk the channels in the
+// same order at a rate balanced by the host, so a channel's input is fetched from HBM once and shared through L2
+// (two separate launches would each read the whole input from HBM: measured).
+__global__ void __launch_bounds__(TC_THREADS, 1)
+xc_i8_tc_mixed_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams pd, const TcParams po, const int n_solo_clusters) {
+    const int cluster = static_cast<int>(blockIdx.x >> 1);
+    if (cluster < n_solo_clusters)
+        tc_body<256, 1, false, false, 128, true>(tmap, pd, static_cast<int>(blockIdx.x), 2 * n_solo_clusters);
+    else
+        tc_body<256, 2, false, false, 128, false>(tmap, po, cluster - n_solo_clusters,
+                                                  static_cast<int>(gridDim.x >> 1) - n_solo_clusters);
 }
 
 }  // namespace xc

@@ -74,7 +74,7 @@ def test_compute_without_gpu_fails_loudly():
     assert rc in (-5, -2)
 
 
-@pytest.mark.parametrize("mode", [0, 1, 2, 3])
+@pytest.mark.parametrize("mode", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("N", [1, 2, 3, 5, 16, 31, 32, 33, 64, 65, 100, 128, 129, 256, 500, 512, 1024])
 def test_tile_schedule_covers_triangle_exactly_once(N, mode):
     p = xcb.Plan(N, 1, 8)

@@ -25,7 +25,7 @@ def _built():
     assert torch.cuda.is_available()
 
 
-TILE_MODES = [xcb.TILE_1CTA_128x128, xcb.TILE_1CTA_128x256, xcb.TILE_2CTA_256x256]
+TILE_MODES = [xcb.TILE_1CTA_128x128, xcb.TILE_1CTA_128x256, xcb.TILE_2CTA_256x256, xcb.TILE_SPLIT, xcb.TILE_MIXED]
 
 
 EPI_MODES = [xcb.EPI_DIRECT, xcb.EPI_STAGED]
