@@ -160,10 +160,23 @@ int xc_correlate_f32(xc_plan_t* plan, const float* in_dev, float* vis_dev, int a
 int xc_correlate_pipelined(xc_plan_t* plan, const int8_t* in_host_pinned, int n_blocks, int8_t* dev_buf2,
                            int32_t* vis_dev, void* compute_stream, void* copy_stream);
 
-/* xc_correlate_host -- convenience end-to-end call with HOST buffers: copies in_host
- *   (xc_in_bytes(), pinned for full speed) to in_dev_scratch, runs xc_correlate, copies the
- *   result back into vis_host (xc_vis_bytes()) and synchronises the stream before returning.
- *   in_dev_scratch / vis_dev_scratch are caller-owned device buffers of the plan's sizes. */
+/* xc_correlate_channels -- the same operation restricted to channels [f0, f0 + nf) of the plan's F ("evaluated
+ *   independently for every frequency"; the paper's multi-GPU plan hands different channels to
+ *   different devices).  in_dev / vis_dev are the FULL block and cube of the plan (the range is
+ *   addressed inside them with the plan's F as channel pitch); only vis[f0 .. f0+nf) is written.  accumulate != 0
+ *   adds.  Ranges of one block may run concurrently on different streams.  Errors: INVALID_ARG for a range outside
+ *   [0, F); UNSUPPORTED when the input needs the staging pass (N % 4 != 0, re-pitched N, misaligned pointer) or
+ *   the SIMT kernel is selected -- those work on whole blocks only. */
+int xc_correlate_channels(xc_plan_t* plan, const int8_t* in_dev, int32_t* vis_dev, int f0, int nf, int accumulate,
+                          void* cuda_stream);
+
+/* xc_correlate_host -- the integrated run with HOST buffers (Fig. 7: host->device copy,
+ *   X-engine, device->host copy of the result): copies in_host (xc_in_bytes(), pinned for full speed) to
+ *   in_dev_scratch, correlates, copies the result into vis_host (xc_vis_bytes(), pinned for full speed) and
+ *   synchronises the stream before returning.  Blocks of 8 MiB and more are cut into up to 16 channel ranges so
+ *   that the copy-in of range c+1, the X-engine on range c and the copy-out of range c-1 overlap; the copies then
+ *   run on two plan-owned streams ordered against cuda_stream by events (the only place the library uses streams
+ *   of its own).  in_dev_scratch / vis_dev_scratch are caller-owned device buffers of the plan's sizes. */
 int xc_correlate_host(xc_plan_t* plan, const int8_t* in_host, int32_t* vis_host, int8_t* in_dev_scratch,
                       int32_t* vis_dev_scratch, void* cuda_stream);
 

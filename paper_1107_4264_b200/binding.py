@@ -22,7 +22,7 @@ TILE_AUTO, TILE_1CTA_128x128, TILE_1CTA_128x256, TILE_2CTA_256x256, TILE_SPLIT, 
 EXPORTED_SYMBOLS = (
     "xc_plan", "xc_destroy", "xc_in_bytes", "xc_in_bytes_f32", "xc_vis_bytes", "xc_n_baselines",
     "xc_workspace_bytes", "xc_set_workspace", "xc_set_option", "xc_correlate", "xc_correlate_acc",
-    "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_tile_count", "xc_tile_get",
+    "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_tile_count", "xc_tile_get",
     "xc_debug_set_trace", "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error",
     "xc_version",
 )
@@ -58,6 +58,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_set_option": (i, [p, i, i]),
         "xc_correlate": (i, [p, p, p, p]), "xc_correlate_acc": (i, [p, p, p, p]),
         "xc_correlate_f32": (i, [p, p, p, i, p]),
+        "xc_correlate_channels": (i, [p, p, p, i, i, i, p]),
         "xc_correlate_pipelined": (i, [p, p, i, p, p, p, p]),
         "xc_correlate_host": (i, [p, p, p, p, p, p]),
         "xc_debug_set_trace": (i, [p, p]),
@@ -225,6 +226,16 @@ class Plan:
         self._chk_vis(vis, torch.int32)
         self._check(lib().xc_correlate_acc(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(vis.data_ptr()),
                                            _stream_handle(stream)), "xc_correlate_acc")
+        return vis
+
+    def correlate_channels(self, x, vis, f0: int, nf: int, accumulate=False, stream=None):
+        """vis[f0:f0+nf] (+)= X-engine(x[:, f0:f0+nf]); x and vis are the plan's full block and cube."""
+        import torch
+        self._chk_in(x, torch.int8)
+        self._chk_vis(vis, torch.int32)
+        self._check(lib().xc_correlate_channels(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(vis.data_ptr()),
+                                                f0, nf, 1 if accumulate else 0, _stream_handle(stream)),
+                    "xc_correlate_channels")
         return vis
 
     def correlate_f32(self, x, vis=None, accumulate=False, stream=None):

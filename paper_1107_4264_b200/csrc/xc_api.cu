@@ -103,7 +103,9 @@ struct xc_plan_s {
     long long* trace = nullptr;
     CUtensorMap tmap;
     const void* tmap_src = nullptr;
-    int tmap_nrow = 0, tmap_bk = 0;
+    int tmap_nrow = 0, tmap_bk = 0, tmap_nf = 0;
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;       // xc_correlate_host: plan-owned copy streams
+    std::vector<cudaEvent_t> ev_chunk;                   // xc_correlate_host: per-chunk events
     cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_entry = nullptr;
     int last_launches = 0;
     std::string last_err;
@@ -268,9 +270,10 @@ int stage_if_needed(xc_plan_t* p, const int8_t* in_dev, cudaStream_t st, const v
     return XC_OK;
 }
 
-int encode_tmap(xc_plan_t* p, const void* src, int nrow, int bk) {
-    if (p->tmap_src == src && p->tmap_nrow == nrow && p->tmap_bk == bk) return XC_OK;
-    const cuuint64_t gdim[3] = {static_cast<cuuint64_t>(4) * nrow, static_cast<cuuint64_t>(p->F),
+// Tensor map over channels [.., nf) of the block that starts at src (the channel pitch stays the plan's F).
+int encode_tmap(xc_plan_t* p, const void* src, int nrow, int bk, int nf) {
+    if (p->tmap_src == src && p->tmap_nrow == nrow && p->tmap_bk == bk && p->tmap_nf == nf) return XC_OK;
+    const cuuint64_t gdim[3] = {static_cast<cuuint64_t>(4) * nrow, static_cast<cuuint64_t>(nf),
                                 static_cast<cuuint64_t>(p->T)};
     const cuuint64_t gstride[2] = {static_cast<cuuint64_t>(4) * nrow,
                                    static_cast<cuuint64_t>(4) * nrow * static_cast<cuuint64_t>(p->F)};
@@ -289,17 +292,26 @@ int encode_tmap(xc_plan_t* p, const void* src, int nrow, int bk) {
     p->tmap_src = src;
     p->tmap_nrow = nrow;
     p->tmap_bk = bk;
+    p->tmap_nf = nf;
     return XC_OK;
 }
 
-int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* stream, int accumulate) {
+// X-engine on channels [f0, f0 + nf) of the block at in_dev / the cube at vis_dev (both addressed with the plan's F).
+int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* stream, int accumulate, int f0 = 0,
+                 int nf = -1) {
     if (!p || !in_dev || !vis_dev) return XC_ERR_INVALID_ARG;
+    if (nf < 0) nf = p->F;
+    if (f0 < 0 || nf < 1 || f0 + nf > p->F) return XC_ERR_INVALID_ARG;
+    const bool sub = (f0 != 0 || nf != p->F);
     if (reinterpret_cast<uintptr_t>(vis_dev) & 15u) return XC_ERR_ALIGNMENT;
     int rc = ensure_device(p);
     if (rc != XC_OK) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     p->last_launches = 0;
 
+    // a channel sub-range is read in place through its own tensor map: not with the SIMT kernel, not through staging
+    const bool need_stage = p->opt_force_stage || (p->Npad != p->N) || (reinterpret_cast<uintptr_t>(in_dev) & 15u);
+    if (sub && (p->opt_kernel == XC_I8_KERNEL_SIMT || need_stage)) return XC_ERR_UNSUPPORTED;
     if (p->opt_kernel == XC_I8_KERNEL_SIMT) {
         if (p->F > 65535) return XC_ERR_UNSUPPORTED;
         xc::SimtParams sp{p->N, p->F, p->T, p->NB, in_dev, vis_dev, accumulate};
@@ -318,17 +330,17 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     const bool bkopt = p->tile_mode == XC_TILE_2CTA_256x256 && p->opt_epilogue != XC_EPI_STAGED;
     const bool bk256 = bkopt && p->opt_bk == 256, bk64 = bkopt && p->opt_bk == 64;
     const int bk = bk256 ? 256 : (bk64 ? 64 : 128);
-    rc = encode_tmap(p, src, nrow, bk);
+    rc = encode_tmap(p, static_cast<const int8_t*>(src) + static_cast<size_t>(4) * nrow * f0, nrow, bk, nf);
     if (rc != XC_OK) return rc;
 
     rc = upload_tiles(p);
     if (rc != XC_OK) return rc;
     xc::TcParams tp;
     tp.N = p->N;
-    tp.F = p->F;
+    tp.F = nf;
     tp.T = p->T;
     tp.NB = p->NB;
-    tp.vis = vis_dev;
+    tp.vis = vis_dev + static_cast<size_t>(f0) * p->NB * 8;
     tp.accumulate = accumulate;
     tp.debug_skip = p->opt_debug_skip;
     tp.trace = p->trace;
@@ -336,8 +348,8 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
         tp.tiles_per_f = static_cast<int>(host.size());
         tp.tiles = dev;
         tp.group_shift = group_shift;
-        if (static_cast<long long>(p->F) * tp.tiles_per_f > 0x7FFFFFFFLL) return false;
-        tp.total_tiles = p->F * tp.tiles_per_f;
+        if (static_cast<long long>(nf) * tp.tiles_per_f > 0x7FFFFFFFLL) return false;
+        tp.total_tiles = nf * tp.tiles_per_f;
         return true;
     };
     const bool staged = p->opt_epilogue == XC_EPI_STAGED;   // AUTO = direct stores (measured faster)
@@ -354,7 +366,7 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
         }
         int clusters = (p->opt_max_ctas > 0 ? p->opt_max_ctas : p->sm_count) / 2;
         if (clusters < 2) clusters = 2;
-        const int n_solo = p->tiles_tc.empty() ? clusters : mixed_split(p->N, p->F, clusters, nullptr);
+        const int n_solo = p->tiles_tc.empty() ? clusters : mixed_split(p->N, nf, clusters, nullptr);
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(static_cast<unsigned>(2 * clusters));
         cfg.blockDim = dim3(xc::TC_THREADS);
@@ -437,6 +449,9 @@ void xc_destroy(xc_plan_t* p) {
         if (p->ev_free[k]) cudaEventDestroy(p->ev_free[k]);
     }
     if (p->ev_entry) cudaEventDestroy(p->ev_entry);
+    for (cudaEvent_t e : p->ev_chunk) cudaEventDestroy(e);
+    if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
+    if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
     delete p;
 }
 
@@ -563,15 +578,66 @@ int xc_correlate_pipelined(xc_plan_t* p, const int8_t* in_host, int n_blocks, in
     return XC_OK;
 }
 
+int xc_correlate_channels(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, int f0, int nf, int accumulate,
+                          void* stream) {
+    return correlate_i8(p, in_dev, vis_dev, stream, accumulate ? 1 : 0, f0, nf);
+}
+
 int xc_correlate_host(xc_plan_t* p, const int8_t* in_host, int32_t* vis_host, int8_t* in_dev_scratch,
                       int32_t* vis_dev_scratch, void* stream) {
     if (!p || !in_host || !vis_host || !in_dev_scratch || !vis_dev_scratch) return XC_ERR_INVALID_ARG;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    XC_CUDA(p, cudaMemcpyAsync(in_dev_scratch, in_host, xc_in_bytes(p), cudaMemcpyHostToDevice, st));
-    int rc = correlate_i8(p, in_dev_scratch, vis_dev_scratch, stream, 0);
+    int rc = ensure_device(p);
     if (rc != XC_OK) return rc;
-    XC_CUDA(p, cudaMemcpyAsync(vis_host, vis_dev_scratch, xc_vis_bytes(p), cudaMemcpyDeviceToHost, st));
+    const bool need_stage = p->opt_force_stage || (p->Npad != p->N) || (reinterpret_cast<uintptr_t>(in_dev_scratch) & 15u);
+    int chunks = p->F < 16 ? p->F : 16;
+    if (need_stage || p->opt_kernel == XC_I8_KERNEL_SIMT || xc_in_bytes(p) < (static_cast<size_t>(8) << 20)) chunks = 1;
+    if (chunks == 1) {
+        XC_CUDA(p, cudaMemcpyAsync(in_dev_scratch, in_host, xc_in_bytes(p), cudaMemcpyHostToDevice, st));
+        rc = correlate_i8(p, in_dev_scratch, vis_dev_scratch, stream, 0);
+        if (rc != XC_OK) return rc;
+        XC_CUDA(p, cudaMemcpyAsync(vis_host, vis_dev_scratch, xc_vis_bytes(p), cudaMemcpyDeviceToHost, st));
+        XC_CUDA(p, cudaStreamSynchronize(st));
+        return XC_OK;
+    }
+    // Channels are independent, so the block is cut into channel ranges and the three legs of the
+    // paper's integrated run (host->device, X-engine, device->host: Fig. 7) overlap: range c+1 is
+    // copied in (a strided 2-D copy: T rows of the range's bytes) while range c is correlated and range c-1 is
+    // copied out, on two plan-owned copy streams ordered against the caller's stream by events.
+    if (!p->s_h2d) XC_CUDA(p, cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking));
+    if (!p->s_d2h) XC_CUDA(p, cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking));
+    while (p->ev_chunk.size() < static_cast<size_t>(2 * chunks + 2)) {
+        cudaEvent_t e = nullptr;
+        XC_CUDA(p, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        p->ev_chunk.push_back(e);
+    }
+    cudaEvent_t ev_entry = p->ev_chunk[2 * chunks], ev_done = p->ev_chunk[2 * chunks + 1];
+    XC_CUDA(p, cudaEventRecord(ev_entry, st));           // earlier work on the caller's stream may still use the scratch
+    XC_CUDA(p, cudaStreamWaitEvent(p->s_h2d, ev_entry, 0));
+    XC_CUDA(p, cudaStreamWaitEvent(p->s_d2h, ev_entry, 0));
+    const size_t row = static_cast<size_t>(4) * p->N;    // bytes of one (t, f) row
+    const size_t pitch = row * p->F;
+    int launches = 0;
+    for (int c = 0; c < chunks; ++c) {
+        const int f0 = static_cast<int>(static_cast<long long>(p->F) * c / chunks);
+        const int f1 = static_cast<int>(static_cast<long long>(p->F) * (c + 1) / chunks);
+        XC_CUDA(p, cudaMemcpy2DAsync(in_dev_scratch + row * f0, pitch, in_host + row * f0, pitch, row * (f1 - f0),
+                                     static_cast<size_t>(p->T), cudaMemcpyHostToDevice, p->s_h2d));
+        XC_CUDA(p, cudaEventRecord(p->ev_chunk[2 * c], p->s_h2d));
+        XC_CUDA(p, cudaStreamWaitEvent(st, p->ev_chunk[2 * c], 0));
+        rc = correlate_i8(p, in_dev_scratch, vis_dev_scratch, stream, 0, f0, f1 - f0);
+        if (rc != XC_OK) return rc;
+        launches += p->last_launches;
+        XC_CUDA(p, cudaEventRecord(p->ev_chunk[2 * c + 1], st));
+        XC_CUDA(p, cudaStreamWaitEvent(p->s_d2h, p->ev_chunk[2 * c + 1], 0));
+        const size_t voff = static_cast<size_t>(f0) * p->NB * 8;
+        XC_CUDA(p, cudaMemcpyAsync(vis_host + voff, vis_dev_scratch + voff, static_cast<size_t>(f1 - f0) * p->NB * 32,
+                                   cudaMemcpyDeviceToHost, p->s_d2h));
+    }
+    XC_CUDA(p, cudaEventRecord(ev_done, p->s_d2h));
+    XC_CUDA(p, cudaStreamWaitEvent(st, ev_done, 0));
     XC_CUDA(p, cudaStreamSynchronize(st));
+    p->last_launches = launches;
     return XC_OK;
 }
 

@@ -222,6 +222,62 @@ def test_host_end_to_end_call():
     assert np.array_equal(vh.numpy(), xo.correlate_i8(x))
 
 
+def test_host_call_chunked_overlap():
+    """Blocks of 8 MiB and more go through xc_correlate_host's channel-range pipeline (copy-in, X-engine and copy-out
+    of different ranges overlap): same bits as the oracle, every output written, repeatable into the same buffers."""
+    N, F, T = 64, 43, 1000                                   # 11 MB; F not a multiple of the 16 ranges
+    x = wl.gaussian(N, F, T, seed=77, sigma=4.0)
+    p = xcb.Plan(N, F, T)
+    xh = torch.from_numpy(x).pin_memory()
+    vh = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32).pin_memory()
+    xd = torch.zeros(p.in_shape(), dtype=torch.int8, device="cuda")
+    vd = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+    p.correlate_host(xh, vh, xd, vd)
+    assert p.last_launches == 16
+    ref = xo.correlate_i8(x)
+    assert np.array_equal(vh.numpy(), ref)
+    vh.fill_(0)
+    s = torch.cuda.Stream()
+    p.correlate_host(xh, vh, xd, vd, stream=s)
+    assert np.array_equal(vh.numpy(), ref)
+
+
+def test_correlate_channels_ranges():
+    """xc_correlate_channels: ranges of one block, processed separately (here on two streams),
+    write exactly their own slice of the cube; accumulate adds to that slice only."""
+    N, F, T = 96, 11, 150
+    x = wl.full_range(N, F, T, seed=5)
+    ref = xo.correlate_i8(x)
+    p = xcb.Plan(N, F, T)
+    xd = torch.from_numpy(x).cuda()
+    poison = 0x5A5A5A5A
+    vis = torch.full(p.vis_shape(), poison, dtype=torch.int32, device="cuda")
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    p.correlate_channels(xd, vis, 0, 4, stream=s1)
+    p.correlate_channels(xd, vis, 7, 4, stream=s2)
+    torch.cuda.synchronize()
+    got = vis.cpu().numpy()
+    assert np.array_equal(got[0:4], ref[0:4]) and np.array_equal(got[7:11], ref[7:11])
+    assert (got[4:7] == poison).all()
+    p.correlate_channels(xd, vis, 4, 3)
+    p.correlate_channels(xd, vis, 2, 5, accumulate=True)
+    torch.cuda.synchronize()
+    got = vis.cpu().numpy()
+    want = ref.copy()
+    want[2:7] *= 2
+    assert np.array_equal(got, want)
+    for f0, nf in [(-1, 2), (0, 0), (10, 2), (0, 12)]:
+        with pytest.raises(xcb.XcError):
+            p.correlate_channels(xd, vis, f0, nf)
+    # a block that needs the staging pass works on whole blocks only
+    p2 = xcb.Plan(5, 4, 8)
+    x2 = torch.zeros(p2.in_shape(), dtype=torch.int8, device="cuda")
+    with pytest.raises(xcb.XcError):
+        p2.correlate_channels(x2, p2.new_vis(), 1, 2)
+    assert torch.equal(p2.correlate_channels(x2, p2.new_vis(), 0, 4), torch.zeros(p2.vis_shape(), dtype=torch.int32, device="cuda"))
+
+
 # ---------------------------------------------------------------------------------------------
 # fp32 path
 # ---------------------------------------------------------------------------------------------
