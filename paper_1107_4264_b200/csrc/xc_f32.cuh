@@ -6,8 +6,13 @@
 // only at the innermost level.  Re-sized for sm_100a: 2 x 4 station pairs per thread (64 fp32
 // accumulators; the paper's Fermi kernel 11 used 2 x 2), a 32 x 64 station tile per 256-thread
 // block, and a 3-stage cp.async ring in place of the paper's double-buffered texture loads.
-// Only tiles that intersect i <= j are launched; threads above the diagonal
-// compute but do not write (the paper's software-cache choice).
+// The 16 FMAs of a station pair are issued as 8 packed FFMA2 (fma.rn.f32x2) on (re, im) pairs.
+// Only tiles that intersect i <= j are launched.  The paper lets threads above
+// the diagonal compute without writing (its software-cache choice); here each warp
+// owns a 16 x 16-station block and skips the arithmetic when the whole block is above the diagonal,
+// which cuts the paper's wasted work from 32 x 64 to 16 x 16 granularity.
+// Measured variants (B200, config 3 values): stages of 8 / 16 / 32 samples x 2-4 stages and 1 vs 2
+// blocks per SM -- 16 x 3 x 2 is the fastest.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -16,8 +21,17 @@ namespace xc {
 
 constexpr int F32_SI = 32;       // stations per tile on the i side
 constexpr int F32_SJ = 64;       // stations per tile on the j side
-constexpr int F32_BK = 16;       // samples per ring stage
-constexpr int F32_STAGES = 3;
+#ifndef XC_F32_BK
+#define XC_F32_BK 16
+#endif
+#ifndef XC_F32_STAGES
+#define XC_F32_STAGES 3
+#endif
+#ifndef XC_F32_MINB
+#define XC_F32_MINB 2
+#endif
+constexpr int F32_BK = XC_F32_BK;       // samples per ring stage
+constexpr int F32_STAGES = XC_F32_STAGES;
 constexpr int F32_THREADS = 256;
 constexpr int F32_STAGE_F4 = F32_BK * (F32_SI + F32_SJ);             // float4 per stage
 constexpr int F32_SMEM_BYTES = F32_STAGES * F32_STAGE_F4 * 16;       // 72 KB
@@ -41,24 +55,42 @@ __device__ __forceinline__ void cp_async_wait() {
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-// acc[(pi*2+pj)*2 + c] += a_{pi} * conj(b_{pj}): 16 FMAs.
-__device__ __forceinline__ void cmac4(float (&acc)[8], const float4& a, const float4& b) {
-    // pi = 0: (a.x, a.y); pi = 1: (a.z, a.w); pj = 0: (b.x, b.y); pj = 1: (b.z, b.w)
-    acc[0] = fmaf(a.x, b.x, acc[0]); acc[0] = fmaf(a.y, b.y, acc[0]);
-    acc[1] = fmaf(a.y, b.x, acc[1]); acc[1] = fmaf(-a.x, b.y, acc[1]);
-    acc[2] = fmaf(a.x, b.z, acc[2]); acc[2] = fmaf(a.y, b.w, acc[2]);
-    acc[3] = fmaf(a.y, b.z, acc[3]); acc[3] = fmaf(-a.x, b.w, acc[3]);
-    acc[4] = fmaf(a.z, b.x, acc[4]); acc[4] = fmaf(a.w, b.y, acc[4]);
-    acc[5] = fmaf(a.w, b.x, acc[5]); acc[5] = fmaf(-a.z, b.y, acc[5]);
-    acc[6] = fmaf(a.z, b.z, acc[6]); acc[6] = fmaf(a.w, b.w, acc[6]);
-    acc[7] = fmaf(a.w, b.z, acc[7]); acc[7] = fmaf(-a.z, b.w, acc[7]);
+// Packed fp32 FMA (sm_100 FFMA2): d.lo = a.lo * b.lo + c.lo, d.hi = a.hi * b.hi + c.hi, each rounded once like
+// fmaf.  The SASS instruction takes a scalar-broadcast, a half-swap and per-half negation as operand modifiers, so
+// the (re, im) pair algebra below costs no extra instructions (checked with cuobjdump: FFMA2 ... .F32x2.LO_HI.NP).
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {
+    unsigned long long ua, ub, uc, ud;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ua) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ub) : "f"(b.x), "f"(b.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(uc) : "f"(c.x), "f"(c.y));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(ud) : "l"(ua), "l"(ub), "l"(uc));
+    float2 d;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(ud));
+    return d;
 }
 
-__global__ void __launch_bounds__(F32_THREADS, 2) xc_f32_kernel(const F32Params p) {
+// acc[pi*2+pj] = (re, im) += a_{pi} * conj(b_{pj}): 16 FMAs as 8 packed ones.  Per output the order
+// is  re = fma(a.im, b.im, fma(a.re, b.re, re)),  im = fma(-a.re, b.im, fma(a.im, b.re, im)).
+__device__ __forceinline__ void cmac4(float2 (&acc)[4], const float4& a, const float4& b) {
+    // pi = 0: (a.x, a.y); pi = 1: (a.z, a.w); pj = 0: (b.x, b.y); pj = 1: (b.z, b.w)
+    const float2 a0 = make_float2(a.x, a.y), a0s = make_float2(a.y, -a.x);
+    const float2 a1 = make_float2(a.z, a.w), a1s = make_float2(a.w, -a.z);
+    acc[0] = ffma2(a0, make_float2(b.x, b.x), acc[0]); acc[0] = ffma2(a0s, make_float2(b.y, b.y), acc[0]);
+    acc[1] = ffma2(a0, make_float2(b.z, b.z), acc[1]); acc[1] = ffma2(a0s, make_float2(b.w, b.w), acc[1]);
+    acc[2] = ffma2(a1, make_float2(b.x, b.x), acc[2]); acc[2] = ffma2(a1s, make_float2(b.y, b.y), acc[2]);
+    acc[3] = ffma2(a1, make_float2(b.z, b.z), acc[3]); acc[3] = ffma2(a1s, make_float2(b.w, b.w), acc[3]);
+}
+
+__global__ void __launch_bounds__(F32_THREADS, XC_F32_MINB) xc_f32_kernel(const F32Params p) {
     extern __shared__ __align__(16) float4 smem_f4[];
     const int tid = threadIdx.x;
-    const int ti = tid & 15;   // stations i0 + ti, i0 + ti + 16
-    const int tj = tid >> 4;   // stations j0 + tj + 16 n, n = 0..3
+    // Each warp owns a 16 x 16-station block of the tile (2 blocks on the i side x 4 on the j side), its lanes an
+    // 8 (i) x 4 (j) grid, each lane 2 x 4 station pairs.  A warp whose whole block lies above the diagonal (every
+    // i > j) or beyond N skips the arithmetic -- it still loads and synchronises -- so diagonal tiles cost what
+    // they store at 16-station granularity, and the co-resident CTA's warps take the freed issue slots.
+    const int warp = tid >> 5, lane = tid & 31;
+    const int ti = 16 * (warp & 1) + (lane & 7);    // stations i0 + ti, i0 + ti + 8
+    const int tj = 16 * (warp >> 1) + (lane >> 3);  // stations j0 + tj + 4 n, n = 0..3
 
     const long long w = blockIdx.x;
     const int f = static_cast<int>(w / p.tiles_per_f);
@@ -85,13 +117,13 @@ __global__ void __launch_bounds__(F32_THREADS, 2) xc_f32_kernel(const F32Params 
         }
     };
 
-    float acc[2][4][8];
+    float2 acc[2][4][4];
 #pragma unroll
     for (int a = 0; a < 2; ++a)
 #pragma unroll
         for (int b = 0; b < 4; ++b)
 #pragma unroll
-            for (int c = 0; c < 8; ++c) acc[a][b][c] = 0.f;
+            for (int c = 0; c < 4; ++c) acc[a][b][c] = make_float2(0.f, 0.f);
 
 #pragma unroll
     for (int s = 0; s < F32_STAGES - 1; ++s) {
@@ -99,18 +131,23 @@ __global__ void __launch_bounds__(F32_THREADS, 2) xc_f32_kernel(const F32Params 
         cp_async_commit();
     }
 
+    // warp-uniform: does this warp's 16 x 16 block hold any stored pair (i <= j < N)?
+    const int wi0 = i0 + 16 * (warp & 1), wj0 = j0 + 16 * (warp >> 1);
+    const bool active = (wi0 <= wj0 + 15) && (wi0 < p.N) && (wj0 < p.N);
+
     for (int kb = 0; kb < KB; ++kb) {
         cp_async_wait<F32_STAGES - 2>();
         __syncthreads();
         load_stage(kb + F32_STAGES - 1, (kb + F32_STAGES - 1) % F32_STAGES);
         cp_async_commit();
+        if (!active) continue;
         const float4* sA = smem_f4 + (kb % F32_STAGES) * F32_STAGE_F4;
 #pragma unroll
         for (int k = 0; k < F32_BK; ++k) {
             const float4* row = sA + k * (F32_SI + F32_SJ);
-            const float4 a0 = row[ti], a1 = row[ti + 16];
-            const float4 b0 = row[F32_SI + tj], b1 = row[F32_SI + tj + 16];
-            const float4 b2 = row[F32_SI + tj + 32], b3 = row[F32_SI + tj + 48];
+            const float4 a0 = row[ti], a1 = row[ti + 8];
+            const float4 b0 = row[F32_SI + tj], b1 = row[F32_SI + tj + 4];
+            const float4 b2 = row[F32_SI + tj + 8], b3 = row[F32_SI + tj + 12];
             cmac4(acc[0][0], a0, b0); cmac4(acc[0][1], a0, b1); cmac4(acc[0][2], a0, b2); cmac4(acc[0][3], a0, b3);
             cmac4(acc[1][0], a1, b0); cmac4(acc[1][1], a1, b1); cmac4(acc[1][2], a1, b2); cmac4(acc[1][3], a1, b3);
         }
@@ -120,14 +157,14 @@ __global__ void __launch_bounds__(F32_THREADS, 2) xc_f32_kernel(const F32Params 
     float* visf = p.vis + static_cast<long long>(f) * p.NB * 8;
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
-        const int j = j0 + tj + 16 * b;
+        const int j = j0 + tj + 4 * b;
 #pragma unroll
         for (int a = 0; a < 2; ++a) {
-            const int i = i0 + ti + 16 * a;
+            const int i = i0 + ti + 8 * a;
             if (i <= j && j < p.N) {
                 float4* dst = reinterpret_cast<float4*>(visf + (static_cast<long long>(j) * (j + 1) / 2 + i) * 8);
-                float4 lo = make_float4(acc[a][b][0], acc[a][b][1], acc[a][b][2], acc[a][b][3]);
-                float4 hi = make_float4(acc[a][b][4], acc[a][b][5], acc[a][b][6], acc[a][b][7]);
+                float4 lo = make_float4(acc[a][b][0].x, acc[a][b][0].y, acc[a][b][1].x, acc[a][b][1].y);
+                float4 hi = make_float4(acc[a][b][2].x, acc[a][b][2].y, acc[a][b][3].x, acc[a][b][3].y);
                 if (p.accumulate) {
                     const float4 o0 = dst[0], o1 = dst[1];
                     lo.x += o0.x; lo.y += o0.y; lo.z += o0.z; lo.w += o0.w;
