@@ -96,6 +96,8 @@ typedef enum {
     XC_OPT_TILE = 4,       /* one of XC_TILE_*; rebuilds the tile schedule (synchronising on next call) */
     XC_OPT_EPILOGUE = 5,   /* one of XC_EPI_*                                                  */
     XC_OPT_BK = 6,         /* samples per pipeline stage of the CTA-pair kernel: 0 (auto), 128 or 256 */
+    XC_OPT_PDL = 7,        /* 1 (default) = launch the tensor-core kernels with programmatic stream            */
+                           /* serialization: the prologue overlaps the previous kernel's tail; 0 = plain launch */
     XC_OPT_DEBUG_SKIP = 3  /* PROFILING ONLY, results become meaningless: bit 0 = no TMA loads  */
                            /* after the first ring fill, bit 1 = no MMAs, bit 2 = no stores     */
 } xc_option;

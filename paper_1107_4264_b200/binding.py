@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(HERE, "libxc.so")
 MAX_T = 65535
 TRACE_WORDS = 3 * 256 * 4 + 4
 I8_KERNEL_AUTO, I8_KERNEL_TC, I8_KERNEL_SIMT = 0, 1, 2
-OPT_I8_KERNEL, OPT_MAX_CTAS, OPT_FORCE_STAGE, OPT_DEBUG_SKIP, OPT_TILE, OPT_EPILOGUE, OPT_BK = 0, 1, 2, 3, 4, 5, 6
+OPT_I8_KERNEL, OPT_MAX_CTAS, OPT_FORCE_STAGE, OPT_DEBUG_SKIP, OPT_TILE, OPT_EPILOGUE, OPT_BK, OPT_PDL = 0, 1, 2, 3, 4, 5, 6, 7
 EPI_AUTO, EPI_DIRECT, EPI_STAGED = 0, 1, 2
 TILE_AUTO, TILE_1CTA_128x128, TILE_1CTA_128x256, TILE_2CTA_256x256, TILE_SPLIT, TILE_MIXED = 0, 1, 2, 3, 4, 5
 

@@ -99,7 +99,7 @@ struct xc_plan_s {
     void* ws = nullptr;
     size_t ws_bytes = 0;
     bool ws_owned = false;
-    int opt_kernel = XC_I8_KERNEL_AUTO, opt_max_ctas = 0, opt_force_stage = 0, opt_debug_skip = 0, opt_epilogue = 0, opt_bk = 0;
+    int opt_kernel = XC_I8_KERNEL_AUTO, opt_max_ctas = 0, opt_force_stage = 0, opt_debug_skip = 0, opt_epilogue = 0, opt_bk = 0, opt_pdl = 1;
     long long* trace = nullptr;
     CUtensorMap tmap;
     const void* tmap_src = nullptr;
@@ -188,13 +188,17 @@ int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
     cfg.blockDim = dim3(xc::TC_THREADS);
     cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CG;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    // programmatic dependent launch: this kernel's prologue may overlap the previous kernel's tail (it executes
+    // griddepcontrol.wait before its first global access)
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = p->opt_pdl ? 2 : 1;
     auto kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, false, BK, DIAG>;
     if (CG == 2 && UMMA_N == 256 && BK == 128 && tp.trace)
         kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, (CG == 2 && UMMA_N == 256 && BK == 128), BK, DIAG>;
@@ -498,6 +502,9 @@ int xc_set_option(xc_plan_t* p, int option, int value) {
         case XC_OPT_EPILOGUE:
             if (value < XC_EPI_AUTO || value > XC_EPI_STAGED) return XC_ERR_INVALID_ARG;
             p->opt_epilogue = value;
+            return XC_OK;
+        case XC_OPT_PDL:
+            p->opt_pdl = value ? 1 : 0;
             return XC_OK;
         case XC_OPT_DEBUG_SKIP:
             p->opt_debug_skip = value & 15;

@@ -199,6 +199,12 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
     if (CG == 2) cluster_sync_all(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+    // Programmatic dependent launch: everything above (barrier init, TMEM allocation, descriptor prefetch) touched no
+    // global memory and may overlap the tail of the previous kernel in the stream; from here on this kernel reads the
+    // input / tile table and writes vis, so it first waits for that kernel to complete.  The next launch may in turn
+    // begin its own prologue while this grid drains.
+    pdl_grid_dependency_wait();
+    pdl_launch_dependents();
 
     const int KB = (p.T + Cfg::BK - 1) / Cfg::BK;
     // profiling only: CTA 0 records (SM cycle counter, global nanosecond timer) at start and end, from which the

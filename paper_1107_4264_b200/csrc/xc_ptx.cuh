@@ -98,6 +98,14 @@ __device__ __forceinline__ uint32_t elect_one() {
     return pred;
 }
 
+// ---- programmatic dependent launch ---------------------------------------------------------------
+// launch_dependents: the next kernel in the stream (if it was launched with the programmatic-serialization
+// attribute) may start its CTAs as soon as every CTA of this grid has executed this or exited.
+// grid_dependency_wait: returns once the preceding grid has completed and its memory is visible; a no-op when the
+// kernel was launched without the attribute.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // ---- TMA --------------------------------------------------------------------------------------
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tmap) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
