@@ -122,10 +122,9 @@ size_t xc_vis_bytes(const xc_plan_t* plan);     /* 32*NB*F (int32 and float alik
 size_t xc_n_baselines(const xc_plan_t* plan);
 
 /* Staging.  The tensor-core kernel reads the input through TMA, which
- * needs a 16-byte-aligned base and 16-byte-multiple row pitch (4N bytes -> N % 4 == 0); for N >= 192 the
- * library also re-pitches rows to a multiple of 128 bytes (N % 32 == 0) because that doubles the fill rate.
+ * needs a 16-byte-aligned base and a 16-byte-multiple row pitch (4N bytes -> N % 4 == 0).
  * Otherwise the input is first copied by a padding kernel into a workspace of
- * xc_workspace_bytes() bytes (0 when never needed).  The caller may hand one in (device
+ * xc_workspace_bytes() bytes.  The caller may hand one in (device
  * memory, 128-byte aligned, kept until xc_destroy or replaced); if none was set the
  * library cudaMallocs one on first need (a synchronising call) and frees it in xc_destroy. */
 size_t xc_workspace_bytes(const xc_plan_t* plan);
@@ -167,7 +166,7 @@ int xc_correlate_pipelined(xc_plan_t* plan, const int8_t* in_host_pinned, int n_
  *   different devices).  in_dev / vis_dev are the FULL block and cube of the plan (the range is
  *   addressed inside them with the plan's F as channel pitch); only vis[f0 .. f0+nf) is written.  accumulate != 0
  *   adds.  Ranges of one block may run concurrently on different streams.  Errors: INVALID_ARG for a range outside
- *   [0, F); UNSUPPORTED when the input needs the staging pass (N % 4 != 0, re-pitched N, misaligned pointer) or
+ *   [0, F); UNSUPPORTED when the input needs the staging pass (N % 4 != 0, misaligned pointer) or
  *   the SIMT kernel is selected -- those work on whole blocks only. */
 int xc_correlate_channels(xc_plan_t* plan, const int8_t* in_dev, int32_t* vis_dev, int f0, int nf, int accumulate,
                           void* cuda_stream);

@@ -81,8 +81,8 @@ __global__ void xc_stage_pad_kernel(const int8_t* __restrict__ in, uint32_t* __r
     }
 }
 
-// Same, 16 bytes (4 stations) per thread, for N % 4 == 0 and a 16-byte aligned input: used to re-pitch rows to a
-// multiple of 128 bytes (a TMA box row that straddles 128-byte lines costs two L2 requests).
+// Same, 16 bytes (4 stations) per thread, for N % 4 == 0 and a 16-byte aligned input: only reached with
+// XC_OPT_FORCE_STAGE (a plain copy into the workspace, for testing S0 on aligned shapes).
 __global__ void xc_stage_pad16_kernel(const uint4* __restrict__ in, uint4* __restrict__ out, long long rows, int n4,
                                       int npad4) {
     const long long total = rows * npad4;
