@@ -322,7 +322,20 @@ def main():
             vv = pp.new_vis()
             d = time_kernel(pp, xx, vv, stream, 10, 3)
             ms = sorted(d)[len(d) // 2]
+            # the same launch 20 times back to back between two events: what a caller streaming blocks sees (the
+            # kernels are launched with programmatic stream serialization, so launch latency and prologue overlap
+            # the previous kernel's tail -- the difference matters for the microsecond-scale small-N configs)
+            with torch.cuda.stream(stream):
+                b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                stream.synchronize()
+                b0.record(stream)
+                for _ in range(20):
+                    pp.correlate(xx, vv, stream=stream)
+                b1.record(stream)
+                stream.synchronize()
+            ms_b2b = b0.elapsed_time(b1) / 20
             by_config[name] = {"N": ww.N, "F": ww.F, "T": ww.T, "kernel_ms": ms,
+                               "back_to_back_ms": ms_b2b, "tops_back_to_back": ww.ops / (ms_b2b * 1e-3) / 1e12,
                                "tops": ww.ops / (ms * 1e-3) / 1e12,
                                "frac_i8_peak": ww.ops / (ms * 1e-3) / 1e12 / i8_peak,
                                "hbm_gbs": (ww.in_bytes + ww.vis_bytes) / (ms * 1e-3) / 1e9,

@@ -202,7 +202,13 @@ int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
     auto kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, false, BK, DIAG>;
     if (CG == 2 && UMMA_N == 256 && BK == 128 && tp.trace)
         kern = xc::xc_i8_tc_kernel<UMMA_N, CG, STAGED, (CG == 2 && UMMA_N == 256 && BK == 128), BK, DIAG>;
-    XC_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+    // the shared-memory opt-in is per function and per device: set once per (kernel variant, device), not per call
+    static int attr_done_dev[2] = {-1, -1};
+    int& done = attr_done_dev[tp.trace ? 1 : 0];
+    if (done != p->device) {
+        XC_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+        done = p->device;
+    }
     XC_CUDA(p, cudaLaunchKernelEx(&cfg, kern, p->tmap, tp));
     p->last_launches += 1;
     return XC_OK;
