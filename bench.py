@@ -179,6 +179,8 @@ def main():
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
     ap.add_argument("--no-sweep", action="store_true", help="skip the by_config sweep")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--f32-only", type=int, default=0, metavar="F",
+                    help="profiling aid: run only xc_correlate_f32 on config 3's values cut to F channels, 4 launches")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "native" else args.warmup
 
@@ -207,6 +209,24 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
         dist.barrier()
     xcb.load_library()
+
+    if args.f32_only:
+        w3 = wl.CONFIGS["cfg3"]
+        sub = wl.Workload("cfg3_f32", w3.N, args.f32_only, w3.T, w3.kind, w3.sigma, w3.seed)
+        x3 = torch.from_numpy(wl.make_input(sub)).cuda().to(torch.float32)
+        p3 = xcb.Plan(sub.N, sub.F, sub.T)
+        v3 = p3.new_vis(torch.float32)
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        p3.correlate_f32(x3, v3)
+        e[0].record()
+        for _ in range(3):
+            p3.correlate_f32(x3, v3)
+        e[1].record()
+        torch.cuda.synchronize()
+        ms = e[0].elapsed_time(e[1]) / 3
+        print(json.dumps({"f32_only": True, "N": sub.N, "F": sub.F, "T": sub.T, "kernel_ms": ms,
+                          "tflops": sub.ops / (ms * 1e-3) / 1e12}))
+        return
 
     peaks = load_peaks()
     w = wl.CONFIGS[args.workload]
