@@ -453,8 +453,8 @@ def main():
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of xc_i8_tc_kernel from `ncu --set full`
 # captures (see profiles/*.md for the command and the raw numbers); null until captured.
 TRAFFIC_NCU: dict = {
-    "cfg2": 524514048 + 237975296,        # profiles/r1_ncu_full_cfg2.md
-    "cfg4": 524439808 + 1019201000,       # profiles/r1_ncu_full_cfg4.md
+    "cfg2": 524557824 + 237699584,        # profiles/r1_ncu_full_cfg2.md
+    "cfg4": 524457216 + 1019722000,       # profiles/r1_ncu_full_cfg4.md
     "cfg5_N1024": 537382656 + 1022897000,  # profiles/r1_ncu_full_cfg5N1024.md
 }
 
