@@ -48,11 +48,12 @@ def lib() -> ctypes.CDLL:
         L.xo_channel_i8.argtypes = [p, i, i, i, i, p, i]
         L.xo_correlate_i8.argtypes = [p, i, i, i, p, i]
         L.xo_channels_i8.argtypes = [p, i, i, i, p, i, p]
+        L.xo_channels_i8_wide.argtypes = [p, i, i, i, p, i, p]
         L.xo_baseline_i8.argtypes = [p, i, i, i, i, i, i, p]
         L.xo_full_i8.argtypes = [p, i, i, i, i, p]
         L.xo_channel_f64.argtypes = [p, i, i, i, i, p]
         L.xo_channels_f64.argtypes = [p, i, i, i, p, i, p]
-        for name in ("xo_channel_i8", "xo_correlate_i8", "xo_channels_i8", "xo_baseline_i8",
+        for name in ("xo_channel_i8", "xo_correlate_i8", "xo_channels_i8", "xo_channels_i8_wide", "xo_baseline_i8",
                      "xo_full_i8", "xo_channel_f64", "xo_channels_f64"):
             getattr(L, name).restype = i
         _lib = L
@@ -108,6 +109,18 @@ def channels_i8(x: np.ndarray, fsel) -> np.ndarray:
     rc = lib().xo_channels_i8(_ptr(x), N, F, T, _ptr(fs), len(fs), _ptr(vis))
     if rc != XO_OK:
         raise OracleError(rc, "xo_channels_i8")
+    return vis
+
+
+def channels_i8_wide(x: np.ndarray, fsel=None) -> np.ndarray:
+    """Long integrations: chosen channels (default all) with int64 sums and no int32 check
+    -> int64 [len(fsel)][NB][2][2][2]; x holds the whole integration (blocks concatenated along t)."""
+    x, N, F, T = _check_in(x, np.int8)
+    fs = np.ascontiguousarray(np.asarray(range(F) if fsel is None else fsel, dtype=np.int32))
+    vis = np.empty((len(fs), n_baselines(N), 2, 2, 2), np.int64)
+    rc = lib().xo_channels_i8_wide(_ptr(x), N, F, T, _ptr(fs), len(fs), _ptr(vis))
+    if rc != XO_OK:
+        raise OracleError(rc, "xo_channels_i8_wide")
     return vis
 
 

@@ -119,6 +119,19 @@ int xo_channel_i8(const int8_t *in, int N, int F, int T, int f, int32_t *vis_f, 
     return rc;
 }
 
+/* Long integrations (I = N_p * I'): chosen channels, the same Eq. 4 sums kept in int64 with no
+ * int32 check; vis64_sel = nsel*NB*8 int64.  T is the whole integration length (blocks concatenated in time). */
+int xo_channels_i8_wide(const int8_t *in, int N, int F, int T, const int *fsel, int nsel, int64_t *vis64_sel)
+{
+    if (!in || !vis64_sel || !fsel || N < 1 || F < 1 || T < 0 || nsel < 0) return XO_ERR_ARG;
+    const size_t NB = (size_t)N * (N + 1) / 2;
+    for (int k = 0; k < nsel; ++k)
+        if (fsel[k] < 0 || fsel[k] >= F) return XO_ERR_ARG;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int k = 0; k < nsel; ++k) xo_channel_sum_i8(in, N, F, T, fsel[k], vis64_sel + (size_t)k * NB * 8);
+    return XO_OK;
+}
+
 /* All channels; vis = F*NB*8 int32. */
 int xo_correlate_i8(const int8_t *in, int N, int F, int T, int32_t *vis, int accumulate)
 {

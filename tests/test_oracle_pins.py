@@ -272,3 +272,32 @@ def test_config3_tone_structure():
             den += F
     mean = num / den
     assert abs(mean.real / (4 * T) - 1) < 0.1 and abs(mean.imag) < 0.1 * 4 * T
+
+
+def test_wide_oracle_long_integration():
+    """Long integrations: the int64 entry point equals the int32 one where that fits, equals
+    numpy's complex x x^H beyond it, and reaches the closed form 2 * 128^2 * T for all -128 input where int32 overflows."""
+    x = wl.full_range(6, 3, 50, seed=21)
+    assert np.array_equal(xo.channels_i8_wide(x), xo.correlate_i8(x).astype(np.int64))
+    assert np.array_equal(xo.channels_i8_wide(x, [2, 0]), xo.correlate_i8(x).astype(np.int64)[[2, 0]])
+    T = 70000                                                  # > XC_MAX_T: 2 * 128^2 * T = 2 293 760 000 > 2^31
+    big = np.full((T, 1, 2, 2, 2), -128, np.int8)
+    w = xo.channels_i8_wide(big)
+    assert w[0, :, :, :, 0].min() == w[0, :, :, :, 0].max() == 2 * 128 * 128 * T > 2 ** 31
+    assert (w[..., 1] == 0).all()
+    with pytest.raises(xo.OracleError):
+        xo.correlate_i8(big)
+    # random long block against numpy (complex128 is exact here: |sums| < 2^53)
+    y = wl.full_range(3, 2, 66000, seed=22)
+    z = y.astype(np.float64)
+    zc = (z[..., 0] + 1j * z[..., 1]).reshape(66000, 2, 6)      # [t][f][(s,p)]
+    ref = np.einsum("tfa,tfb->fab", zc, zc.conj())
+    w = xo.channels_i8_wide(y)
+    for j in range(3):
+        for i in range(j + 1):
+            for pi in range(2):
+                for pj in range(2):
+                    v = ref[:, 2 * i + pi, 2 * j + pj]
+                    b = j * (j + 1) // 2 + i
+                    assert np.array_equal(w[:, b, pi, pj, 0], np.rint(v.real).astype(np.int64))
+                    assert np.array_equal(w[:, b, pi, pj, 1], np.rint(v.imag).astype(np.int64))
