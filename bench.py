@@ -419,6 +419,22 @@ def main():
                                 "total_ms": 1e3 * tot, "copy_alone_ms": 1e3 * t_copy, "compute_alone_ms": 1e3 * t_comp,
                                 "h2d_gbs": 8 * w5.in_bytes / tot / 1e9, "tops": 8 * w5.ops / tot / 1e12,
                                 "overlap_efficiency": max(t_copy, t_comp) / tot}
+        # the integrated run (Fig. 7): the same 8 blocks through xc_integrate -- int64 widening of the
+        # int32 partial sums and the copy of the result back to the host inside the timed region
+        v64 = torch.empty(p5.vis_shape(), dtype=torch.int64, device="cuda")
+        v64h = torch.empty(p5.vis_shape(), dtype=torch.int64).pin_memory()
+        p5.integrate(host, dev2, v5, v64, stream, s2, vis64_host=v64h)
+        stream.synchronize()
+        t0 = time.perf_counter()
+        p5.integrate(host, dev2, v5, v64, stream, s2, vis64_host=v64h)
+        stream.synchronize()
+        tot_i = time.perf_counter() - t0
+        extras["integrated"] = {"workload": "cfg5_N1024 x 8 pinned host blocks (16384 samples), xc_integrate: H2D pipeline, "
+                                            "X-engine, int64 widening, D2H of the int64 result",
+                                "total_ms": 1e3 * tot_i, "tops": 8 * w5.ops / tot_i / 1e12,
+                                "h2d_bytes": 8 * w5.in_bytes, "d2h_bytes": 2 * w5.vis_bytes,
+                                "pcie_floor_ms": 1e3 * (t_copy + 2 * w5.vis_bytes / (8 * w5.in_bytes / t_copy))}
+        del v64, v64h
         p5.close()
         del host, dev2, v5
         torch.cuda.empty_cache()

@@ -161,6 +161,16 @@ int xc_correlate_f32(xc_plan_t* plan, const float* in_dev, float* vis_dev, int a
 int xc_correlate_pipelined(xc_plan_t* plan, const int8_t* in_host_pinned, int n_blocks, int8_t* dev_buf2,
                            int32_t* vis_dev, void* compute_stream, void* copy_stream);
 
+/* xc_integrate -- long integration I = n_blocks * T ("I = N_p I'"; the integrated run of Sec. 6 / Fig. 7,
+ *   PAPER.md:283): Algorithm 1 over n_blocks pinned host blocks as in xc_correlate_pipelined, with the int32 partial sums
+ *   (exact for at most XC_MAX_T samples) added into an int64 cube after every floor(XC_MAX_T / T) blocks, so the result is
+ *   exact for ANY integration length.  vis32_dev: scratch cube of xc_vis_bytes(); vis64_dev: int64 [F][NB][2][2][2]
+ *   (2 * xc_vis_bytes(), 16-byte aligned), overwritten with the sum over all blocks; vis64_host: if not NULL the result is
+ *   also copied there (the paper's "matrix_h <- matrix_d"), asynchronously on compute_stream.  Returns after
+ *   enqueueing; the caller synchronises compute_stream. */
+int xc_integrate(xc_plan_t* plan, const int8_t* in_host_pinned, int n_blocks, int8_t* dev_buf2, int32_t* vis32_dev,
+                 int64_t* vis64_dev, int64_t* vis64_host, void* compute_stream, void* copy_stream);
+
 /* xc_correlate_channels -- the same operation restricted to channels [f0, f0 + nf) of the plan's F ("evaluated
  *   independently for every frequency"; the paper's multi-GPU plan hands different channels to
  *   different devices).  in_dev / vis_dev are the FULL block and cube of the plan (the range is

@@ -22,7 +22,7 @@ TILE_AUTO, TILE_1CTA_128x128, TILE_1CTA_128x256, TILE_2CTA_256x256, TILE_SPLIT, 
 EXPORTED_SYMBOLS = (
     "xc_plan", "xc_destroy", "xc_in_bytes", "xc_in_bytes_f32", "xc_vis_bytes", "xc_n_baselines",
     "xc_workspace_bytes", "xc_set_workspace", "xc_set_option", "xc_correlate", "xc_correlate_acc",
-    "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_tile_count", "xc_tile_get",
+    "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_integrate", "xc_tile_count", "xc_tile_get",
     "xc_debug_set_trace", "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error",
     "xc_version",
 )
@@ -59,6 +59,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_correlate": (i, [p, p, p, p]), "xc_correlate_acc": (i, [p, p, p, p]),
         "xc_correlate_f32": (i, [p, p, p, i, p]),
         "xc_correlate_channels": (i, [p, p, p, i, i, i, p]),
+        "xc_integrate": (i, [p, p, i, p, p, p, p, p, p]),
         "xc_correlate_pipelined": (i, [p, p, i, p, p, p, p]),
         "xc_correlate_host": (i, [p, p, p, p, p, p]),
         "xc_debug_set_trace": (i, [p, p]),
@@ -264,6 +265,27 @@ class Plan:
             ctypes.c_void_p(compute_stream.cuda_stream), ctypes.c_void_p(copy_stream.cuda_stream)),
             "xc_correlate_pipelined")
         return vis
+
+    def integrate(self, blocks_host, dev_buf2, vis32, vis64, compute_stream, copy_stream, vis64_host=None):
+        """Long integration over pinned host blocks [n_blocks][T][F][N][2][2] into the int64 CUDA cube vis64 (and the
+        pinned int64 host cube vis64_host if given).  Enqueues and returns; sync compute_stream."""
+        import torch
+        if not (blocks_host.dtype == torch.int8 and blocks_host.is_contiguous() and not blocks_host.is_cuda
+                and tuple(blocks_host.shape[1:]) == self.in_shape()):
+            raise ValueError("blocks_host must be a contiguous CPU int8 tensor [n_blocks][T][F][N][2][2]")
+        if dev_buf2.numel() * dev_buf2.element_size() < 2 * self.in_bytes:
+            raise ValueError("dev_buf2 too small")
+        self._chk_vis(vis32, torch.int32)
+        self._chk_vis(vis64, torch.int64)
+        if vis64_host is not None and not (vis64_host.dtype == torch.int64 and vis64_host.is_contiguous()
+                                           and tuple(vis64_host.shape) == self.vis_shape() and not vis64_host.is_cuda):
+            raise ValueError("vis64_host must be a contiguous CPU int64 tensor of the cube's shape")
+        self._check(lib().xc_integrate(
+            self._h, ctypes.c_void_p(blocks_host.data_ptr()), int(blocks_host.shape[0]),
+            ctypes.c_void_p(dev_buf2.data_ptr()), ctypes.c_void_p(vis32.data_ptr()), ctypes.c_void_p(vis64.data_ptr()),
+            ctypes.c_void_p(vis64_host.data_ptr() if vis64_host is not None else 0),
+            ctypes.c_void_p(compute_stream.cuda_stream), ctypes.c_void_p(copy_stream.cuda_stream)), "xc_integrate")
+        return vis64
 
     def correlate_host(self, x_host, vis_host, in_dev, vis_dev, stream=None):
         """End to end with HOST buffers (H2D copy, X-engine, D2H copy, stream sync)."""

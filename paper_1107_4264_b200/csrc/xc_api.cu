@@ -593,6 +593,54 @@ int xc_correlate_pipelined(xc_plan_t* p, const int8_t* in_host, int n_blocks, in
     return XC_OK;
 }
 
+int xc_integrate(xc_plan_t* p, const int8_t* in_host, int n_blocks, int8_t* dev_buf2, int32_t* vis32_dev,
+                 int64_t* vis64_dev, int64_t* vis64_host, void* compute_stream, void* copy_stream) {
+    if (!p || !in_host || !dev_buf2 || !vis32_dev || !vis64_dev || n_blocks < 1) return XC_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(dev_buf2) & 127u) || (reinterpret_cast<uintptr_t>(vis64_dev) & 15u)) return XC_ERR_ALIGNMENT;
+    int rc = ensure_device(p);
+    if (rc != XC_OK) return rc;
+    cudaStream_t cs = static_cast<cudaStream_t>(compute_stream), xs = static_cast<cudaStream_t>(copy_stream);
+    for (int k = 0; k < 2; ++k) {
+        if (!p->ev_copied[k]) XC_CUDA(p, cudaEventCreateWithFlags(&p->ev_copied[k], cudaEventDisableTiming));
+        if (!p->ev_free[k]) XC_CUDA(p, cudaEventCreateWithFlags(&p->ev_free[k], cudaEventDisableTiming));
+    }
+    if (!p->ev_entry) XC_CUDA(p, cudaEventCreateWithFlags(&p->ev_entry, cudaEventDisableTiming));
+    const size_t blk = xc_in_bytes(p);
+    const int group = XC_MAX_T / p->T;              // blocks whose int32 partial sum cannot overflow (>= 1)
+    const long long n4 = static_cast<long long>(p->F) * p->NB * 2;   // int4 quadruples in the cube
+    long long wblocks = (n4 + 255) / 256;
+    if (wblocks > 148LL * 16) wblocks = 148LL * 16;
+    int launches = 0;
+    XC_CUDA(p, cudaEventRecord(p->ev_entry, cs));
+    XC_CUDA(p, cudaStreamWaitEvent(xs, p->ev_entry, 0));
+    XC_CUDA(p, cudaMemcpyAsync(dev_buf2, in_host, blk, cudaMemcpyHostToDevice, xs));
+    XC_CUDA(p, cudaEventRecord(p->ev_copied[0], xs));
+    for (int b = 0; b < n_blocks; ++b) {
+        if (b + 1 < n_blocks) {
+            const int nb = (b + 1) & 1;
+            if (b >= 1) XC_CUDA(p, cudaStreamWaitEvent(xs, p->ev_free[nb], 0));
+            XC_CUDA(p, cudaMemcpyAsync(dev_buf2 + nb * blk, in_host + static_cast<size_t>(b + 1) * blk, blk,
+                                       cudaMemcpyHostToDevice, xs));
+            XC_CUDA(p, cudaEventRecord(p->ev_copied[nb], xs));
+        }
+        XC_CUDA(p, cudaStreamWaitEvent(cs, p->ev_copied[b & 1], 0));
+        rc = correlate_i8(p, dev_buf2 + (b & 1) * blk, vis32_dev, compute_stream, (b % group) ? 1 : 0);
+        if (rc != XC_OK) return rc;
+        launches += p->last_launches;
+        XC_CUDA(p, cudaEventRecord(p->ev_free[b & 1], cs));
+        if ((b + 1) % group == 0 || b + 1 == n_blocks) {
+            xc::xc_widen_kernel<<<static_cast<unsigned>(wblocks), 256, 0, cs>>>(
+                reinterpret_cast<const int4*>(vis32_dev), reinterpret_cast<longlong2*>(vis64_dev), n4, b < group ? 1 : 0);
+            XC_CUDA(p, cudaGetLastError());
+            launches += 1;
+        }
+    }
+    if (vis64_host)
+        XC_CUDA(p, cudaMemcpyAsync(vis64_host, vis64_dev, 2 * xc_vis_bytes(p), cudaMemcpyDeviceToHost, cs));
+    p->last_launches = launches;
+    return XC_OK;
+}
+
 int xc_correlate_channels(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, int f0, int nf, int accumulate,
                           void* stream) {
     return correlate_i8(p, in_dev, vis_dev, stream, accumulate ? 1 : 0, f0, nf);

@@ -94,4 +94,20 @@ __global__ void xc_stage_pad16_kernel(const uint4* __restrict__ in, uint4* __res
     }
 }
 
+// (c) Long integrations (I = N_p * I'): vis64 (+)= vis32, four values per thread.  int32 partial
+// sums of at most XC_MAX_T samples are exact; this widening add makes any integration length exact in int64.
+__global__ void xc_widen_kernel(const int4* __restrict__ v32, longlong2* __restrict__ v64, long long n4, int first) {
+    for (long long k = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; k < n4;
+         k += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const int4 a = __ldcs(v32 + k);
+        longlong2 lo = make_longlong2(a.x, a.y), hi = make_longlong2(a.z, a.w);
+        if (!first) {
+            const longlong2 o0 = v64[2 * k], o1 = v64[2 * k + 1];
+            lo.x += o0.x; lo.y += o0.y; hi.x += o1.x; hi.y += o1.y;
+        }
+        v64[2 * k] = lo;
+        v64[2 * k + 1] = hi;
+    }
+}
+
 }  // namespace xc

@@ -242,6 +242,42 @@ def test_host_call_chunked_overlap():
     assert np.array_equal(vh.numpy(), ref)
 
 
+def test_integrate_long_integration_int64():
+    """xc_integrate: Algorithm 1 with int64 widening.  (a) all -128 over 3 x 30000 samples leaves
+    int32 (2 * 128^2 * 90000 > 2^31) and must hit the closed form; (b) random full-range blocks against the oracle's
+    int64 sums over the concatenated integration, with a widening period of 2 blocks and a ragged last group; the host
+    copy of the result is the same cube."""
+    N, F, T, nblk = 8, 2, 30000, 3
+    p = xcb.Plan(N, F, T)
+    host = torch.full((nblk,) + p.in_shape(), -128, dtype=torch.int8).pin_memory()
+    dev2 = torch.empty(2 * p.in_bytes, dtype=torch.int8, device="cuda")
+    v32 = p.new_vis()
+    v64 = torch.full(p.vis_shape(), -7, dtype=torch.int64, device="cuda")
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    p.integrate(host, dev2, v32, v64, s1, s2)
+    s1.synchronize()
+    got = v64.cpu().numpy()
+    assert (got[..., 0] == 2 * 128 * 128 * T * nblk).all() and (got[..., 1] == 0).all()
+    assert 2 * 128 * 128 * T * nblk > 2 ** 31
+
+    N, F, T, nblk = 40, 3, 30000, 7                          # group = 65535 // 30000 = 2 blocks -> widenings after 2, 4, 6, 7
+    blocks = [wl.full_range(N, F, T, seed=300 + k) for k in range(nblk)]
+    p = xcb.Plan(N, F, T)
+    host = torch.from_numpy(np.stack(blocks)).pin_memory()
+    dev2 = torch.empty(2 * p.in_bytes, dtype=torch.int8, device="cuda")
+    v32 = p.new_vis()
+    v64 = torch.full(p.vis_shape(), -7, dtype=torch.int64, device="cuda")
+    v64h = torch.zeros(p.vis_shape(), dtype=torch.int64).pin_memory()
+    p.integrate(host, dev2, v32, v64, s1, s2, vis64_host=v64h)
+    s1.synchronize()
+    assert p.last_launches == nblk + 4
+    ref = xo.channels_i8_wide(np.concatenate(blocks, axis=0))
+    assert np.array_equal(v64.cpu().numpy(), ref)
+    assert np.array_equal(v64h.numpy(), ref)
+    assert np.abs(ref).max() > 2 ** 31                       # the case really needs the widening
+
+
 def test_cuda_graph_capture_and_pdl_chain():
     """xc_correlate / xc_correlate_acc are plain stream work (after the first call has created the plan's device
     state): they can be captured into a CUDA graph and replayed, and a chain of accumulate calls keeps its
