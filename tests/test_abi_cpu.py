@@ -130,3 +130,22 @@ def test_shard_channels_partition():
             assert all(parts[k][1] == parts[k + 1][0] for k in range(ws - 1))
             sizes = [hi - lo for lo, hi in parts]
             assert max(sizes) - min(sizes) <= 1
+
+
+def test_option_validation():
+    """xc_set_option rejects values outside each option's range and unknown options (no device needed)."""
+    p = xcb.Plan(64, 4, 128)
+    L, h = xcb.lib(), p._h
+    ok = [(xcb.OPT_I8_KERNEL, 2), (xcb.OPT_MAX_CTAS, 0), (xcb.OPT_MAX_CTAS, 37), (xcb.OPT_FORCE_STAGE, 1), (xcb.OPT_TILE, 5),
+          (xcb.OPT_TILE, 0), (xcb.OPT_EPILOGUE, 2), (xcb.OPT_BK, 256), (xcb.OPT_BK, 0), (xcb.OPT_PDL, 0), (xcb.OPT_PDL, 1)]
+    bad = [(xcb.OPT_I8_KERNEL, 3), (xcb.OPT_MAX_CTAS, -1), (xcb.OPT_TILE, 6), (xcb.OPT_TILE, -1), (xcb.OPT_EPILOGUE, 3),
+           (xcb.OPT_BK, 96), (99, 0)]
+    for opt, val in ok:
+        assert L.xc_set_option(h, opt, val) == 0, (opt, val)
+    for opt, val in bad:
+        assert L.xc_set_option(h, opt, val) == -1, (opt, val)
+    assert L.xc_set_option(None, xcb.OPT_TILE, 0) == -1
+    # every tile mode keeps an exact-cover schedule after switching back and forth
+    for mode in (5, 3, 4, 1, 0):
+        p.set_option(xcb.OPT_TILE, mode)
+        assert len(p.tiles()) >= 1
