@@ -235,9 +235,13 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
             const bool a_in_b = DIAG || ((m_a >= m_b) && (m_a < m_b + Cfg::B_BOXES * 128));   // diagonal: A rows are B rows
             // DIAG: a row block that lies in the tile's second column box needs nothing of the first one (every pair
             // there has i > j): only box 1 is loaded and the MMA shrinks to N = 128
+            // Such a tile keeps 32 KB / 512 tensor cycles per stage by putting TWO time slices of box 1 into the stage's
+            // two box slots (256 samples per stage): a 128-sample stage of N = 128 MMAs would hold only 256 tensor cycles,
+            // less than the barrier round trip of a stage.
             const int h0 = (DIAG && m_a >= m_b + 128) ? 1 : 0;
-            const uint32_t my_bytes = a_in_b ? static_cast<uint32_t>(Cfg::B_BYTES - h0 * Cfg::BOX_BYTES) : Cfg::STAGE_BYTES;
-            for (int kb = 0; kb < KB; ++kb) {
+            const uint32_t my_bytes = a_in_b ? static_cast<uint32_t>(Cfg::B_BYTES) : Cfg::STAGE_BYTES;
+            const int KBt = h0 ? (p.T + 2 * Cfg::BK - 1) / (2 * Cfg::BK) : KB;
+            for (int kb = 0; kb < KBt; ++kb) {
                 const bool tr = TRACE && p.trace && blockIdx.x == 0 && it < TC_TRACE_ITERS && elected;
                 if (tr) p.trace[(0 * TC_TRACE_ITERS + it) * 4 + 0] = clock64();
                 mbar_wait(empty_bar(stage), phase ^ 1u);
@@ -245,15 +249,20 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
                 if (elected) {
                     const uint32_t sa = ring0 + stage * Cfg::STAGE_BYTES;
                     const uint32_t sb = sa + Cfg::A_BYTES;
-                    const int t0 = kb * Cfg::BK;
+                    const int t0 = kb * Cfg::BK * (1 + h0);
                     if ((p.debug_skip & 1) && (n != 0 || kb >= Cfg::STAGES)) {
                         if (rank == 0) mbar_arrive(full_bar(stage));
+                    } else if (DIAG && h0) {
+                        const bool two = t0 + Cfg::BK < p.T;     // the second time slice exists
+                        mbar_arrive_expect_tx(full_bar(stage), two ? 2 * Cfg::BOX_BYTES : Cfg::BOX_BYTES);
+                        tma_load_3d(sb, &tmap, full_bar(stage), m_b + 128, f, t0);
+                        if (two) tma_load_3d(sb + Cfg::BOX_BYTES, &tmap, full_bar(stage), m_b + 128, f, t0 + Cfg::BK);
                     } else if (CG == 1) {
                         mbar_arrive_expect_tx(full_bar(stage), my_bytes);
                         if (!a_in_b) tma_load_3d(sa, &tmap, full_bar(stage), m_a, f, t0);
 #pragma unroll
                         for (int h = 0; h < Cfg::B_BOXES; ++h)
-                            if (h >= h0) tma_load_3d(sb + h * Cfg::BOX_BYTES, &tmap, full_bar(stage), m_b + 128 * h, f, t0);
+                            tma_load_3d(sb + h * Cfg::BOX_BYTES, &tmap, full_bar(stage), m_b + 128 * h, f, t0);
                     } else {
                         // both CTAs' bytes are counted on the LEADER's barrier (a_in_b is the same in both)
                         const uint32_t lead_full = mapa_u32(full_bar(stage), 0);
@@ -291,14 +300,17 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
                 const int m_b = static_cast<int>(tb >> 16) * UMMA_N;
                 const bool a_in_b = DIAG || ((m_a >= m_b) && (m_a < m_b + Cfg::B_BOXES * 128));
                 // byte offset of the A operand inside a stage: its own box, or the B box holding the same rows
-                const uint32_t a_off = a_in_b ? static_cast<uint32_t>(Cfg::A_BYTES + ((m_a - m_b) >> 7) * Cfg::BOX_BYTES) : 0u;
-                // DIAG, row block in the second column box: N = 128 MMA on box 1 into the accumulator's upper 128 columns
+                // DIAG, row block in the second column box: N = 128 MMAs on box 1 (A = B = that box; the stage's two slots
+                // hold two consecutive time slices of it) into the accumulator's upper 128 columns
                 const uint32_t h0 = (DIAG && m_a >= m_b + 128) ? 1u : 0u;
+                const uint32_t a_off = h0 ? 0u : (a_in_b ? static_cast<uint32_t>(Cfg::A_BYTES + ((m_a - m_b) >> 7) * Cfg::BOX_BYTES) : 0u);
                 const uint32_t idesc_t = h0 ? make_idesc_i8_mn(Cfg::M, 128) : idesc;
+                const int BKt = Cfg::BK * (1 + static_cast<int>(h0));           // samples per stage of this tile
+                const int KBt = (p.T + BKt - 1) / BKt;
                 mbar_wait(tempty_bar(buf), ((tphase >> buf) & 1u) ^ 1u);  // epilogues have drained this accumulator
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + buf * UMMA_N + h0 * 128u;
-                for (int kb = 0; kb < KB; ++kb) {
+                for (int kb = 0; kb < KBt; ++kb) {
                     const bool tr = TRACE && p.trace && blockIdx.x == 0 && it < TC_TRACE_ITERS && elected;
                     if (tr) p.trace[(1 * TC_TRACE_ITERS + it) * 4 + 0] = clock64();
                     mbar_wait(full_bar(stage), phase);
@@ -307,11 +319,11 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
                     if (elected) {
                         const uint32_t sa = ring0 + stage * Cfg::STAGE_BYTES;
                         const uint64_t adesc = make_smem_desc_mn_sw128(sa + a_off, Cfg::BOX_BYTES, 1024);
-                        const uint64_t bdesc = make_smem_desc_mn_sw128(sa + Cfg::A_BYTES + h0 * Cfg::BOX_BYTES, Cfg::BOX_BYTES, 1024);
-                        const int rows = min(Cfg::BK, p.T - kb * Cfg::BK);           // valid samples in this stage
+                        const uint64_t bdesc = make_smem_desc_mn_sw128(sa + Cfg::A_BYTES, Cfg::BOX_BYTES, 1024);
+                        const int rows = min(BKt, p.T - kb * BKt);                // valid samples in this stage
                         const int nk = (rows + TC_UMMA_K - 1) / TC_UMMA_K;       // rows beyond T are TMA zero fill
 #pragma unroll
-                        for (int ks = 0; ks < Cfg::BK / TC_UMMA_K; ++ks) {
+                        for (int ks = 0; ks < (DIAG ? 2 : 1) * Cfg::BK / TC_UMMA_K; ++ks) {
                             if (ks < nk && !(p.debug_skip & 2)) {
                                 // K advance: 32 samples = 4 swizzle atoms = 4096 B -> +256 in the address field
                                 umma_i8<CG>(d_tmem, adesc + static_cast<uint64_t>(ks * 256),
@@ -320,7 +332,7 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
                         }
                         if (tr) p.trace[(1 * TC_TRACE_ITERS + it) * 4 + 2] = clock64();
                         umma_commit<CG>(empty_bar(stage));  // frees the ring slot (in both CTAs) when these MMAs retire
-                        if (kb == KB - 1) umma_commit<CG>(tfull_bar(buf));  // accumulator complete -> epilogues
+                        if (kb == KBt - 1) umma_commit<CG>(tfull_bar(buf));  // accumulator complete -> epilogues
                     }
                     __syncwarp();
                     if (tr) p.trace[(1 * TC_TRACE_ITERS + it) * 4 + 3] = clock64();
@@ -353,21 +365,26 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
             if (w_next >= 0) tb_next = __ldg(p.tiles + w_next % p.tiles_per_f);
             if (tb == TC_TILE_EMPTY) continue;
             const int i0 = static_cast<int>(tb & 0xFFFFu) * Cfg::SI + 32 * static_cast<int>(rank) + 8 * q;
-            const int j0 = static_cast<int>(tb >> 16) * Cfg::SJ + 8 * CHUNKS * half;   // first station of this warp's columns
+            // DIAG tile whose row block sits in the second column box: only accumulator columns 128..255 exist, and
+            // all eight warps share them (two 32-column chunks each instead of four)
+            const bool h0 = DIAG && (static_cast<int>(tb & 0xFFFFu) * Cfg::SI >= static_cast<int>(tb >> 16) * Cfg::SJ + 32);
+            const int nchunks = h0 ? CHUNKS / 2 : CHUNKS;
+            const int col0 = h0 ? 128 + 32 * nchunks * half : 32 * CHUNKS * half;    // first accumulator column of this warp
+            const int j0 = static_cast<int>(tb >> 16) * Cfg::SJ + col0 / 4;           // first station of this warp's columns
             const int i = i0 + (lane >> 2);                     // i0 = first station of this warp's rows
             int32_t* visf = p.vis + static_cast<long long>(f) * p.NB * 8;
 
             mbar_wait(tfull_bar(buf), (tphase >> buf) & 1u);
             tc_fence_after();
             if (tr) p.trace[(2 * TC_TRACE_ITERS + it) * 4 + 1] = clock64();
-            const uint32_t taddr0 = tmem_base + (static_cast<uint32_t>(32 * q) << 16) + buf * UMMA_N + 32 * CHUNKS * half;
+            const uint32_t taddr0 = tmem_base + (static_cast<uint32_t>(32 * q) << 16) + buf * UMMA_N + col0;
             if (STAGED) {
                 // the previous tile's bulk stores must have finished reading the staging buffer
                 if (warp < 4) bulk_wait_read0();            // warps 2-3 issue the bulk stores
                 named_bar_sync(1, 32 * TC_EPI_WARPS);
             }
 #pragma unroll 1
-            for (int cc = 0; cc < CHUNKS; ++cc) {
+            for (int cc = 0; cc < nchunks; ++cc) {
                 const int jbase = j0 + 8 * cc;
                 if (jbase >= p.N || jbase + 7 < i0) continue;  // warp-uniform: nothing of this chunk is stored
                 uint32_t v[32];
