@@ -242,6 +242,26 @@ def test_host_call_chunked_overlap():
     assert np.array_equal(vh.numpy(), ref)
 
 
+def test_random_shapes_auto_mode():
+    """Seeded sweep of ragged shapes through the launch configuration xc_plan picks by itself (AUTO), overwrite and
+    accumulate, against the oracle -- bit-exact, every output written (poison check via the accumulate identity)."""
+    rng = np.random.default_rng(20261104)
+    shapes = [(int(rng.integers(1, 301)), int(rng.integers(1, 6)), int(rng.integers(1, 701))) for _ in range(36)]
+    shapes += [(256, 2, 129), (255, 1, 128), (260, 1, 127), (64, 5, 1), (129, 2, 256)]
+    for N, F, T in shapes:
+        x = wl.full_range(N, F, T, seed=7 * N + T)
+        ref = xo.correlate_i8(x)
+        p = xcb.Plan(N, F, T)
+        xd = torch.from_numpy(x).cuda()
+        vis = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+        p.correlate(xd, vis)
+        got = vis.cpu().numpy()
+        assert np.array_equal(got, ref), (N, F, T)
+        p.correlate_acc(xd, vis)
+        assert np.array_equal(vis.cpu().numpy(), 2 * ref), (N, F, T, "acc")
+        p.close()
+
+
 def test_integrate_long_integration_int64():
     """xc_integrate: Algorithm 1 with int64 widening.  (a) all -128 over 3 x 30000 samples leaves
     int32 (2 * 128^2 * 90000 > 2^31) and must hit the closed form; (b) random full-range blocks against the oracle's
