@@ -400,6 +400,25 @@ def test_f32_against_fp64_oracle(N, F, T):
     f32_tolerance_check(got, xo.channels_f64(x), N)
 
 
+def test_f32_random_shapes_exact_on_integer_input_and_accumulate():
+    """The fp32 kernel's 16 x 16-station warp blocks and diagonal skipping at ragged sizes: integer-valued input keeps
+    every fp32 sum exact, so the result must equal the integer oracle bit for bit; accumulate adds exactly."""
+    rng = np.random.default_rng(99)
+    shapes = [(int(rng.integers(1, 200)), int(rng.integers(1, 4)), int(rng.integers(1, 300))) for _ in range(16)]
+    shapes += [(15, 1, 16), (16, 1, 17), (17, 2, 15), (47, 1, 33), (48, 1, 48), (49, 1, 31), (96, 2, 50), (97, 1, 64)]
+    for N, F, T in shapes:
+        x = wl.full_range(N, F, T, seed=13 * N + T)
+        ref = xo.correlate_i8(x).astype(np.float32)
+        p = xcb.Plan(N, F, T)
+        xd = torch.from_numpy(x).cuda().to(torch.float32)
+        vis = torch.full(p.vis_shape(), float("nan"), dtype=torch.float32, device="cuda")
+        p.correlate_f32(xd, vis)
+        assert np.array_equal(vis.cpu().numpy(), ref), (N, F, T)
+        p.correlate_f32(xd, vis, accumulate=True)
+        assert np.array_equal(vis.cpu().numpy(), 2 * ref), (N, F, T, "acc")
+        p.close()
+
+
 def test_f32_equals_int8_for_integer_input():
     """Config 3's values as float: all products and sums are exact in fp32 -> identical results."""
     w = wl.Workload("cfg3small", 256, 4, 1000, "gauss_tone", 4.0, 1003)
