@@ -27,6 +27,10 @@
  * Streams are cudaStream_t passed as void*; all device work is enqueued on the stream
  * given, asynchronously, with no hidden device synchronisation unless stated.
  *
+ * A plan binds to the CUDA device that is current at its first compute call (its tile table, workspace and helper
+ * streams live there; later calls with another device current return XC_ERR_INVALID_ARG).  A plan is not thread-safe:
+ * calls on one plan must not overlap in time on the host; different plans are independent.
+ *
  * Every function returns an xc_status (0 = OK, negative = error); nothing is thrown
  * across this boundary; on error no output is promised.  There is no CPU fallback: on a
  * machine without an sm_100 GPU every compute entry point returns XC_ERR_CUDA /

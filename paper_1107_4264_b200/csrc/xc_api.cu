@@ -215,9 +215,15 @@ int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
 }
 
 int ensure_device(xc_plan_t* p) {
-    if (p->dev_ready) return XC_OK;
     int dev = 0;
     XC_CUDA(p, cudaGetDevice(&dev));
+    if (p->dev_ready) {
+        if (dev != p->device) {   // the plan's tables, workspace and streams live on the device of its first compute call
+            p->last_err = "plan is bound to another CUDA device than the current one";
+            return XC_ERR_INVALID_ARG;
+        }
+        return XC_OK;
+    }
     int major = 0, sms = 0;
     XC_CUDA(p, cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
     XC_CUDA(p, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
