@@ -124,6 +124,26 @@ def channels_i8_wide(x: np.ndarray, fsel=None) -> np.ndarray:
     return vis
 
 
+def unpack_i4(x4: np.ndarray) -> np.ndarray:
+    """4-bit complex samples ("typically four to eight bits of precision is sufficient"; two's complement,
+    PAPER.md:45).  The paper fixes no packing; reading 17: one byte per complex sample, LOW nibble = real part,
+    HIGH nibble = imaginary part, each a two's-complement 4-bit integer in [-8, 7].
+    x4: uint8 [T][F][N][2 pol] -> int8 [T][F][N][2][2 re,im].  Written out per nibble: value = n if n < 8 else n - 16."""
+    x4 = np.ascontiguousarray(x4)
+    if x4.dtype != np.uint8 or x4.ndim != 4 or x4.shape[3] != 2:
+        raise ValueError("packed input must be uint8 [T][F][N][2]")
+    lo = (x4 & np.uint8(0x0F)).astype(np.int16)
+    hi = (x4 >> np.uint8(4)).astype(np.int16)
+    re = np.where(lo < 8, lo, lo - 16)
+    im = np.where(hi < 8, hi, hi - 16)
+    return np.stack([re, im], axis=-1).astype(np.int8)
+
+
+def correlate_i4(x4: np.ndarray) -> np.ndarray:
+    """Eq. 4 on 4-bit samples: unpack, then the int8 definition.  -> int32 [F][NB][2][2][2]."""
+    return correlate_i8(unpack_i4(x4))
+
+
 def baseline_i8(x: np.ndarray, f: int, i: int, j: int) -> np.ndarray:
     """One station pair (any i, j) of one channel -> int64 [2][2][2]."""
     x, N, F, T = _check_in(x, np.int8)

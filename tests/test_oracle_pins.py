@@ -301,3 +301,25 @@ def test_wide_oracle_long_integration():
                     b = j * (j + 1) // 2 + i
                     assert np.array_equal(w[:, b, pi, pj, 0], np.rint(v.real).astype(np.int64))
                     assert np.array_equal(w[:, b, pi, pj, 1], np.rint(v.imag).astype(np.int64))
+
+
+def test_unpack_i4_all_codes_and_hand_example():
+    """4-bit format (reading 17): low nibble real, high nibble imaginary, two's complement.  All 256 byte
+    codes against Python integer arithmetic; one product by hand: byte 0x2F = (-1 + 2i), byte 0x9A = (-6 - 7i):
+    (-1 + 2i) conj(-6 - 7i) = (-1 + 2i)(-6 + 7i) = 6 - 7i - 12i - 14 = -8 - 19i."""
+    codes = np.arange(256, dtype=np.uint8).reshape(256, 1, 1, 1).repeat(2, axis=3)
+    got = xo.unpack_i4(codes)
+    for b in range(256):
+        re = (b & 15) - 16 if (b & 15) >= 8 else (b & 15)
+        im = (b >> 4) - 16 if (b >> 4) >= 8 else (b >> 4)
+        assert tuple(got[b, 0, 0, 0]) == (re, im) and tuple(got[b, 0, 0, 1]) == (re, im)
+    assert got.min() == -8 and got.max() == 7
+    x4 = np.zeros((1, 1, 2, 2), np.uint8)
+    x4[0, 0, 0, 0] = 0x2F
+    x4[0, 0, 1, 0] = 0x9A
+    v = xo.correlate_i4(x4)
+    assert tuple(v[0, 1, 0, 0]) == (-8, -19)                  # baseline (i=0, j=1), pols (0, 0)
+    assert tuple(v[0, 0, 0, 0]) == (5, 0) and tuple(v[0, 2, 0, 0]) == (85, 0)   # |-1+2i|^2, |-6-7i|^2
+    x = wl.packed_i4(5, 2, 40, seed=4)
+    assert np.array_equal(xo.correlate_i4(x), xo.correlate_i8(xo.unpack_i4(x)))
+    assert xo.unpack_i4(x)[0, 0, 0].tolist() == [[-8, -8], [7, 7]]

@@ -20,7 +20,7 @@ from dataclasses import dataclass
 import numpy as np
 
 __all__ = ["Workload", "CONFIGS", "SWEEP_N", "make_input", "make_blocks", "uniform_small",
-           "gaussian", "gaussian_tone", "common_tone", "full_range"]
+           "gaussian", "gaussian_tone", "common_tone", "full_range", "packed_i4"]
 
 
 @dataclass(frozen=True)
@@ -145,3 +145,17 @@ def make_input(w: Workload, T: int | None = None, seed: int | None = None) -> np
 def make_blocks(w: Workload, n_blocks: int, seed0: int = 1060) -> list[np.ndarray]:
     """Config 5's two-stream run: n_blocks input blocks of w's shape, seeds seed0 + k."""
     return [make_input(w, seed=seed0 + k) for k in range(n_blocks)]
+
+
+def packed_i4(N: int, F: int, T: int, seed: int) -> np.ndarray:
+    """4-bit complex samples, one byte per (t, f, station, pol): uniform random bytes, i.e. both nibbles uniform over
+    all 16 codes, with the codes 0x8 (-8) and 0x7 (+7) forced into every nibble position class of the first row.
+    uint8 [T][F][N][2].  No arithmetic of the method here: the two sides each decode the nibbles themselves."""
+    rng = np.random.default_rng(seed)
+    x = rng.integers(0, 256, size=(T, F, N, 2), dtype=np.uint8)
+    x[0, 0, 0, 0] = 0x88
+    x[0, 0, 0, 1] = 0x77
+    if T > 1:
+        x[1, 0, 0, 0] = 0x78
+        x[1, 0, 0, 1] = 0x87
+    return x
