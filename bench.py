@@ -391,6 +391,36 @@ def main():
         p3.close()
         del x3, v3
         torch.cuda.empty_cache()
+        # 4-bit samples on config 2's shape: device-resident (unpack + X-engine) and
+        # end to end with host buffers (half the H2D bytes of the int8 call)
+        w2 = wl.CONFIGS["cfg2"]
+        x4h = torch.from_numpy(wl.packed_i4(w2.N, w2.F, w2.T, seed=2002)).pin_memory()
+        x4d = x4h.cuda()
+        p4 = xcb.Plan(w2.N, w2.F, w2.T)
+        v4 = p4.new_vis()
+        v4h = torch.empty(p4.vis_shape(), dtype=torch.int32).pin_memory()
+        for _ in range(3):
+            p4.correlate_i4(x4d, v4, stream=stream)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        stream.synchronize()
+        ev[0].record(stream)
+        for _ in range(20):
+            p4.correlate_i4(x4d, v4, stream=stream)
+        ev[1].record(stream)
+        stream.synchronize()
+        ms4 = ev[0].elapsed_time(ev[1]) / 20
+        p4.correlate_host_i4(x4h, v4h, x4d, v4, stream=stream)
+        t0 = time.perf_counter()
+        for _ in range(5):
+            p4.correlate_host_i4(x4h, v4h, x4d, v4, stream=stream)
+        e4 = (time.perf_counter() - t0) / 5
+        extras["i4"] = {"workload": "config 2's shape with 4-bit complex samples (uniform nibbles), xc_correlate_i4 / xc_correlate_host_i4",
+                        "device_ms": ms4, "tops": w2.ops / (ms4 * 1e-3) / 1e12, "launches_per_step": 2,
+                        "e2e_ms": 1e3 * e4, "e2e_tops": w2.ops / e4 / 1e12, "h2d_bytes_per_step": w2.in_bytes // 2,
+                        "d2h_bytes_per_step": w2.vis_bytes}
+        p4.close()
+        del x4h, x4d, v4, v4h
+        torch.cuda.empty_cache()
         # two-stream run of config 5: 8 host blocks (the same seeded block 8 times: only the timing matters here;
         # parity of the 8-distinct-block run is tests/test_xc_gpu.py::test_cfg5_two_stream_eight_blocks)
         w5 = wl.CONFIGS["cfg5_N1024"]

@@ -121,6 +121,7 @@ void xc_destroy(xc_plan_t* plan);
 /* Sizes in bytes of one input block / one output cube for this plan. */
 size_t xc_in_bytes(const xc_plan_t* plan);      /* int8 path:  4*N*F*T            */
 size_t xc_in_bytes_f32(const xc_plan_t* plan);  /* fp32 path: 16*N*F*T            */
+size_t xc_in_bytes_i4(const xc_plan_t* plan);   /* 4-bit path: 2*N*F*T            */
 size_t xc_vis_bytes(const xc_plan_t* plan);     /* 32*NB*F (int32 and float alike) */
 /* N(N+1)/2. */
 size_t xc_n_baselines(const xc_plan_t* plan);
@@ -128,7 +129,7 @@ size_t xc_n_baselines(const xc_plan_t* plan);
 /* Staging.  The tensor-core kernel reads the input through TMA, which
  * needs a 16-byte-aligned base and a 16-byte-multiple row pitch (4N bytes -> N % 4 == 0).
  * Otherwise the input is first copied by a padding kernel into a workspace of
- * xc_workspace_bytes() bytes.  The caller may hand one in (device
+ * xc_workspace_bytes() bytes (4 * roundup(N, 4) * F * T; the 4-bit path always uses it).  The caller may hand one in (device
  * memory, 128-byte aligned, kept until xc_destroy or replaced); if none was set the
  * library cudaMallocs one on first need (a synchronising call) and frees it in xc_destroy. */
 size_t xc_workspace_bytes(const xc_plan_t* plan);
@@ -144,6 +145,15 @@ int xc_set_option(xc_plan_t* plan, int option, int value);
  *   PAPER.md:244; I = N_p * I').  int32 two's-complement addition. */
 int xc_correlate(xc_plan_t* plan, const int8_t* in_dev, int32_t* vis_dev, void* cuda_stream);
 int xc_correlate_acc(xc_plan_t* plan, const int8_t* in_dev, int32_t* vis_dev, void* cuda_stream);
+
+/* xc_correlate_i4 -- the same operation on 4-bit complex samples ("typically four to eight bits of precision is
+ *   sufficient"; two's complement): halves the input bytes that cross PCIe / leave HBM.
+ *   in4_dev: uint8 [T][F][N][2 pol], ONE byte per complex sample: low nibble = real part, high nibble = imaginary
+ *   part, each a two's-complement integer in [-8, 7] (the paper fixes no packing; this is the library's format).
+ *   A staging pass unpacks into the int8 workspace (xc_workspace_bytes(); see xc_set_workspace), then the tensor-core
+ *   path runs as for int8 input; exact.  accumulate != 0 adds to vis_dev.  Errors as xc_correlate; UNSUPPORTED with
+ *   the SIMT kernel selected. */
+int xc_correlate_i4(xc_plan_t* plan, const uint8_t* in4_dev, int32_t* vis_dev, int accumulate, void* cuda_stream);
 
 /* xc_correlate_f32 -- same operation on float samples with fp32 FMA arithmetic on the CUDA
  *   cores (the paper's own arithmetic: PAPER.md:75, 16 FMAs per station pair per sample;
@@ -194,6 +204,11 @@ int xc_correlate_channels(xc_plan_t* plan, const int8_t* in_dev, int32_t* vis_de
  *   of its own).  in_dev_scratch / vis_dev_scratch are caller-owned device buffers of the plan's sizes. */
 int xc_correlate_host(xc_plan_t* plan, const int8_t* in_host, int32_t* vis_host, int8_t* in_dev_scratch,
                       int32_t* vis_dev_scratch, void* cuda_stream);
+
+/* xc_correlate_host_i4 -- xc_correlate_host for 4-bit samples (format of xc_correlate_i4): in4_host / in4_dev_scratch hold
+ *   xc_in_bytes_i4() bytes; half the host->device bytes of the int8 call, same result cube. */
+int xc_correlate_host_i4(xc_plan_t* plan, const uint8_t* in4_host, int32_t* vis_host, uint8_t* in4_dev_scratch,
+                         int32_t* vis_dev_scratch, void* cuda_stream);
 
 /* PROFILING ONLY: trace_dev = device buffer of 3*256*4 + 4 int64 (or NULL to switch off); CTA 0 of the
  * tensor-core kernel writes clock64() stamps of its first 256 pipeline iterations per warp role

@@ -22,7 +22,7 @@ TILE_AUTO, TILE_1CTA_128x128, TILE_1CTA_128x256, TILE_2CTA_256x256, TILE_SPLIT, 
 EXPORTED_SYMBOLS = (
     "xc_plan", "xc_destroy", "xc_in_bytes", "xc_in_bytes_f32", "xc_vis_bytes", "xc_n_baselines",
     "xc_workspace_bytes", "xc_set_workspace", "xc_set_option", "xc_correlate", "xc_correlate_acc",
-    "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_integrate", "xc_tile_count", "xc_tile_get",
+    "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_integrate", "xc_correlate_i4", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get",
     "xc_debug_set_trace", "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error",
     "xc_version",
 )
@@ -58,10 +58,13 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_set_option": (i, [p, i, i]),
         "xc_correlate": (i, [p, p, p, p]), "xc_correlate_acc": (i, [p, p, p, p]),
         "xc_correlate_f32": (i, [p, p, p, i, p]),
+        "xc_correlate_i4": (i, [p, p, p, i, p]),
+        "xc_in_bytes_i4": (sz, [p]),
         "xc_correlate_channels": (i, [p, p, p, i, i, i, p]),
         "xc_integrate": (i, [p, p, i, p, p, p, p, p, p]),
         "xc_correlate_pipelined": (i, [p, p, i, p, p, p, p]),
         "xc_correlate_host": (i, [p, p, p, p, p, p]),
+        "xc_correlate_host_i4": (i, [p, p, p, p, p, p]),
         "xc_debug_set_trace": (i, [p, p]),
         "xc_tile_count": (i, [p]),
         "xc_tile_get": (i, [p, i, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i)]),
@@ -239,6 +242,19 @@ class Plan:
                     "xc_correlate_channels")
         return vis
 
+    def correlate_i4(self, x4, vis=None, accumulate=False, stream=None):
+        """vis (+)= X-engine(x4) for 4-bit samples.  x4: uint8 CUDA [T][F][N][2] (low nibble re, high nibble im)."""
+        import torch
+        if not (isinstance(x4, torch.Tensor) and x4.is_cuda and x4.dtype == torch.uint8 and x4.is_contiguous()
+                and tuple(x4.shape) == (self.T, self.F, self.N, 2)):
+            raise ValueError(f"input must be a contiguous CUDA uint8 tensor of shape {(self.T, self.F, self.N, 2)}")
+        if vis is None:
+            vis = self.new_vis(torch.int32, x4.device)
+        self._chk_vis(vis, torch.int32)
+        self._check(lib().xc_correlate_i4(self._h, ctypes.c_void_p(x4.data_ptr()), ctypes.c_void_p(vis.data_ptr()),
+                                          1 if accumulate else 0, _stream_handle(stream)), "xc_correlate_i4")
+        return vis
+
     def correlate_f32(self, x, vis=None, accumulate=False, stream=None):
         import torch
         self._chk_in(x, torch.float32)
@@ -286,6 +302,14 @@ class Plan:
             ctypes.c_void_p(vis64_host.data_ptr() if vis64_host is not None else 0),
             ctypes.c_void_p(compute_stream.cuda_stream), ctypes.c_void_p(copy_stream.cuda_stream)), "xc_integrate")
         return vis64
+
+    def correlate_host_i4(self, x4_host, vis_host, in4_dev, vis_dev, stream=None):
+        """End to end with HOST buffers for 4-bit samples (uint8 [T][F][N][2])."""
+        self._check(lib().xc_correlate_host_i4(
+            self._h, ctypes.c_void_p(x4_host.data_ptr()), ctypes.c_void_p(vis_host.data_ptr()),
+            ctypes.c_void_p(in4_dev.data_ptr()), ctypes.c_void_p(vis_dev.data_ptr()), _stream_handle(stream)),
+            "xc_correlate_host_i4")
+        return vis_host
 
     def correlate_host(self, x_host, vis_host, in_dev, vis_dev, stream=None):
         """End to end with HOST buffers (H2D copy, X-engine, D2H copy, stream sync)."""

@@ -254,8 +254,10 @@ int ensure_device(xc_plan_t* p) {
 }
 
 // S0: decide whether the padding kernel is needed and run it; *src / *nrow describe what TMA reads.
-int stage_if_needed(xc_plan_t* p, const int8_t* in_dev, cudaStream_t st, const void** src, int* nrow) {
-    const bool need = p->opt_force_stage || (p->Npad != p->N) || (reinterpret_cast<uintptr_t>(in_dev) & 15u);
+int stage_if_needed(xc_plan_t* p, const int8_t* in_dev, cudaStream_t st, const void** src, int* nrow, int fmt_i4 = 0,
+                    int f0 = 0, int nf = -1) {
+    if (nf < 0) nf = p->F;
+    const bool need = fmt_i4 || p->opt_force_stage || (p->Npad != p->N) || (reinterpret_cast<uintptr_t>(in_dev) & 15u);
     if (!need) {
         *src = in_dev;
         *nrow = p->N;
@@ -272,7 +274,21 @@ int stage_if_needed(xc_plan_t* p, const int8_t* in_dev, cudaStream_t st, const v
     const long long total = rows * p->Npad;
     long long blocks = (total + 255) / 256;
     if (blocks > 148LL * 32) blocks = 148LL * 32;
-    if (p->N % 4 == 0 && !(reinterpret_cast<uintptr_t>(in_dev) & 15u)) {
+    if (fmt_i4) {
+        // 4-bit samples: the staging pass is the unpacking pass (in_dev then points at 2*N*F*T packed bytes)
+        const long long units = static_cast<long long>(p->T) * nf * p->Npad;
+        if (p->N % 8 == 0 && !(reinterpret_cast<uintptr_t>(in_dev) & 15u)) {
+            long long b16 = (units / 8 + 255) / 256;
+            if (b16 > 148LL * 32) b16 = 148LL * 32;
+            xc::xc_unpack_i4x8_kernel<<<static_cast<unsigned>(b16 < 1 ? 1 : b16), 256, 0, st>>>(
+                reinterpret_cast<const uint4*>(in_dev), static_cast<uint4*>(p->ws), p->T, p->F, f0, nf, p->N / 8);
+        } else {
+            long long b1 = (units + 255) / 256;
+            if (b1 > 148LL * 32) b1 = 148LL * 32;
+            xc::xc_unpack_i4_kernel<<<static_cast<unsigned>(b1), 256, 0, st>>>(
+                reinterpret_cast<const uint8_t*>(in_dev), static_cast<uint32_t*>(p->ws), p->T, p->F, f0, nf, p->N, p->Npad);
+        }
+    } else if (p->N % 4 == 0 && !(reinterpret_cast<uintptr_t>(in_dev) & 15u)) {
         xc::xc_stage_pad16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(
             reinterpret_cast<const uint4*>(in_dev), static_cast<uint4*>(p->ws), rows, p->N / 4, p->Npad / 4);
     } else {
@@ -314,7 +330,7 @@ int encode_tmap(xc_plan_t* p, const void* src, int nrow, int bk, int nf) {
 
 // X-engine on channels [f0, f0 + nf) of the block at in_dev / the cube at vis_dev (both addressed with the plan's F).
 int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* stream, int accumulate, int f0 = 0,
-                 int nf = -1) {
+                 int nf = -1, int fmt_i4 = 0) {
     if (!p || !in_dev || !vis_dev) return XC_ERR_INVALID_ARG;
     if (nf < 0) nf = p->F;
     if (f0 < 0 || nf < 1 || f0 + nf > p->F) return XC_ERR_INVALID_ARG;
@@ -326,8 +342,9 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     p->last_launches = 0;
 
     // a channel sub-range is read in place through its own tensor map: not with the SIMT kernel, not through staging
-    const bool need_stage = p->opt_force_stage || (p->Npad != p->N) || (reinterpret_cast<uintptr_t>(in_dev) & 15u);
-    if (sub && (p->opt_kernel == XC_I8_KERNEL_SIMT || need_stage)) return XC_ERR_UNSUPPORTED;
+    const bool need_stage = fmt_i4 || p->opt_force_stage || (p->Npad != p->N) || (reinterpret_cast<uintptr_t>(in_dev) & 15u);
+    if (sub && (p->opt_kernel == XC_I8_KERNEL_SIMT || (need_stage && !fmt_i4))) return XC_ERR_UNSUPPORTED;
+    if (fmt_i4 && p->opt_kernel == XC_I8_KERNEL_SIMT) return XC_ERR_UNSUPPORTED;
     if (p->opt_kernel == XC_I8_KERNEL_SIMT) {
         if (p->F > 65535) return XC_ERR_UNSUPPORTED;
         xc::SimtParams sp{p->N, p->F, p->T, p->NB, in_dev, vis_dev, accumulate};
@@ -341,7 +358,7 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
 
     const void* src = nullptr;
     int nrow = 0;
-    rc = stage_if_needed(p, in_dev, st, &src, &nrow);
+    rc = stage_if_needed(p, in_dev, st, &src, &nrow, fmt_i4, f0, nf);
     if (rc != XC_OK) return rc;
     const bool bkopt = p->tile_mode == XC_TILE_2CTA_256x256 && p->opt_epilogue != XC_EPI_STAGED;
     const bool bk256 = bkopt && p->opt_bk == 256, bk64 = bkopt && p->opt_bk == 64;
@@ -474,6 +491,7 @@ void xc_destroy(xc_plan_t* p) {
 }
 
 size_t xc_in_bytes(const xc_plan_t* p) { return p ? static_cast<size_t>(4) * p->N * p->F * p->T : 0; }
+size_t xc_in_bytes_i4(const xc_plan_t* p) { return p ? static_cast<size_t>(2) * p->N * p->F * p->T : 0; }
 size_t xc_in_bytes_f32(const xc_plan_t* p) { return p ? static_cast<size_t>(16) * p->N * p->F * p->T : 0; }
 size_t xc_vis_bytes(const xc_plan_t* p) { return p ? static_cast<size_t>(32) * p->NB * p->F : 0; }
 size_t xc_n_baselines(const xc_plan_t* p) { return p ? static_cast<size_t>(p->NB) : 0; }
@@ -533,6 +551,10 @@ int xc_correlate(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
 }
 int xc_correlate_acc(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* stream) {
     return correlate_i8(p, in_dev, vis_dev, stream, 1);
+}
+
+int xc_correlate_i4(xc_plan_t* p, const uint8_t* in4_dev, int32_t* vis_dev, int accumulate, void* stream) {
+    return correlate_i8(p, reinterpret_cast<const int8_t*>(in4_dev), vis_dev, stream, accumulate ? 1 : 0, 0, -1, 1);
 }
 
 int xc_correlate_f32(xc_plan_t* p, const float* in_dev, float* vis_dev, int accumulate, void* stream) {
@@ -652,18 +674,20 @@ int xc_correlate_channels(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, 
     return correlate_i8(p, in_dev, vis_dev, stream, accumulate ? 1 : 0, f0, nf);
 }
 
-int xc_correlate_host(xc_plan_t* p, const int8_t* in_host, int32_t* vis_host, int8_t* in_dev_scratch,
-                      int32_t* vis_dev_scratch, void* stream) {
+static int correlate_host_impl(xc_plan_t* p, const int8_t* in_host, int32_t* vis_host, int8_t* in_dev_scratch,
+                               int32_t* vis_dev_scratch, void* stream, int fmt_i4) {
     if (!p || !in_host || !vis_host || !in_dev_scratch || !vis_dev_scratch) return XC_ERR_INVALID_ARG;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int rc = ensure_device(p);
     if (rc != XC_OK) return rc;
-    const bool need_stage = p->opt_force_stage || (p->Npad != p->N) || (reinterpret_cast<uintptr_t>(in_dev_scratch) & 15u);
+    // int8 blocks that need the staging pass work on whole blocks only; 4-bit blocks are unpacked range by range
+    const bool need_stage = !fmt_i4 && (p->opt_force_stage || (p->Npad != p->N) || (reinterpret_cast<uintptr_t>(in_dev_scratch) & 15u));
+    const size_t in_bytes = fmt_i4 ? xc_in_bytes_i4(p) : xc_in_bytes(p);
     int chunks = p->F < 16 ? p->F : 16;
-    if (need_stage || p->opt_kernel == XC_I8_KERNEL_SIMT || xc_in_bytes(p) < (static_cast<size_t>(8) << 20)) chunks = 1;
+    if (need_stage || p->opt_kernel == XC_I8_KERNEL_SIMT || in_bytes < (static_cast<size_t>(8) << 20)) chunks = 1;
     if (chunks == 1) {
-        XC_CUDA(p, cudaMemcpyAsync(in_dev_scratch, in_host, xc_in_bytes(p), cudaMemcpyHostToDevice, st));
-        rc = correlate_i8(p, in_dev_scratch, vis_dev_scratch, stream, 0);
+        XC_CUDA(p, cudaMemcpyAsync(in_dev_scratch, in_host, in_bytes, cudaMemcpyHostToDevice, st));
+        rc = correlate_i8(p, in_dev_scratch, vis_dev_scratch, stream, 0, 0, -1, fmt_i4);
         if (rc != XC_OK) return rc;
         XC_CUDA(p, cudaMemcpyAsync(vis_host, vis_dev_scratch, xc_vis_bytes(p), cudaMemcpyDeviceToHost, st));
         XC_CUDA(p, cudaStreamSynchronize(st));
@@ -684,7 +708,7 @@ int xc_correlate_host(xc_plan_t* p, const int8_t* in_host, int32_t* vis_host, in
     XC_CUDA(p, cudaEventRecord(ev_entry, st));           // earlier work on the caller's stream may still use the scratch
     XC_CUDA(p, cudaStreamWaitEvent(p->s_h2d, ev_entry, 0));
     XC_CUDA(p, cudaStreamWaitEvent(p->s_d2h, ev_entry, 0));
-    const size_t row = static_cast<size_t>(4) * p->N;    // bytes of one (t, f) row
+    const size_t row = static_cast<size_t>(fmt_i4 ? 2 : 4) * p->N;    // bytes of one (t, f) row
     const size_t pitch = row * p->F;
     int launches = 0;
     for (int c = 0; c < chunks; ++c) {
@@ -694,7 +718,7 @@ int xc_correlate_host(xc_plan_t* p, const int8_t* in_host, int32_t* vis_host, in
                                      static_cast<size_t>(p->T), cudaMemcpyHostToDevice, p->s_h2d));
         XC_CUDA(p, cudaEventRecord(p->ev_chunk[2 * c], p->s_h2d));
         XC_CUDA(p, cudaStreamWaitEvent(st, p->ev_chunk[2 * c], 0));
-        rc = correlate_i8(p, in_dev_scratch, vis_dev_scratch, stream, 0, f0, f1 - f0);
+        rc = correlate_i8(p, in_dev_scratch, vis_dev_scratch, stream, 0, f0, f1 - f0, fmt_i4);
         if (rc != XC_OK) return rc;
         launches += p->last_launches;
         XC_CUDA(p, cudaEventRecord(p->ev_chunk[2 * c + 1], st));
@@ -708,6 +732,17 @@ int xc_correlate_host(xc_plan_t* p, const int8_t* in_host, int32_t* vis_host, in
     XC_CUDA(p, cudaStreamSynchronize(st));
     p->last_launches = launches;
     return XC_OK;
+}
+
+int xc_correlate_host(xc_plan_t* p, const int8_t* in_host, int32_t* vis_host, int8_t* in_dev_scratch,
+                      int32_t* vis_dev_scratch, void* stream) {
+    return correlate_host_impl(p, in_host, vis_host, in_dev_scratch, vis_dev_scratch, stream, 0);
+}
+
+int xc_correlate_host_i4(xc_plan_t* p, const uint8_t* in4_host, int32_t* vis_host, uint8_t* in4_dev_scratch,
+                         int32_t* vis_dev_scratch, void* stream) {
+    return correlate_host_impl(p, reinterpret_cast<const int8_t*>(in4_host), vis_host, reinterpret_cast<int8_t*>(in4_dev_scratch),
+                               vis_dev_scratch, stream, 1);
 }
 
 int xc_debug_set_trace(xc_plan_t* p, void* trace_dev) {

@@ -94,6 +94,57 @@ __global__ void xc_stage_pad16_kernel(const uint4* __restrict__ in, uint4* __res
     }
 }
 
+// (d) 4-bit complex samples (reading 17): one byte per (t, f, station, pol), low nibble = real,
+// high nibble = imaginary, two's complement.  Unpacked into the int8 workspace the tensor-core kernel reads (station pitch
+// Npad).  Four packed bytes (two stations) -> eight int8: per byte lane (n ^ 8) - 8 sign-extends the nibble.
+__device__ __forceinline__ void unpack_i4_word(uint32_t w, uint32_t* o0, uint32_t* o1) {
+    const uint32_t lo = __vsub4((w & 0x0F0F0F0Fu) ^ 0x08080808u, 0x08080808u);          // real parts, one per byte lane
+    const uint32_t hi = __vsub4(((w >> 4) & 0x0F0F0F0Fu) ^ 0x08080808u, 0x08080808u);   // imaginary parts
+    *o0 = __byte_perm(lo, hi, 0x5140);   // (re0, im0, re1, im1): station s,   pol 0 and 1
+    *o1 = __byte_perm(lo, hi, 0x7362);   // (re2, im2, re3, im3): station s+1, pol 0 and 1
+}
+// Both kernels work on the channel range [f0, f0 + nf) of every time sample (row r = t * F + f), so that ranges of one
+// block can be unpacked and correlated one after the other (xc_correlate_host_i4).
+// general: one thread per destination station (2 packed bytes -> 4 int8), zero padding for s >= N
+__global__ void xc_unpack_i4_kernel(const uint8_t* __restrict__ in4, uint32_t* __restrict__ out, int T, int F, int f0, int nf,
+                                    int N, int Npad) {
+    const long long per_t = static_cast<long long>(nf) * Npad;
+    const long long total = per_t * T;
+    for (long long k = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; k < total;
+         k += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long t = k / per_t;
+        const long long rem = k - t * per_t;
+        const long long r = t * F + f0 + rem / Npad;
+        const int s = static_cast<int>(rem % Npad);
+        uint32_t o0 = 0, o1 = 0;
+        if (s < N) {
+            const uint8_t* src = in4 + (r * N + s) * 2;
+            unpack_i4_word(static_cast<uint32_t>(src[0]) | (static_cast<uint32_t>(src[1]) << 8), &o0, &o1);
+        }
+        out[r * Npad + s] = o0;
+    }
+}
+// N % 8 == 0 and a 16-byte aligned input: 16 packed bytes (8 stations) -> 32 int8 per thread; n8 = N / 8
+__global__ void xc_unpack_i4x8_kernel(const uint4* __restrict__ in4, uint4* __restrict__ out, int T, int F, int f0, int nf,
+                                      int n8) {
+    const long long per_t = static_cast<long long>(nf) * n8;
+    const long long total = per_t * T;
+    for (long long k = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; k < total;
+         k += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long t = k / per_t;
+        const long long rem = k - t * per_t;
+        const long long idx = (t * F + f0 + rem / n8) * n8 + rem % n8;
+        const uint4 w = __ldcs(in4 + idx);
+        uint4 a, b;
+        unpack_i4_word(w.x, &a.x, &a.y);
+        unpack_i4_word(w.y, &a.z, &a.w);
+        unpack_i4_word(w.z, &b.x, &b.y);
+        unpack_i4_word(w.w, &b.z, &b.w);
+        out[2 * idx] = a;
+        out[2 * idx + 1] = b;
+    }
+}
+
 // (c) Long integrations (I = N_p * I'): vis64 (+)= vis32, four values per thread.  int32 partial
 // sums of at most XC_MAX_T samples are exact; this widening add makes any integration length exact in int64.
 __global__ void xc_widen_kernel(const int4* __restrict__ v32, longlong2* __restrict__ v64, long long n4, int first) {

@@ -262,6 +262,64 @@ def test_random_shapes_auto_mode():
         p.close()
 
 
+@pytest.mark.parametrize("N,F,T", [(1, 1, 1), (3, 2, 17), (8, 3, 40), (16, 2, 129), (37, 2, 100), (64, 3, 257), (100, 2, 130),
+                                   (136, 1, 300)])
+def test_i4_small_shapes(N, F, T):
+    """4-bit samples (DESIGN reading 17) against the oracle's own nibble decoding: bit-exact, every
+    output written, accumulate adds; both unpack kernels (N % 8 == 0 fast path and the general one) are covered."""
+    x4 = wl.packed_i4(N, F, T, seed=50 + N)
+    ref = xo.correlate_i4(x4)
+    p = xcb.Plan(N, F, T)
+    xd = torch.from_numpy(x4).cuda()
+    vis = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+    p.correlate_i4(xd, vis)
+    assert np.array_equal(vis.cpu().numpy(), ref)
+    p.correlate_i4(xd, vis, accumulate=True)
+    assert np.array_equal(vis.cpu().numpy(), 2 * ref)
+    # the same values as int8 through xc_correlate give the same cube
+    v8 = p.correlate(torch.from_numpy(xo.unpack_i4(x4)).cuda())
+    assert np.array_equal(v8.cpu().numpy(), ref)
+
+
+def test_i4_host_call_chunked():
+    """xc_correlate_host_i4 on a block large enough for the channel-range pipeline (unpack and X-engine per range):
+    same cube as the oracle; and xc_correlate_channels stays whole-block-only for int8 input that needs staging."""
+    N, F, T = 64, 70, 1000                                   # 8.96 MB packed
+    x4 = wl.packed_i4(N, F, T, seed=71)
+    p = xcb.Plan(N, F, T)
+    xh = torch.from_numpy(x4).pin_memory()
+    vh = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32).pin_memory()
+    xd = torch.zeros((T, F, N, 2), dtype=torch.uint8, device="cuda")
+    vd = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+    p.correlate_host_i4(xh, vh, xd, vd)
+    assert p.last_launches == 32                              # 16 ranges x (unpack + X-engine)
+    assert np.array_equal(vh.numpy(), xo.correlate_i4(x4))
+    # ragged N (general unpack kernel, padded workspace rows), small block -> unchunked
+    x4 = wl.packed_i4(13, 3, 50, seed=72)
+    p = xcb.Plan(13, 3, 50)
+    xh = torch.from_numpy(x4).pin_memory()
+    vh = torch.zeros(p.vis_shape(), dtype=torch.int32).pin_memory()
+    p.correlate_host_i4(xh, vh, torch.zeros((50, 3, 13, 2), dtype=torch.uint8, device="cuda"), p.new_vis())
+    assert np.array_equal(vh.numpy(), xo.correlate_i4(x4))
+
+
+def test_i4_config2_shape_sampled():
+    """Config 2's shape with 4-bit samples: sampled channels against the oracle, every output against xc_correlate on the
+    unpacked values (itself parity-tested at this size)."""
+    w = wl.CONFIGS["cfg2"]
+    x4 = wl.packed_i4(w.N, w.F, w.T, seed=2002)
+    p = xcb.Plan(w.N, w.F, w.T)
+    xd = torch.from_numpy(x4).cuda()
+    vis = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+    p.correlate_i4(xd, vis)
+    assert p.last_launches == 2
+    fsel = [0, 511, 1023]
+    ref = xo.correlate_i4(np.ascontiguousarray(x4[:, fsel]))
+    assert np.array_equal(vis[torch.tensor(fsel, device="cuda")].cpu().numpy(), ref)
+    x8 = torch.from_numpy(xo.unpack_i4(x4)).cuda()
+    assert torch.equal(p.correlate(x8), vis)
+
+
 def test_integrate_long_integration_int64():
     """xc_integrate: Algorithm 1 with int64 widening.  (a) all -128 over 3 x 30000 samples leaves
     int32 (2 * 128^2 * 90000 > 2^31) and must hit the closed form; (b) random full-range blocks against the oracle's
