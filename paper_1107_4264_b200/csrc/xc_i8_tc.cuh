@@ -238,7 +238,10 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
             // Such a tile keeps 32 KB / 512 tensor cycles per stage by putting TWO time slices of box 1 into the stage's
             // two box slots (256 samples per stage): a 128-sample stage of N = 128 MMAs would hold only 256 tensor cycles,
             // less than the barrier round trip of a stage.
-            const int h0 = (DIAG && m_a >= m_b + 128) ? 1 : 0;
+            // The same holds for the diagonal tile of the single-CTA 128x128 variant (A rows = B rows = one box).
+            constexpr bool SOLO128 = (CG == 1 && UMMA_N == 128 && !STAGED);
+            const int h0 = ((DIAG && m_a >= m_b + 128) || (SOLO128 && a_in_b)) ? 1 : 0;
+            const int m_ts = DIAG ? m_b + 128 : m_b;       // rows of the one box a two-slice tile loads
             const uint32_t my_bytes = a_in_b ? static_cast<uint32_t>(Cfg::B_BYTES) : Cfg::STAGE_BYTES;
             const int KBt = h0 ? (p.T + 2 * Cfg::BK - 1) / (2 * Cfg::BK) : KB;
             for (int kb = 0; kb < KBt; ++kb) {
@@ -252,11 +255,11 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
                     const int t0 = kb * Cfg::BK * (1 + h0);
                     if ((p.debug_skip & 1) && (n != 0 || kb >= Cfg::STAGES)) {
                         if (rank == 0) mbar_arrive(full_bar(stage));
-                    } else if (DIAG && h0) {
+                    } else if ((DIAG || SOLO128) && h0) {
                         const bool two = t0 + Cfg::BK < p.T;     // the second time slice exists
                         mbar_arrive_expect_tx(full_bar(stage), two ? 2 * Cfg::BOX_BYTES : Cfg::BOX_BYTES);
-                        tma_load_3d(sb, &tmap, full_bar(stage), m_b + 128, f, t0);
-                        if (two) tma_load_3d(sb + Cfg::BOX_BYTES, &tmap, full_bar(stage), m_b + 128, f, t0 + Cfg::BK);
+                        tma_load_3d(sa, &tmap, full_bar(stage), m_ts, f, t0);
+                        if (two) tma_load_3d(sa + Cfg::BOX_BYTES, &tmap, full_bar(stage), m_ts, f, t0 + Cfg::BK);
                     } else if (CG == 1) {
                         mbar_arrive_expect_tx(full_bar(stage), my_bytes);
                         if (!a_in_b) tma_load_3d(sa, &tmap, full_bar(stage), m_a, f, t0);
@@ -302,14 +305,15 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
                 // byte offset of the A operand inside a stage: its own box, or the B box holding the same rows
                 // DIAG, row block in the second column box: N = 128 MMAs on box 1 (A = B = that box; the stage's two slots
                 // hold two consecutive time slices of it) into the accumulator's upper 128 columns
-                const uint32_t h0 = (DIAG && m_a >= m_b + 128) ? 1u : 0u;
+                constexpr bool SOLO128 = (CG == 1 && UMMA_N == 128 && !STAGED);
+                const uint32_t h0 = ((DIAG && m_a >= m_b + 128) || (SOLO128 && a_in_b)) ? 1u : 0u;
                 const uint32_t a_off = h0 ? 0u : (a_in_b ? static_cast<uint32_t>(Cfg::A_BYTES + ((m_a - m_b) >> 7) * Cfg::BOX_BYTES) : 0u);
                 const uint32_t idesc_t = h0 ? make_idesc_i8_mn(Cfg::M, 128) : idesc;
                 const int BKt = Cfg::BK * (1 + static_cast<int>(h0));           // samples per stage of this tile
                 const int KBt = (p.T + BKt - 1) / BKt;
                 mbar_wait(tempty_bar(buf), ((tphase >> buf) & 1u) ^ 1u);  // epilogues have drained this accumulator
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + buf * UMMA_N + h0 * 128u;
+                const uint32_t d_tmem = tmem_base + buf * UMMA_N + (DIAG ? h0 * 128u : 0u);
                 for (int kb = 0; kb < KBt; ++kb) {
                     const bool tr = TRACE && p.trace && blockIdx.x == 0 && it < TC_TRACE_ITERS && elected;
                     if (tr) p.trace[(1 * TC_TRACE_ITERS + it) * 4 + 0] = clock64();
@@ -319,11 +323,11 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
                     if (elected) {
                         const uint32_t sa = ring0 + stage * Cfg::STAGE_BYTES;
                         const uint64_t adesc = make_smem_desc_mn_sw128(sa + a_off, Cfg::BOX_BYTES, 1024);
-                        const uint64_t bdesc = make_smem_desc_mn_sw128(sa + Cfg::A_BYTES, Cfg::BOX_BYTES, 1024);
+                        const uint64_t bdesc = make_smem_desc_mn_sw128(sa + (h0 ? 0u : static_cast<uint32_t>(Cfg::A_BYTES)), Cfg::BOX_BYTES, 1024);
                         const int rows = min(BKt, p.T - kb * BKt);                // valid samples in this stage
                         const int nk = (rows + TC_UMMA_K - 1) / TC_UMMA_K;       // rows beyond T are TMA zero fill
 #pragma unroll
-                        for (int ks = 0; ks < (DIAG ? 2 : 1) * Cfg::BK / TC_UMMA_K; ++ks) {
+                        for (int ks = 0; ks < ((DIAG || SOLO128) ? 2 : 1) * Cfg::BK / TC_UMMA_K; ++ks) {
                             if (ks < nk && !(p.debug_skip & 2)) {
                                 // K advance: 32 samples = 4 swizzle atoms = 4096 B -> +256 in the address field
                                 umma_i8<CG>(d_tmem, adesc + static_cast<uint64_t>(ks * 256),
