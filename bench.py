@@ -387,7 +387,9 @@ def main():
         extras["f32"] = {"workload": "cfg3 values as float32 through xc_correlate_f32", "kernel_ms": ms,
                          "tflops": w3.ops / (ms * 1e-3) / 1e12, "bound": "alu", "peak_tflops": fp32_peak,
                          "frac": w3.ops / (ms * 1e-3) / 1e12 / fp32_peak,
-                         "peak_source": "SMs x 128 FMA/clk x 2 x clocks.max.sm (derived, DESIGN.md 5.2)"}
+                         "peak_source": "SMs x 128 FMA/clk x 2 x clocks.max.sm (derived, DESIGN.md 5.2)",
+                         "context": "pure-register FFMA2 streams on this pool: 65.2 TFLOPS (constant operands), 57.7 TFLOPS "
+                                    "(this kernel's operand pattern); round-1 probe, DESIGN.md 5.2"}
         p3.close()
         del x3, v3
         torch.cuda.empty_cache()
