@@ -144,6 +144,33 @@ def test_forced_staging_and_unaligned_pointer():
     assert np.array_equal(vis.cpu().numpy(), ref)
 
 
+def test_error_paths_on_device():
+    """Status codes promised by include/xc.h: misaligned vis, workspace too small / misaligned, null pointers; and a
+    failed call leaves the plan usable."""
+    import ctypes
+    N, F, T = 10, 2, 40                                       # N % 4 != 0 -> staging needed
+    x = wl.full_range(N, F, T, seed=1)
+    p = xcb.Plan(N, F, T)
+    L, h = xcb.lib(), p._h
+    xd = torch.from_numpy(x).cuda()
+    vbuf = torch.zeros(p.vis_bytes // 4 + 16, dtype=torch.int32, device="cuda")
+    st = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    assert L.xc_correlate(h, ctypes.c_void_p(xd.data_ptr()), ctypes.c_void_p(vbuf.data_ptr() + 4), st) == -4   # XC_ERR_ALIGNMENT
+    assert L.xc_correlate(h, None, ctypes.c_void_p(vbuf.data_ptr()), st) == -1
+    assert L.xc_correlate(h, ctypes.c_void_p(xd.data_ptr()), None, st) == -1
+    small = torch.zeros(256, dtype=torch.int8, device="cuda")
+    assert L.xc_set_workspace(h, ctypes.c_void_p(small.data_ptr()), 256) == -6            # XC_ERR_NO_WORKSPACE
+    big = torch.zeros(p.workspace_bytes + 256, dtype=torch.int8, device="cuda")
+    assert L.xc_set_workspace(h, ctypes.c_void_p(big.data_ptr() + 8), p.workspace_bytes) == -4
+    assert L.xc_set_workspace(h, ctypes.c_void_p(big.data_ptr()), p.workspace_bytes) == 0
+    vis = p.correlate(xd)
+    assert np.array_equal(vis.cpu().numpy(), xo.correlate_i8(x))
+    assert L.xc_set_workspace(h, None, 0) == 0                                             # back to a library-owned one
+    assert np.array_equal(p.correlate(xd).cpu().numpy(), xo.correlate_i8(x))
+    assert L.xc_integrate(h, None, 1, None, None, None, None, st, st) == -1
+    assert L.xc_correlate_pipelined(h, ctypes.c_void_p(1 << 20), 0, ctypes.c_void_p(1 << 20), ctypes.c_void_p(vbuf.data_ptr()), st, st) == -1
+
+
 def test_persistent_schedule_independent_of_cta_count():
     N, F, T = 100, 5, 200
     x = wl.gaussian(N, F, T, seed=11, sigma=30.0)
