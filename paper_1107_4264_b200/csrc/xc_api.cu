@@ -362,7 +362,8 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     if (rc != XC_OK) return rc;
     const bool bkopt = p->tile_mode == XC_TILE_2CTA_256x256 && p->opt_epilogue != XC_EPI_STAGED;
     const bool bk256 = bkopt && p->opt_bk == 256, bk64 = bkopt && p->opt_bk == 64;
-    const int bk = bk256 ? 256 : (bk64 ? 64 : 128);
+    const bool solo128_bk256 = p->tile_mode == XC_TILE_1CTA_128x128 && p->opt_epilogue != XC_EPI_STAGED && p->opt_bk != 128;
+    const int bk = (bk256 || solo128_bk256) ? 256 : (bk64 ? 64 : 128);
     rc = encode_tmap(p, static_cast<const int8_t*>(src) + static_cast<size_t>(4) * nrow * f0, nrow, bk, nf);
     if (rc != XC_OK) return rc;
 
@@ -439,7 +440,8 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     else if (p->tile_mode == XC_TILE_1CTA_128x256)
         rc = staged ? launch_tc<256, 1, true>(p, tp, st) : launch_tc<256, 1, false>(p, tp, st);
     else
-        rc = staged ? launch_tc<128, 1, true>(p, tp, st) : launch_tc<128, 1, false>(p, tp, st);
+        rc = staged ? launch_tc<128, 1, true>(p, tp, st)
+                    : (solo128_bk256 ? launch_tc<128, 1, false, 256>(p, tp, st) : launch_tc<128, 1, false>(p, tp, st));
     return rc;
 }
 
