@@ -25,7 +25,11 @@
  * retains caller memory beyond the call (except the workspace handed to
  * xc_set_workspace, which it uses until the plan is destroyed or the workspace replaced).
  * Streams are cudaStream_t passed as void*; all device work is enqueued on the stream
- * given, asynchronously, with no hidden device synchronisation unless stated.
+ * given, asynchronously, with no hidden device synchronisation unless stated (the one
+ * exception that uses streams of its own, xc_correlate_host, says so).  The tensor-core
+ * kernels are launched with programmatic stream serialization (XC_OPT_PDL): they wait for
+ * the preceding kernel of the stream before their first global access, so stream order is
+ * kept; calls can be captured into CUDA graphs once the plan has made one compute call.
  *
  * A plan binds to the CUDA device that is current at its first compute call (its tile table, workspace and helper
  * streams live there; later calls with another device current return XC_ERR_INVALID_ARG).  A plan is not thread-safe:
