@@ -333,7 +333,7 @@ def main():
     if rank == 0 and world == 1 and not args.no_sweep:
         del xd, vis, xh, vh
         torch.cuda.empty_cache()
-        for name in ["cfg3", "cfg4", "cfg5_N32", "cfg5_N64", "cfg5_N100", "cfg5_N500", "cfg5_N1024"]:
+        for name in ["cfg1", "cfg3", "cfg4", "cfg5_N32", "cfg5_N64", "cfg5_N100", "cfg5_N500", "cfg5_N1024"]:
             if name == args.workload:
                 continue
             ww = wl.CONFIGS[name]
