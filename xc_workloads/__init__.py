@@ -20,7 +20,7 @@ from dataclasses import dataclass
 import numpy as np
 
 __all__ = ["Workload", "CONFIGS", "SWEEP_N", "make_input", "make_blocks", "uniform_small",
-           "gaussian", "gaussian_tone", "common_tone", "full_range", "packed_i4"]
+           "gaussian", "gaussian_tone", "common_tone", "full_range", "packed_i4", "voltages", "fengine_scale"]
 
 
 @dataclass(frozen=True)
@@ -159,3 +159,36 @@ def packed_i4(N: int, F: int, T: int, seed: int) -> np.ndarray:
         x[1, 0, 0, 0] = 0x78
         x[1, 0, 0, 1] = 0x87
     return x
+
+
+def voltages(N: int, F: int, T: int, seed: int, sigma: float = 16.0, tones: int = 2, amp: float = 12.0,
+             full_range_mix: bool = False) -> np.ndarray:
+    """Time-domain station voltages for the F-engine in front of the X-engine: complex int8, station-major,
+    int8 [N][2 pol][T*F samples][2 re,im] ("the voltage time-series from each antenna ... digitized").
+    Gaussian noise of `sigma` per real component plus `tones` sky tones common to all stations (bin-centred on seeded
+    channels of an F-point transform, station-dependent fixed phase, fresh random phase per time block so that the tone is
+    coherent between stations but not in time), rounded half to even and clipped to [-127, 127].  full_range_mix
+    replaces one signal in eight by uniform samples over the whole int8 range (-128 included).  Only draws samples: the
+    transform itself is the oracle's and the library's business."""
+    rng = np.random.default_rng(seed)
+    out = np.empty((N, 2, T * F, 2), np.int8)
+    f_tone = rng.integers(0, F, size=max(tones, 0))
+    phi = rng.random(size=(max(tones, 0), N)).astype(np.float32) * np.float32(2 * np.pi)
+    k = np.arange(F, dtype=np.float32)
+    for s in range(N):
+        g = rng.standard_normal(size=(2, T, F, 2), dtype=np.float32) * np.float32(sigma)
+        for j in range(len(f_tone)):
+            theta = np.random.default_rng(seed * 1000003 + j).random(size=T).astype(np.float32) * np.float32(2 * np.pi)
+            ph = (np.float32(2 * np.pi) * np.float32(f_tone[j]) * k / np.float32(F))[None, :] + theta[:, None] + phi[j, s]
+            g[:, :, :, 0] += np.float32(amp) * np.cos(ph)[None]
+            g[:, :, :, 1] += np.float32(amp) * np.sin(ph)[None]
+        out[s] = _quantise(g, -127, 127).reshape(2, T * F, 2)
+        if full_range_mix and s % 8 == 3:
+            out[s, s % 2] = rng.integers(-128, 128, size=(T * F, 2), dtype=np.int8)
+    return out
+
+
+def fengine_scale(F: int, sigma: float = 16.0, target: float = 8.0) -> float:
+    """A power-of-two output scale for the F-engine's quantiser such that Gaussian input of `sigma` per component gives
+    channel samples of about `target` per component (the spectrum grows like sigma * sqrt(F))."""
+    return float(2.0 ** np.round(np.log2(target / (sigma * np.sqrt(F)))))
