@@ -1,27 +1,30 @@
 #!/usr/bin/env python
-"""bench.py -- X-engine throughput on B200 (BASELINE.json metric: Tops/s at 8 ops per complex MAC).
+"""bench.py -- X-engine throughput on B200 (BASELINE.json metric: Tops/s at 8 ops per complex MAC, vs N stations).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5_N1024] [--impl reference]
 
-A "step" is one pass of the whole hot path (S0-S3 of SURVEY 8(a): staging if needed, tile schedule,
-tcgen05 X-engine, packing epilogue) over one synthetic input block through the C-ABI library.
-Default workload = BASELINE.json configs[1] (N=128, F=1024, T=1000).  Prints ONE JSON line.
+A "step" is one pass of the whole hot path (S0-S4 of SURVEY 8(a): staging if needed, tile schedule, tcgen05 X-engine,
+packing epilogue) over one synthetic input block through the C-ABI library.  Default workload = the largest single-GPU
+configuration of BASELINE.json (configs[4], N = 1024: the regime north_star's target is defined on).  Prints ONE JSON line.
 
-  value        whole-job Tops/s, inputs resident in HBM (ops = 8 * F * T * N(2N+1), Eq. 5)
+  value        whole-job Tops/s, inputs resident in HBM (ops = 8 * F * T * N(2N+1), Eq. 5), K steps back to back
   e2e          same metric through xc_correlate_host with HOST buffers (H2D + X-engine + D2H per step)
-  roofline     dominant kernel against the measured HBM / int8-tensor peak (MEASURED_PEAKS.json)
+  roofline     the dominant kernel (xc_i8_tc_kernel) of the headline workload: burst (isolated launches, duration from the
+               kernel's own globaltimer stamps) against the burst peak, `sustained` (>= 2 s of back-to-back launches, NVML
+               power / clock trace) against the sustained peak, and `per_config`: the same for every BASELINE config
   cpu_baseline the oracle (oracle/xo_oracle.c, as it stands) on the box's host cores, bounded sample
-  by_config    kernel-only Tops/s for the other BASELINE configs (the metric is "vs N stations")
+  extras       fp32 variant, 4-bit samples, two-stream pipeline, integrated run, pitched N = 500, F-engine + FX chain
 
-N > 1 (torchrun): every rank runs its own block of F channels (channels are independent, PAPER.md:65,
-285): no data-path collective, "scaling": "weak"; time = max over ranks.
+N > 1 (torchrun): every rank runs its own block of F channels (channels are independent): no data-path
+collective, "scaling": "weak"; time = max over ranks.
 """
 from __future__ import annotations
 
 import argparse
+import csv
+import glob
 import json
 import os
-import subprocess
 import sys
 import threading
 import time
@@ -30,7 +33,10 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 NOMINAL_I8_OVER_BF16 = 2.0          # 4.5 / 2.25 PFLOP/s dense (B200_PROFILING.md nominal table)
+NOMINAL_I8_TOPS = 4500.0            # dense int8 = fp8 nominal (B200_PROFILING.md)
 FALLBACK_HBM_GBS, FALLBACK_BF16_TF = 6650.0, 1590.0
+SWEEP = ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5_N32", "cfg5_N64", "cfg5_N100", "cfg5_N500", "cfg5_N1024"]
+SUSTAINED = {"cfg2", "cfg3", "cfg4", "cfg5_N500", "cfg5_N1024"}      # the configs north_star's target speaks about (+ cfg2)
 
 
 def load_peaks():
@@ -44,9 +50,42 @@ def load_peaks():
             "source": "fallback"}
 
 
+def ncu_profile(workload):
+    """Counters of xc_i8_tc_kernel from the tracked ncu export profiles/r2_ncu_<workload>.csv (written by
+    `ncu -i <rep> --page raw --csv --print-units base --metrics ...`; the .md beside it names the commands).  Returns
+    {} when no capture of this round exists: nothing is hard-coded here."""
+    path = os.path.join(ROOT, "profiles", f"r2_ncu_{workload}.csv")
+    if not os.path.exists(path):
+        return {}
+    with open(path, newline="") as fh:
+        rows = list(csv.reader(fh))
+    rows = [r for r in rows if r and r[0].strip('"') not in ("",) or (r and len(r) > 4)]
+    hdr = next((r for r in rows if "Kernel Name" in r), None)
+    if hdr is None:
+        return {}
+    ki = hdr.index("Kernel Name")
+    data = [r for r in rows if len(r) == len(hdr) and "xc_i8_tc_kernel" in r[ki]]
+    if not data:
+        return {}
+
+    def col(name):
+        if name not in hdr:
+            return None
+        vals = [float(r[hdr.index(name)]) for r in data if r[hdr.index(name)] not in ("", "n/a")]
+        return sum(vals) / len(vals) if vals else None
+    rd, wr = col("dram__bytes_read.sum"), col("dram__bytes_write.sum")
+    out = {"file": os.path.relpath(path, ROOT), "launches": len(data),
+           "dram_bytes": (rd + wr) if rd is not None and wr is not None else None,
+           "duration_us": (col("gpu__time_duration.sum") or 0) / 1e3 or None,
+           "tensor_pipe_active_pct": col("sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_elapsed"),
+           "l2_to_sm_read_bytes": col("l1tex__m_xbar2l1tex_read_bytes.sum"),
+           "sm_ghz": (col("sm__cycles_elapsed.avg.per_second") or 0) / 1e9 or None}
+    return out
+
+
 class ClockSampler:
-    """SM clock and throttle reasons sampled through NVML (pynvml) every ~1 ms by a thread, DURING the
-    timed region (the recipe's clocks line, without nvidia-smi's start-up latency)."""
+    """SM clock, power and throttle reasons sampled through NVML (pynvml) every ~1 ms by a thread, DURING the timed
+    regions (the recipe's clocks line, without nvidia-smi's start-up latency)."""
     REASONS = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
 
     def __init__(self, index: int):
@@ -88,11 +127,12 @@ class ClockSampler:
             rows = [r for r in self.rows if t1 < r[0] <= t1 + 0.02][:3]
             where = "first samples after the timed region (region shorter than the sampling period)"
         sm = sorted(r[1] for r in rows)
+        pw = sorted(r[3] for r in rows)
         bits = 0
         for r in rows:
             bits |= r[2]
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": self.max_sm, "samples": len(sm),
-                "power_w_max": max((r[3] for r in rows), default=None),
+                "power_w_median": pw[len(pw) // 2] if pw else None, "power_w_max": pw[-1] if pw else None,
                 "reasons": sorted(n for n, b in self.REASONS.items() if bits & b), "window": where}
 
     def stop(self):
@@ -154,33 +194,129 @@ def run_reference(args, rank):
         "gpu_launches": 0}))
 
 
-def time_kernel(p, xd, vis, stream, steps, warmup):
-    """Per-launch durations (ms) with CUDA events on the launching stream."""
+# ------------------------------------------------------------------------------------------------------------------
+# timing helpers (all on the launching stream)
+# ------------------------------------------------------------------------------------------------------------------
+
+def kernel_durations(p, xd, vis, stream, n):
+    """n isolated launches; per launch (a) the duration from the kernel's own globaltimer stamps (min over CTAs at entry,
+    max at exit: xc_set_timing_buffer), (b) the CUDA-event time around the call (includes the launch gap), (c) the SM clock
+    from CTA 0's cycle counter.  Returns medians: (kernel_ms, event_ms, sm_mhz_in_kernel)."""
     import torch
+    import paper_1107_4264_b200 as xcb
+    init = torch.tensor([2 ** 62, 0, 0, 0, 0, 0], dtype=torch.int64, device="cuda")
+    st = init.repeat(n, 1).contiguous()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
     with torch.cuda.stream(stream):
-        for _ in range(warmup):
-            p.correlate(xd, vis, stream=stream)
-        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        p.correlate(xd, vis, stream=stream)
         stream.synchronize()
-        for a, b in evs:
+        for k, (a, b) in enumerate(evs):
+            p.set_timing_buffer(st[k])
             a.record(stream)
             p.correlate(xd, vis, stream=stream)
             b.record(stream)
+            stream.synchronize()                      # isolated: nothing overlaps the next launch's prologue
+    p.set_timing_buffer(None)
+    rows = st.tolist()
+    dur = sorted((r[1] - r[0]) / 1e6 for r in rows)
+    ev = sorted(a.elapsed_time(b) for a, b in evs)
+    mhz = sorted((r[4] - r[2]) / (r[5] - r[3]) * 1e3 for r in rows if r[5] > r[3])
+    assert xcb.TIMING_WORDS == 6
+    return dur[len(dur) // 2], ev[len(ev) // 2], (mhz[len(mhz) // 2] if mhz else None)
+
+
+def back_to_back(p, xd, vis, stream, n):
+    import torch
+    with torch.cuda.stream(stream):
+        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         stream.synchronize()
-    return [a.elapsed_time(b) for a, b in evs]
+        b0.record(stream)
+        for _ in range(n):
+            p.correlate(xd, vis, stream=stream)
+        b1.record(stream)
+        stream.synchronize()
+    return b0.elapsed_time(b1) / n
+
+
+def sustained_leg(p, xd, vis, stream, sampler, seconds, est_ms):
+    """>= `seconds` of back-to-back launches; throughput, power and clocks over the SECOND half (steady state under the
+    power cap).  Returns dict with ms per launch and the NVML summary."""
+    import torch
+    batch = max(8, min(2000, int(0.1 / (est_ms * 1e-3))))            # ~0.1 s of work per batch
+    marks = []
+    with torch.cuda.stream(stream):
+        stream.synchronize()
+        t_begin = time.perf_counter()
+        e_prev = torch.cuda.Event(enable_timing=True)
+        e_prev.record(stream)
+        queued = 0
+        while True:
+            for _ in range(batch):
+                p.correlate(xd, vis, stream=stream)
+            e = torch.cuda.Event(enable_timing=True)
+            e.record(stream)
+            queued += 1
+            marks.append((e_prev, e, None))
+            e_prev = e
+            if queued >= 2:                                            # keep at most two batches in flight
+                marks[queued - 2][1].synchronize()
+                marks[queued - 2] = (marks[queued - 2][0], marks[queued - 2][1], time.perf_counter())
+            if time.perf_counter() - t_begin >= seconds and queued >= 4:
+                break
+        stream.synchronize()
+        t_end = time.perf_counter()
+    marks[-1] = (marks[-1][0], marks[-1][1], t_end)
+    if marks[-2][2] is None:
+        marks[-2] = (marks[-2][0], marks[-2][1], t_end)
+    half = len(marks) // 2
+    ms = sum(a.elapsed_time(b) for a, b, _ in marks[half:]) / (batch * (len(marks) - half))
+    first_ms = marks[0][0].elapsed_time(marks[0][1]) / batch
+    t_half = marks[half - 1][2] if half >= 1 and marks[half - 1][2] else t_begin
+    nv = sampler.window(t_half, t_end)
+    return {"seconds": t_end - t_begin, "launches": batch * len(marks), "ms_per_launch": ms, "first_batch_ms_per_launch": first_ms,
+            "nvml": {k: nv.get(k) for k in ("sm_mhz", "power_w_median", "power_w_max", "reasons", "samples")}}
+
+
+def roofline_entry(w, k_ms, peaks, i8_burst, prof):
+    """algorithmic bytes = input once + output once; algorithmic ops = Eq. 5.  The bound is the roof that
+    takes longer at its measured peak."""
+    alg_bytes = w.in_bytes + w.vis_bytes
+    t_hbm = alg_bytes / (peaks["hbm_gbs"] * 1e9)
+    t_tc = w.ops / (i8_burst * 1e12)
+    tops = w.ops / (k_ms * 1e-3) / 1e12
+    gbs = alg_bytes / (k_ms * 1e-3) / 1e9
+    if t_hbm >= t_tc:
+        e = {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"]}
+    else:
+        e = {"bound": "tensor", "achieved": tops, "peak": i8_burst, "unit": "Tops/s", "frac": tops / i8_burst}
+    e.update({"traffic": prof.get("dram_bytes"), "kernel_ms": k_ms, "tops": tops, "hbm_gbs": gbs,
+              "frac_tensor_burst_peak": tops / i8_burst, "frac_tensor_nominal_4500": tops / NOMINAL_I8_TOPS,
+              "frac_hbm_peak": gbs / peaks["hbm_gbs"], "algorithmic_bytes": alg_bytes, "algorithmic_ops": w.ops})
+    if prof:
+        e["ncu"] = prof
+    return e
+
+
+def useful_over_raw(p, w):
+    """Stored baselines / baselines the scheduled tiles compute (the paper's wasted-work measure)."""
+    raw = sum(si * sj for _, _, si, sj in p.tiles())
+    return (w.N * (w.N + 1) / 2) / raw
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--workload", default="cfg5_N1024")
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
-    ap.add_argument("--no-sweep", action="store_true", help="skip the by_config sweep")
+    ap.add_argument("--no-sweep", action="store_true", help="skip roofline.per_config and the extras")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
-    ap.add_argument("--f32-only", type=int, default=0, metavar="F",
-                    help="profiling aid: run only xc_correlate_f32 on config 3's values cut to F channels, 4 launches")
+    ap.add_argument("--no-sustained", action="store_true", help="skip the sustained legs")
+    ap.add_argument("--sustained-seconds", type=float, default=2.0)
+    ap.add_argument("--pitch", type=int, default=0, help="profiling aid: run the workload from a block with this row pitch")
+    ap.add_argument("--only", default="", choices=["", "f32", "fengine"],
+                    help="profiling aid: run only a few launches of that leg (for ncu) and print a short JSON line")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "native" else args.warmup
 
@@ -199,6 +335,7 @@ def main():
     import paper_1107_4264_b200 as xcb
     import xc_workloads as wl
     from paper_1107_4264_b200 import build as xc_build
+    import bench_legs
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the X-engine has no CPU path")
@@ -209,33 +346,26 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
         dist.barrier()
     xcb.load_library()
+    stream = torch.cuda.Stream()
 
-    if args.f32_only:
-        w3 = wl.CONFIGS["cfg3"]
-        sub = wl.Workload("cfg3_f32", w3.N, args.f32_only, w3.T, w3.kind, w3.sigma, w3.seed)
-        x3 = torch.from_numpy(wl.make_input(sub)).cuda().to(torch.float32)
-        p3 = xcb.Plan(sub.N, sub.F, sub.T)
-        v3 = p3.new_vis(torch.float32)
-        e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-        p3.correlate_f32(x3, v3)
-        e[0].record()
-        for _ in range(3):
-            p3.correlate_f32(x3, v3)
-        e[1].record()
-        torch.cuda.synchronize()
-        ms = e[0].elapsed_time(e[1]) / 3
-        print(json.dumps({"f32_only": True, "N": sub.N, "F": sub.F, "T": sub.T, "kernel_ms": ms,
-                          "tflops": sub.ops / (ms * 1e-3) / 1e12}))
+    if args.only:
+        print(json.dumps(bench_legs.only_leg(args.only, args.workload, stream)))
         return
 
     peaks = load_peaks()
+    i8_burst = peaks["bf16_burst"] * NOMINAL_I8_OVER_BF16          # Tops/s: measured bf16 burst x nominal int8/bf16 ratio
+    i8_sustained = peaks["bf16_sustained"] * NOMINAL_I8_OVER_BF16
     w = wl.CONFIGS[args.workload]
     # weak scaling: every rank holds its own block of F channels (seed differs per rank)
     x_np = wl.make_input(w, seed=w.seed + 7919 * rank)
     p = xcb.Plan(w.N, w.F, w.T)
-    stream = torch.cuda.Stream()
     xh = torch.from_numpy(x_np).pin_memory()
-    xd = xh.cuda()
+    if args.pitch:
+        p.set_in_pitch(args.pitch)
+        xd = torch.zeros((w.T, w.F, args.pitch), dtype=torch.int8, device="cuda")
+        xd[:, :, :4 * w.N] = xh.cuda().view(w.T, w.F, 4 * w.N)
+    else:
+        xd = xh.cuda()
     vis = p.new_vis()
     torch.cuda.synchronize()
 
@@ -268,57 +398,52 @@ def main():
     ms_step = ms_total / args.steps
     tops = world * w.ops / (ms_step * 1e-3) / 1e12
 
-    # ---- per-launch duration of the dominant kernel (events around each launch) -------------
-    per = time_kernel(p, xd, vis, stream, min(args.steps, 50), 1)
-    k_ms = sum(per) / len(per)
-    alg_bytes = w.in_bytes + w.vis_bytes                      # input once + output once
-    i8_peak = peaks["bf16_burst"] * NOMINAL_I8_OVER_BF16      # Tops/s: measured bf16 x nominal int8/bf16 ratio
-    t_hbm = alg_bytes / (peaks["hbm_gbs"] * 1e9)
-    t_tc = w.ops / (i8_peak * 1e12)
-    traffic = TRAFFIC_NCU.get(w.name)
-    if t_hbm >= t_tc:
-        ach = alg_bytes / (k_ms * 1e-3) / 1e9
-        roof = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": ach / peaks["hbm_gbs"], "traffic": traffic}
-    else:
-        ach = w.ops / (k_ms * 1e-3) / 1e12
-        roof = {"bound": "tensor", "achieved": ach, "peak": i8_peak, "unit": "Tops/s", "frac": ach / i8_peak,
-                "traffic": traffic}
-    roof.update({"kernel": "xc_i8_tc_kernel", "kernel_ms": k_ms, "peak_source": peaks["source"] +
-                 (" hbm_gbs" if roof["bound"] == "hbm" else " bf16_tflops (burst) x 2 (nominal int8/bf16)"),
-                 "algorithmic_bytes": alg_bytes, "algorithmic_ops": w.ops,
-                 "other_roof_frac": (w.ops / (k_ms * 1e-3) / 1e12 / i8_peak) if roof["bound"] == "hbm"
-                 else (alg_bytes / (k_ms * 1e-3) / 1e9 / peaks["hbm_gbs"])})
+    # ---- the dominant kernel: duration from its own stamps, burst roofline ---------------------
+    k_ms, ev_ms, mhz_k = kernel_durations(p, xd, vis, stream, min(max(args.steps, 5), 20))
+    roof = roofline_entry(w, k_ms, peaks, i8_burst, ncu_profile(w.name))
+    roof.update({
+        "kernel": "xc_i8_tc_kernel", "event_ms": ev_ms, "useful_over_raw": useful_over_raw(p, w),
+        "kernel_ms_how": "median over isolated launches of (max over CTAs of globaltimer at exit) - (min at entry), written by "
+                         "the kernel itself (xc_set_timing_buffer); event_ms = CUDA events around the same call (adds the launch gap)",
+        "peak_source": peaks["source"] + (" hbm_gbs (MEASURED_PEAKS.json)" if roof["bound"] == "hbm" else
+                                          " bf16_tflops (burst, MEASURED_PEAKS.json) x 2 (nominal int8/bf16 ratio): NOT a measured int8 number"),
+        "traffic_source": roof.get("ncu", {}).get("file"),
+    })
+    clocks["sm_mhz_in_kernel"] = mhz_k
+    clocks["sm_mhz_in_kernel_how"] = "clock64 / globaltimer stamped by CTA 0 of xc_i8_tc_kernel at entry and exit, median of isolated launches"
 
-    # ---- the SM clock the kernel REALLY ran at: CTA 0 stamps (clock64, globaltimer) at start and end ----------
-    # (NVML keeps reporting clocks.max.sm while the chip's power management already runs the tensor-heavy kernel
-    # slower; measured 1.2-1.6 GHz.  Reported beside the NVML figures, which stay in the contract's keys.)
-    probe = torch.zeros(xcb.TRACE_WORDS, dtype=torch.int64, device="cuda")
-    p.set_trace(probe)
-    mhz = []
-    with torch.cuda.stream(stream):
-        for _ in range(20):
-            p.correlate(xd, vis, stream=stream)
-            stream.synchronize()
-            t4 = probe[-4:].tolist()
-            if t4[3] > t4[1]:
-                mhz.append((t4[2] - t4[0]) / (t4[3] - t4[1]) * 1e3)
-    p.set_trace(None)
-    mhz.sort()
-    clocks["sm_mhz_in_kernel"] = mhz[len(mhz) // 2] if mhz else None
-    clocks["sm_mhz_in_kernel_how"] = ("clock64 / globaltimer stamped by CTA 0 of xc_i8_tc_kernel at its start and end, "
-                                      "median of 20 back-to-back launches after the timed region")
+    # ---- other denominators for "% of int8 tensor peak": measured cuBLAS int8 GEMM, nominal -----------
+    denominators = {"bf16_burst_x2": i8_burst, "bf16_sustained_x2": i8_sustained, "nominal_dense_int8": NOMINAL_I8_TOPS}
+    if rank == 0:
+        denominators.update(bench_legs.cublas_int8_peak(stream))
+    roof["denominators_tops"] = denominators
+    if denominators.get("cublas_int8_burst"):
+        roof["frac_vs_cublas_int8_burst"] = roof["tops"] / denominators["cublas_int8_burst"]
+
+    # ---- sustained leg of the headline workload ------------------------------------------------------------------
+    if not args.no_sustained:
+        s = sustained_leg(p, xd, vis, stream, sampler, args.sustained_seconds, k_ms)
+        s_tops = w.ops / (s["ms_per_launch"] * 1e-3) / 1e12
+        s.update({"tops": s_tops, "peak": i8_sustained, "frac": s_tops / i8_sustained,
+                  "peak_source": peaks["source"] + " bf16_tflops_sustained x 2 (nominal int8/bf16 ratio)",
+                  "frac_hbm_peak": (w.in_bytes + w.vis_bytes) / (s["ms_per_launch"] * 1e-3) / 1e9 / peaks["hbm_gbs"]})
+        if denominators.get("cublas_int8_sustained"):
+            s["frac_vs_cublas_int8_sustained"] = s_tops / denominators["cublas_int8_sustained"]
+        roof["sustained"] = s
 
     # ---- end to end through the C ABI with HOST buffers ---------------------------------------
     vh = torch.empty(p.vis_shape(), dtype=torch.int32).pin_memory()
+    scratch = p.new_scratch()
+    if args.pitch:
+        p.set_in_pitch(0)
     e2e_steps = max(3, min(args.steps, 10))
-    p.correlate_host(xh, vh, xd, vis, stream=stream)
+    p.correlate_host(xh, vh, scratch, vis, stream=stream)
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        p.correlate_host(xh, vh, xd, vis, stream=stream)       # synchronises the stream itself
+        p.correlate_host(xh, vh, scratch, vis, stream=stream)       # synchronises the stream itself
     e2e_s = (time.perf_counter() - t0) / e2e_steps
     if world > 1:
         t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
@@ -326,150 +451,56 @@ def main():
         e2e_s = float(t.item())
     e2e = {"value": world * w.ops / e2e_s / 1e12, "unit": "Tops/s", "h2d_bytes_per_step": world * w.in_bytes,
            "d2h_bytes_per_step": world * w.vis_bytes, "ms_per_step": 1e3 * e2e_s, "steps": e2e_steps,
-           "api": "xc_correlate_host (pinned host in/out)"}
+           "api": "xc_correlate_host (pinned host in/out)",
+           "pcie_floor_ms": 1e3 * max(w.in_bytes, w.vis_bytes) / 55e9}
+    del scratch, vh
 
-    # ---- the metric "vs N stations": kernel-only numbers for the other configs (rank 0, N=1) -----
-    by_config = {}
+    # ---- the metric "vs N stations": every BASELINE config, kernel only (rank 0, N=1) --------------------------
+    per_config = {}
+    extras = {}
     if rank == 0 and world == 1 and not args.no_sweep:
-        del xd, vis, xh, vh
+        per_config[w.name] = {k: roof[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic", "kernel_ms", "event_ms", "tops",
+                                                   "hbm_gbs", "frac_tensor_burst_peak", "frac_tensor_nominal_4500", "frac_hbm_peak",
+                                                   "useful_over_raw")}
+        per_config[w.name]["back_to_back_ms"] = ms_step
+        if "sustained" in roof:
+            per_config[w.name]["sustained"] = {k: roof["sustained"][k] for k in ("ms_per_launch", "tops", "frac", "nvml")}
+        if "ncu" in roof:
+            per_config[w.name]["tensor_pipe_active_ncu_pct"] = roof["ncu"].get("tensor_pipe_active_pct")
+        del xd, vis, xh
         torch.cuda.empty_cache()
-        for name in ["cfg1", "cfg3", "cfg4", "cfg5_N32", "cfg5_N64", "cfg5_N100", "cfg5_N500", "cfg5_N1024"]:
-            if name == args.workload:
+        for name in SWEEP:
+            if name == w.name:
                 continue
             ww = wl.CONFIGS[name]
             xx = torch.from_numpy(wl.make_input(ww)).cuda()
             pp = xcb.Plan(ww.N, ww.F, ww.T)
             vv = pp.new_vis()
-            d = time_kernel(pp, xx, vv, stream, 10, 3)
-            ms = sorted(d)[len(d) // 2]
-            # the same launch 20 times back to back between two events: what a caller streaming blocks sees (the
-            # kernels are launched with programmatic stream serialization, so launch latency and prologue overlap
-            # the previous kernel's tail -- the difference matters for the microsecond-scale small-N configs)
-            with torch.cuda.stream(stream):
-                b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                stream.synchronize()
-                b0.record(stream)
-                for _ in range(20):
-                    pp.correlate(xx, vv, stream=stream)
-                b1.record(stream)
-                stream.synchronize()
-            ms_b2b = b0.elapsed_time(b1) / 20
-            by_config[name] = {"N": ww.N, "F": ww.F, "T": ww.T, "kernel_ms": ms,
-                               "back_to_back_ms": ms_b2b, "tops_back_to_back": ww.ops / (ms_b2b * 1e-3) / 1e12,
-                               "tops": ww.ops / (ms * 1e-3) / 1e12,
-                               "frac_i8_peak": ww.ops / (ms * 1e-3) / 1e12 / i8_peak,
-                               "hbm_gbs": (ww.in_bytes + ww.vis_bytes) / (ms * 1e-3) / 1e9,
-                               "l2": "cold (input > L2)" if ww.in_bytes > 126e6 else "warm (input fits L2)"}
+            km, em, mhz = kernel_durations(pp, xx, vv, stream, 10)
+            prof = ncu_profile(name)
+            ent = roofline_entry(ww, km, peaks, i8_burst, prof)
+            ent.pop("ncu", None)
+            ent.update({"N": ww.N, "F": ww.F, "T": ww.T, "event_ms": em, "sm_mhz_in_kernel": mhz,
+                        "back_to_back_ms": back_to_back(pp, xx, vv, stream, 20 if ww.in_bytes > 60e6 else 200),
+                        "useful_over_raw": useful_over_raw(pp, ww), "tile": pp.tiles()[0][2:], "t_split": pp.t_split,
+                        "tensor_pipe_active_ncu_pct": prof.get("tensor_pipe_active_pct"),
+                        "l2": "cold (input > L2)" if ww.in_bytes > 126e6 else "warm (input fits L2)"})
+            ent["tops_back_to_back"] = ww.ops / (ent["back_to_back_ms"] * 1e-3) / 1e12
+            if name in SUSTAINED and not args.no_sustained:
+                s = sustained_leg(pp, xx, vv, stream, sampler, min(args.sustained_seconds, 1.5), km)
+                s_tops = ww.ops / (s["ms_per_launch"] * 1e-3) / 1e12
+                ent["sustained"] = {"ms_per_launch": s["ms_per_launch"], "tops": s_tops, "frac": s_tops / i8_sustained, "nvml": s["nvml"]}
+            per_config[name] = ent
             pp.close()
             del xx, vv
             torch.cuda.empty_cache()
-
-    # ---- S5 / S6 of the scope table: fp32 variant and two-stream pipeline (rank 0, N=1) -------------
-    extras = {}
-    if rank == 0 and world == 1 and not args.no_sweep:
-        # fp32-input variant on config 3's values (BASELINE.json configs[2]); ALU-bound: peak = SMs x 128 FMA x 2 x f_max
-        w3 = wl.CONFIGS["cfg3"]
-        x3 = torch.from_numpy(wl.make_input(w3)).cuda().to(torch.float32)
-        p3 = xcb.Plan(w3.N, w3.F, w3.T)
-        v3 = p3.new_vis(torch.float32)
-        for _ in range(3):
-            p3.correlate_f32(x3, v3, stream=stream)
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-        stream.synchronize()
-        ev[0].record(stream)
-        for _ in range(5):
-            p3.correlate_f32(x3, v3, stream=stream)
-        ev[1].record(stream)
-        stream.synchronize()
-        ms = ev[0].elapsed_time(ev[1]) / 5
-        sms = torch.cuda.get_device_properties(0).multi_processor_count
-        fp32_peak = sms * 128 * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
-        extras["f32"] = {"workload": "cfg3 values as float32 through xc_correlate_f32", "kernel_ms": ms,
-                         "tflops": w3.ops / (ms * 1e-3) / 1e12, "bound": "alu", "peak_tflops": fp32_peak,
-                         "frac": w3.ops / (ms * 1e-3) / 1e12 / fp32_peak,
-                         "peak_source": "SMs x 128 FMA/clk x 2 x clocks.max.sm (derived, DESIGN.md 5.2)",
-                         "context": "pure-register FFMA2 streams on this pool: 65.2 TFLOPS (constant operands), 57.7 TFLOPS "
-                                    "(this kernel's operand pattern); round-1 probe, DESIGN.md 5.2"}
-        p3.close()
-        del x3, v3
-        torch.cuda.empty_cache()
-        # 4-bit samples on config 2's shape: device-resident (unpack + X-engine) and
-        # end to end with host buffers (half the H2D bytes of the int8 call)
-        w2 = wl.CONFIGS["cfg2"]
-        x4h = torch.from_numpy(wl.packed_i4(w2.N, w2.F, w2.T, seed=2002)).pin_memory()
-        x4d = x4h.cuda()
-        p4 = xcb.Plan(w2.N, w2.F, w2.T)
-        v4 = p4.new_vis()
-        v4h = torch.empty(p4.vis_shape(), dtype=torch.int32).pin_memory()
-        for _ in range(3):
-            p4.correlate_i4(x4d, v4, stream=stream)
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-        stream.synchronize()
-        ev[0].record(stream)
-        for _ in range(20):
-            p4.correlate_i4(x4d, v4, stream=stream)
-        ev[1].record(stream)
-        stream.synchronize()
-        ms4 = ev[0].elapsed_time(ev[1]) / 20
-        p4.correlate_host_i4(x4h, v4h, x4d, v4, stream=stream)
-        t0 = time.perf_counter()
-        for _ in range(5):
-            p4.correlate_host_i4(x4h, v4h, x4d, v4, stream=stream)
-        e4 = (time.perf_counter() - t0) / 5
-        extras["i4"] = {"workload": "config 2's shape with 4-bit complex samples (uniform nibbles), xc_correlate_i4 / xc_correlate_host_i4",
-                        "device_ms": ms4, "tops": w2.ops / (ms4 * 1e-3) / 1e12, "launches_per_step": 2,
-                        "e2e_ms": 1e3 * e4, "e2e_tops": w2.ops / e4 / 1e12, "h2d_bytes_per_step": w2.in_bytes // 2,
-                        "d2h_bytes_per_step": w2.vis_bytes}
-        p4.close()
-        del x4h, x4d, v4, v4h
-        torch.cuda.empty_cache()
-        # two-stream run of config 5: 8 host blocks (the same seeded block 8 times: only the timing matters here;
-        # parity of the 8-distinct-block run is tests/test_xc_gpu.py::test_cfg5_two_stream_eight_blocks)
-        w5 = wl.CONFIGS["cfg5_N1024"]
-        blk = torch.from_numpy(wl.make_input(w5))
-        host = torch.empty((8,) + tuple(blk.shape), dtype=torch.int8).pin_memory()
-        for k in range(8):
-            host[k].copy_(blk)
-        p5 = xcb.Plan(w5.N, w5.F, w5.T)
-        dev2 = torch.empty(2 * p5.in_bytes, dtype=torch.int8, device="cuda")
-        v5 = p5.new_vis()
-        s2 = torch.cuda.Stream()
-        p5.correlate_pipelined(host, dev2, v5, stream, s2)
-        stream.synchronize()
-        t0 = time.perf_counter()
-        p5.correlate_pipelined(host, dev2, v5, stream, s2)
-        stream.synchronize()
-        tot = time.perf_counter() - t0
-        t0 = time.perf_counter()
-        for k in range(8):
-            dev2[:p5.in_bytes].view(torch.int8).copy_(host[k].view(-1), non_blocking=True)
-        torch.cuda.synchronize()
-        t_copy = time.perf_counter() - t0
-        xk = dev2[:p5.in_bytes].view(w5.T, w5.F, w5.N, 2, 2)
-        t_comp = 8e-3 * sorted(time_kernel(p5, xk, v5, stream, 5, 2))[2]
-        extras["two_stream"] = {"workload": "cfg5_N1024 x 8 pinned host blocks, xc_correlate_pipelined (Algorithm 1)",
-                                "total_ms": 1e3 * tot, "copy_alone_ms": 1e3 * t_copy, "compute_alone_ms": 1e3 * t_comp,
-                                "h2d_gbs": 8 * w5.in_bytes / tot / 1e9, "tops": 8 * w5.ops / tot / 1e12,
-                                "overlap_efficiency": max(t_copy, t_comp) / tot}
-        # the integrated run (Fig. 7): the same 8 blocks through xc_integrate -- int64 widening of the
-        # int32 partial sums and the copy of the result back to the host inside the timed region
-        v64 = torch.empty(p5.vis_shape(), dtype=torch.int64, device="cuda")
-        v64h = torch.empty(p5.vis_shape(), dtype=torch.int64).pin_memory()
-        p5.integrate(host, dev2, v5, v64, stream, s2, vis64_host=v64h)
-        stream.synchronize()
-        t0 = time.perf_counter()
-        p5.integrate(host, dev2, v5, v64, stream, s2, vis64_host=v64h)
-        stream.synchronize()
-        tot_i = time.perf_counter() - t0
-        extras["integrated"] = {"workload": "cfg5_N1024 x 8 pinned host blocks (16384 samples), xc_integrate: H2D pipeline, "
-                                            "X-engine, int64 widening, D2H of the int64 result",
-                                "total_ms": 1e3 * tot_i, "tops": 8 * w5.ops / tot_i / 1e12,
-                                "h2d_bytes": 8 * w5.in_bytes, "d2h_bytes": 2 * w5.vis_bytes,
-                                "pcie_floor_ms": 1e3 * (t_copy + 2 * w5.vis_bytes / (8 * w5.in_bytes / t_copy))}
-        del v64, v64h
-        p5.close()
-        del host, dev2, v5
-        torch.cuda.empty_cache()
+        roof["per_config"] = per_config
+        roof["per_config_note"] = ("burst: isolated launches, in-kernel duration, peak = bf16 burst x 2 (tensor) or measured HBM copy; "
+                                   "sustained: >= 1.5 s back to back, frac against bf16 sustained x 2; tensor_pipe_active_ncu_pct from the "
+                                   "tracked ncu exports under profiles/ (null = no capture this round)")
+        extras = bench_legs.extras(stream, clocks, sampler, peaks)
+    else:
+        del xd, vis, xh
 
     # ---- CPU baseline: the oracle on a bounded sample (rank 0 at N=1 only) --------------------
     cpu = None
@@ -488,8 +519,7 @@ def main():
                        "l2": "input block (%.0f MB) + output (%.0f MB) exceed the 126 MB L2: every step is cold"
                              % (w.in_bytes / 1e6, w.vis_bytes / 1e6)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * launches_per_step,
-            "roofline": roof, "cpu_baseline": cpu, "by_config": by_config, "extras": extras,
-            "frac_of_int8_peak": tops / world / i8_peak, "int8_peak_tops": i8_peak,
+            "roofline": roof, "cpu_baseline": cpu, "extras": extras,
             "paper_context": "1058 GFLOPS = 79% of fp32 peak on a GeForce GTX 480 (PAPER.md:267); other hardware",
         }
         print(json.dumps(out))
@@ -497,14 +527,6 @@ def main():
         dist.barrier()
         dist.destroy_process_group()
 
-
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of xc_i8_tc_kernel from `ncu --set full`
-# captures (see profiles/*.md for the command and the raw numbers); null until captured.
-TRAFFIC_NCU: dict = {
-    "cfg2": 524557824 + 237699584,        # profiles/r1_ncu_full_cfg2.md
-    "cfg4": 524457216 + 1019722000,       # profiles/r1_ncu_full_cfg4.md
-    "cfg5_N1024": 537382656 + 1022897000,  # profiles/r1_ncu_full_cfg5N1024.md
-}
 
 if __name__ == "__main__":
     main()

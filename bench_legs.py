@@ -1,0 +1,210 @@
+"""bench_legs.py -- the secondary legs of bench.py (rank 0, one GPU): the other steps of SURVEY 8(a)/(f) beside the int8
+X-engine -- fp32 variant (S5), two-stream pipeline (S6), integrated run, 4-bit samples, pitched N = 500 input, F-engine and
+FX chain -- and the measured cuBLAS int8 GEMM rate used as an extra roofline denominator.  Everything here goes through the
+C-ABI library exactly as bench.py's main leg does; nothing imports the oracle."""
+from __future__ import annotations
+
+import time
+
+
+def _timed(fn, stream, n, warm=3):
+    """Mean ms of n back-to-back calls of fn() between two events on `stream`."""
+    import torch
+    with torch.cuda.stream(stream):
+        for _ in range(warm):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        stream.synchronize()
+        e0.record(stream)
+        for _ in range(n):
+            fn()
+        e1.record(stream)
+        stream.synchronize()
+    return e0.elapsed_time(e1) / n
+
+
+def cublas_int8_peak(stream):
+    """cuBLAS int8 GEMM (torch._int_mm, 8192^3, int32 accumulate) on this very GPU: best of 10 (burst) and the mean of a
+    ~1.5 s back-to-back loop (sustained).  A LIBRARY kernel used only as a denominator: what a vendor GEMM of the same
+    dtype reaches, next to bf16 x 2 and the nominal 4500 Tops."""
+    import torch
+    try:
+        n = 8192
+        a = torch.randint(-127, 128, (n, n), dtype=torch.int8, device="cuda")
+        b = torch.randint(-127, 128, (n, n), dtype=torch.int8, device="cuda")
+        ops = 2.0 * n ** 3
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                torch._int_mm(a, b)
+            best = 1e9
+            for _ in range(10):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                torch._int_mm(a, b)
+                e1.record(stream)
+                stream.synchronize()
+                best = min(best, e0.elapsed_time(e1))
+            reps = max(50, int(1.5 / (best * 1e-3)))
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                torch._int_mm(a, b)
+            e1.record(stream)
+            stream.synchronize()
+            sus = e0.elapsed_time(e1) / reps
+        del a, b
+        torch.cuda.empty_cache()
+        return {"cublas_int8_burst": ops / (best * 1e-3) / 1e12, "cublas_int8_sustained": ops / (sus * 1e-3) / 1e12,
+                "cublas_int8_how": "torch._int_mm 8192^3 measured in this run: best of 10 / mean over ~1.5 s back to back"}
+    except Exception as e:  # noqa: BLE001 -- a missing library routine must not fail the bench
+        return {"cublas_int8_burst": None, "cublas_int8_sustained": None, "cublas_int8_how": f"unavailable: {e!r}"}
+
+
+def f32_leg(stream, clocks, F=None, launches=5):
+    import torch
+    import paper_1107_4264_b200 as xcb
+    import xc_workloads as wl
+    w3 = wl.CONFIGS["cfg3"]
+    if F:
+        w3 = wl.Workload("cfg3_f32", w3.N, F, w3.T, w3.kind, w3.sigma, w3.seed)
+    x3 = torch.from_numpy(wl.make_input(w3)).cuda().to(torch.float32)
+    p3 = xcb.Plan(w3.N, w3.F, w3.T)
+    v3 = p3.new_vis(torch.float32)
+    ms = _timed(lambda: p3.correlate_f32(x3, v3, stream=stream), stream, launches)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    fp32_peak = sms * 128 * 2 * ((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+    out = {"workload": f"cfg3 values (N={w3.N}, F={w3.F}, T={w3.T}) as float32 through xc_correlate_f32", "kernel_ms": ms,
+           "tflops": w3.ops / (ms * 1e-3) / 1e12, "bound": "alu", "peak_tflops": fp32_peak,
+           "frac": w3.ops / (ms * 1e-3) / 1e12 / fp32_peak,
+           "peak_source": "SMs x 128 FMA/clk x 2 x clocks.max.sm (derived, DESIGN.md 5.2)"}
+    p3.close()
+    del x3, v3
+    torch.cuda.empty_cache()
+    return out
+
+
+def only_leg(which, workload, stream):
+    """Profiling aid for ncu captures: a few launches of one secondary kernel."""
+    if which == "f32":
+        return {"only": "f32", **f32_leg(stream, None, F=32, launches=3)}
+    if which == "fengine":
+        return {"only": "fengine", **fengine_leg(stream, workload, launches=3, with_fx=False)}
+    raise ValueError(which)
+
+
+def fengine_leg(stream, workload, launches=10, with_fx=True):
+    """F-engine + corner turn and the FX chain; filled in once the library exports them."""
+    import paper_1107_4264_b200 as xcb
+    if not hasattr(xcb.Plan, "fengine"):
+        return {"unavailable": "this build of the library has no F-engine"}
+    return _fx_leg(stream, workload, launches, with_fx)
+
+
+def extras(stream, clocks, sampler, peaks):
+    import torch
+    import paper_1107_4264_b200 as xcb
+    import xc_workloads as wl
+    out = {}
+    # ---- S5: fp32-input variant on config 3's values (BASELINE.json configs[2]); ALU-bound ------------------
+    out["f32"] = f32_leg(stream, clocks)
+
+    # ---- N = 500 from a block with 128-byte-multiple rows (xc_set_in_pitch; what the F-engine / the host paths produce) ----
+    w5 = wl.CONFIGS["cfg5_N500"]
+    p5 = xcb.Plan(w5.N, w5.F, w5.T)
+    pitch = p5.scratch_pitch
+    xp = torch.zeros((w5.T, w5.F, pitch), dtype=torch.int8, device="cuda")
+    xp[:, :, :4 * w5.N] = torch.from_numpy(wl.make_input(w5)).cuda().view(w5.T, w5.F, 4 * w5.N)
+    p5.set_in_pitch(pitch)
+    v5 = p5.new_vis()
+    ms = _timed(lambda: p5.correlate(xp, v5, stream=stream), stream, 20)
+    i8_burst = peaks["bf16_burst"] * 2.0
+    out["N500_pitched"] = {"workload": f"cfg5_N500 values in a block with row pitch {pitch} B (xc_set_in_pitch) instead of 2000 B",
+                           "back_to_back_ms": ms, "tops": w5.ops / (ms * 1e-3) / 1e12,
+                           "frac_tensor_burst_peak": w5.ops / (ms * 1e-3) / 1e12 / i8_burst}
+    # the same N through the host-buffer call: the H2D copy re-pitches, so end to end N = 500 pays no pitch penalty
+    xh = torch.from_numpy(wl.make_input(w5)).pin_memory()
+    vh = torch.empty(p5.vis_shape(), dtype=torch.int32).pin_memory()
+    p5.set_in_pitch(0)
+    scr = p5.new_scratch()
+    p5.correlate_host(xh, vh, scr, v5, stream=stream)
+    t0 = time.perf_counter()
+    for _ in range(3):
+        p5.correlate_host(xh, vh, scr, v5, stream=stream)
+    e = (time.perf_counter() - t0) / 3
+    out["N500_pitched"].update({"e2e_ms": 1e3 * e, "e2e_tops": w5.ops / e / 1e12, "e2e_h2d_gbs": w5.in_bytes / e / 1e9})
+    p5.close()
+    del xp, v5, xh, vh, scr
+    torch.cuda.empty_cache()
+
+    # ---- 4-bit samples on config 2's shape ---------------------------------
+    w2 = wl.CONFIGS["cfg2"]
+    x4h = torch.from_numpy(wl.packed_i4(w2.N, w2.F, w2.T, seed=2002)).pin_memory()
+    x4d = x4h.cuda()
+    p4 = xcb.Plan(w2.N, w2.F, w2.T)
+    v4 = p4.new_vis()
+    v4h = torch.empty(p4.vis_shape(), dtype=torch.int32).pin_memory()
+    ms4 = _timed(lambda: p4.correlate_i4(x4d, v4, stream=stream), stream, 20)
+    p4.correlate_host_i4(x4h, v4h, x4d, v4, stream=stream)
+    t0 = time.perf_counter()
+    for _ in range(5):
+        p4.correlate_host_i4(x4h, v4h, x4d, v4, stream=stream)
+    e4 = (time.perf_counter() - t0) / 5
+    out["i4"] = {"workload": "config 2's shape with 4-bit complex samples (uniform nibbles), xc_correlate_i4 / xc_correlate_host_i4",
+                 "device_ms": ms4, "tops": w2.ops / (ms4 * 1e-3) / 1e12, "launches_per_step": 2,
+                 "e2e_ms": 1e3 * e4, "e2e_tops": w2.ops / e4 / 1e12, "h2d_bytes_per_step": w2.in_bytes // 2,
+                 "d2h_bytes_per_step": w2.vis_bytes}
+    p4.close()
+    del x4h, x4d, v4, v4h
+    torch.cuda.empty_cache()
+
+    # ---- S6: two-stream run of config 5: 8 host blocks (the same seeded block 8 times: only the timing matters here;
+    # parity of the 8-distinct-block run is tests/test_xc_gpu.py::test_cfg5_two_stream_eight_blocks) -------------------
+    w5 = wl.CONFIGS["cfg5_N1024"]
+    blk = torch.from_numpy(wl.make_input(w5))
+    host = torch.empty((8,) + tuple(blk.shape), dtype=torch.int8).pin_memory()
+    for k in range(8):
+        host[k].copy_(blk)
+    p5 = xcb.Plan(w5.N, w5.F, w5.T)
+    dev2 = p5.new_scratch(2)
+    v5 = p5.new_vis()
+    s2 = torch.cuda.Stream()
+    p5.correlate_pipelined(host, dev2, v5, stream, s2)
+    stream.synchronize()
+    t0 = time.perf_counter()
+    p5.correlate_pipelined(host, dev2, v5, stream, s2)
+    stream.synchronize()
+    tot = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    for k in range(8):
+        dev2[:p5.in_bytes].copy_(host[k].view(-1), non_blocking=True)
+    torch.cuda.synchronize()
+    t_copy = time.perf_counter() - t0
+    xk = dev2[:p5.in_bytes].view(w5.T, w5.F, w5.N, 2, 2)
+    t_comp = 8e-3 * _timed(lambda: p5.correlate(xk, v5, stream=stream), stream, 5, warm=2)
+    out["two_stream"] = {"workload": "cfg5_N1024 x 8 pinned host blocks, xc_correlate_pipelined (Algorithm 1)",
+                         "total_ms": 1e3 * tot, "copy_alone_ms": 1e3 * t_copy, "compute_alone_ms": 1e3 * t_comp,
+                         "h2d_gbs": 8 * w5.in_bytes / tot / 1e9, "tops": 8 * w5.ops / tot / 1e12,
+                         "overlap_efficiency": max(t_copy, t_comp) / tot}
+    # the integrated run (Fig. 7): the same 8 blocks through xc_integrate -- int64 widening of the
+    # int32 partial sums and the copy of the result back to the host inside the timed region
+    v64 = torch.empty(p5.vis_shape(), dtype=torch.int64, device="cuda")
+    v64h = torch.empty(p5.vis_shape(), dtype=torch.int64).pin_memory()
+    p5.integrate(host, dev2, v5, v64, stream, s2, vis64_host=v64h)
+    stream.synchronize()
+    t0 = time.perf_counter()
+    p5.integrate(host, dev2, v5, v64, stream, s2, vis64_host=v64h)
+    stream.synchronize()
+    tot_i = time.perf_counter() - t0
+    out["integrated"] = {"workload": "cfg5_N1024 x 8 pinned host blocks (16384 samples), xc_integrate: H2D pipeline, "
+                                     "X-engine, int64 widening, D2H of the int64 result",
+                         "total_ms": 1e3 * tot_i, "tops": 8 * w5.ops / tot_i / 1e12,
+                         "h2d_bytes": 8 * w5.in_bytes, "d2h_bytes": 2 * w5.vis_bytes,
+                         "pcie_floor_ms": 1e3 * (t_copy + 2 * w5.vis_bytes / (8 * w5.in_bytes / t_copy))}
+    del v64, v64h
+    p5.close()
+    del host, dev2, v5
+    torch.cuda.empty_cache()
+
+    # ---- F-engine + corner turn, and the FX chain ----------------------------------------------------------
+    out["fx"] = fengine_leg(stream, "cfg3")
+    return out

@@ -78,36 +78,29 @@ enum {
     XC_I8_KERNEL_SIMT = 2  /* plain CUDA-core kernel, one thread per baseline: a debugging    */
                            /* aid that shares no device code with the tensor-core kernel     */
 };
-/* Tensor-core tile shapes (Gram rows x Gram columns; 4 Gram rows = 1 station), xc_set_option(XC_OPT_TILE, ...). */
+/* Tensor-core tile shapes (Gram rows x Gram columns; 4 Gram rows = 1 station), xc_set_option(XC_OPT_TILE, ...).
+ * Round 1 also built 128x256 single-CTA tiles, a staged (bulk-store) epilogue, 64/256-sample stages and two
+ * diagonal-specialised schedules (SPLIT, MIXED); all measured slower than these two and were removed. */
 enum {
-    XC_TILE_AUTO = 0,         /* chosen from N at plan time                                        */
+    XC_TILE_AUTO = 0,         /* chosen from N, F and the SM count                                 */
     XC_TILE_1CTA_128x128 = 1, /* 32 x 32 stations on one CTA (small N)                             */
-    XC_TILE_1CTA_128x256 = 2, /* 32 x 64 stations on one CTA                                       */
-    XC_TILE_2CTA_256x256 = 3, /* 64 x 64 stations on a CTA pair (tcgen05 cta_group::2)             */
-    XC_TILE_SPLIT = 4,        /* two launches: every diagonal 64-station block on ONE CTA as two sub-tiles  */
-                              /* (32 x 64 stations, then 32 x 32: the block's i > j quarter is never      */
-                              /* computed), every off-diagonal 64 x 64 block on a CTA pair (reads the      */
-                              /* input from HBM twice: kept for testing)                                   */
-    XC_TILE_MIXED = 5         /* the same schedule in ONE launch: some clusters work as two single CTAs on  */
-                              /* diagonal blocks, the others as CTA pairs on off-diagonal blocks            */
-};
-/* Epilogue store path of the tensor-core kernel, xc_set_option(XC_OPT_EPILOGUE, ...). */
-enum {
-    XC_EPI_AUTO = 0,
-    XC_EPI_DIRECT = 1, /* registers -> 16-byte streaming global stores                                   */
-    XC_EPI_STAGED = 2  /* registers -> packed tile in shared memory -> bulk (TMA) stores / reduce-adds   */
+    XC_TILE_2CTA_256x256 = 3  /* 64 x 64 stations on a CTA pair (tcgen05 cta_group::2)             */
 };
 typedef enum {
     XC_OPT_I8_KERNEL = 0, /* one of XC_I8_KERNEL_*                                            */
     XC_OPT_MAX_CTAS = 1,  /* cap on persistent CTAs of the tensor-core kernel (0 = SM count)  */
-    XC_OPT_FORCE_STAGE = 2, /* 1 = always run the staging (pad/copy) kernel, for testing S0    */
+    XC_OPT_FORCE_STAGE = 2, /* 1 = always run the staging (re-pitch/copy) kernel, for testing S0 */
     XC_OPT_TILE = 4,       /* one of XC_TILE_*; rebuilds the tile schedule (synchronising on next call) */
-    XC_OPT_EPILOGUE = 5,   /* one of XC_EPI_*                                                  */
-    XC_OPT_BK = 6,         /* samples per pipeline stage of the CTA-pair kernel: 0 (auto), 128 or 256 */
     XC_OPT_PDL = 7,        /* 1 (default) = launch the tensor-core kernels with programmatic stream            */
                            /* serialization: the prologue overlaps the previous kernel's tail; 0 = plain launch */
-    XC_OPT_DEBUG_SKIP = 3  /* PROFILING ONLY, results become meaningless: bit 0 = no TMA loads  */
-                           /* after the first ring fill, bit 1 = no MMAs, bit 2 = no stores     */
+    XC_OPT_TSPLIT = 8      /* T-split of the single-CTA tile over a cluster of 2 (the paper's small-N future    */
+                           /* work): 0 = auto (on when 2 * tiles * F <= SM count), 1 = off,   */
+                           /* 2 = on whenever T allows it.  Results are identical either way.                   */
+#ifdef XC_PROFILE
+    , XC_OPT_DEBUG_SKIP = 3 /* PROFILING BUILD ONLY (-DXC_PROFILE), results become meaningless: bit 0 = no TMA */
+                            /* loads after the first ring fill, bit 1 = no MMAs, bit 2 = no stores, bit 3 =    */
+                            /* all stores wrapped into an 8 MB window                                           */
+#endif
 } xc_option;
 
 /* xc_plan -- north_star's xc_plan(N, P=2, F, T, layout).
@@ -123,21 +116,46 @@ int xc_plan(xc_plan_t** out, int N, int P, int F, int T, int layout);
 void xc_destroy(xc_plan_t* plan);
 
 /* Sizes in bytes of one input block / one output cube for this plan. */
-size_t xc_in_bytes(const xc_plan_t* plan);      /* int8 path:  4*N*F*T            */
+size_t xc_in_bytes(const xc_plan_t* plan);      /* int8 path:  xc_in_pitch()*F*T = 4*N*F*T unless xc_set_in_pitch was called */
 size_t xc_in_bytes_f32(const xc_plan_t* plan);  /* fp32 path: 16*N*F*T            */
 size_t xc_in_bytes_i4(const xc_plan_t* plan);   /* 4-bit path: 2*N*F*T            */
 size_t xc_vis_bytes(const xc_plan_t* plan);     /* 32*NB*F (int32 and float alike) */
 /* N(N+1)/2. */
 size_t xc_n_baselines(const xc_plan_t* plan);
 
+/* Row pitch of device input blocks (the paper's coalescing rule -- rows aligned to the memory
+ * line -- is, for TMA, a row pitch that is a multiple of 128 bytes).  By default an input block is dense: the rows
+ * (t, f) of 4N bytes follow each other (pitch 4N).  xc_set_in_pitch declares that the in_dev blocks handed to
+ * xc_correlate / _acc / _channels have their rows row_pitch_bytes apart (>= 4N; bytes beyond 4N of a row are ignored;
+ * 0 restores the dense default).  A producer that is free to choose (the F-engine below, a capture card) should use
+ * xc_scratch_pitch(): with N = 500 the X-engine then runs at the speed of N = 512 instead of ~25 % slower.
+ * xc_in_pitch returns the current value. */
+int xc_set_in_pitch(xc_plan_t* plan, size_t row_pitch_bytes);
+size_t xc_in_pitch(const xc_plan_t* plan);
+/* The library's own pitch, 4N rounded up to 128 bytes (the row pitch of the staging workspace, of the host-buffer
+ * calls' device blocks and of the F-engine's cube), and the size of in_dev_scratch of xc_correlate_host / of each half
+ * of dev_buf2 of xc_correlate_pipelined / xc_integrate: one block with that pitch, plus -- when 4N is not already a
+ * multiple of 128 -- a dense landing area for the host->device copy (a small kernel spreads the rows: the copy engine
+ * moves dense blocks at the full PCIe rate, pitched 2000-byte rows at a quarter of it). */
+size_t xc_scratch_pitch(const xc_plan_t* plan);
+size_t xc_scratch_in_bytes(const xc_plan_t* plan);
+
 /* Staging.  The tensor-core kernel reads the input through TMA, which
- * needs a 16-byte-aligned base and a 16-byte-multiple row pitch (4N bytes -> N % 4 == 0).
- * Otherwise the input is first copied by a padding kernel into a workspace of
- * xc_workspace_bytes() bytes (4 * roundup(N, 4) * F * T; the 4-bit path always uses it).  The caller may hand one in (device
- * memory, 128-byte aligned, kept until xc_destroy or replaced); if none was set the
- * library cudaMallocs one on first need (a synchronising call) and frees it in xc_destroy. */
+ * needs a 16-byte-aligned base and a 16-byte-multiple row pitch (dense rows: N % 4 == 0).
+ * Otherwise the input is first copied by a staging kernel into a workspace of
+ * xc_workspace_bytes() = xc_scratch_in_bytes() bytes (the 4-bit path always unpacks into it).  The caller may hand one
+ * in (device memory, 128-byte aligned, kept until xc_destroy or replaced); if none was set the
+ * library cudaMallocs one on first need (a synchronising call) and frees it in xc_destroy.  The workspace is
+ * plan-wide: staged calls issued on different streams are ordered against each other by an event. */
 size_t xc_workspace_bytes(const xc_plan_t* plan);
 int xc_set_workspace(xc_plan_t* plan, void* ws_dev, size_t bytes);
+
+/* Kernel timing without a profiler: stamps_dev = device buffer of 6 uint64 (or NULL to switch off).  Every CTA of the
+ * tensor-core kernel then atomically folds the global nanosecond timer into [0] (min, at kernel entry) and [1] (max, at
+ * exit) -- the caller presets [0] = UINT64_MAX and [1] = 0 before the launch, and [1] - [0] is the kernel's duration --
+ * and CTA 0 writes (clock64, globaltimer) at its entry into [2], [3] and at its exit into [4], [5], from which the SM
+ * clock the kernel really ran at follows.  Costs two atomics per CTA; nothing when off. */
+int xc_set_timing_buffer(xc_plan_t* plan, uint64_t* stamps_dev);
 
 int xc_set_option(xc_plan_t* plan, int option, int value);
 
@@ -170,8 +188,8 @@ int xc_correlate_f32(xc_plan_t* plan, const float* in_dev, float* vis_dev, int a
 
 /* xc_correlate_pipelined -- Algorithm 1 read as textbook double
  *   buffering: n_blocks input blocks of xc_in_bytes() each lie back to back in PINNED host
- *   memory at in_host; block p+1 is copied host->device on copy_stream into one half of
- *   dev_buf2 (2 * xc_in_bytes() bytes of device memory, 128-byte aligned) while block p is
+ *   memory at in_host (dense, 4*N*F*T bytes each); block p+1 is copied host->device on copy_stream into one half of
+ *   dev_buf2 (2 * xc_scratch_in_bytes() bytes of device memory, 128-byte aligned) while block p is
  *   correlated on compute_stream from the other half; events order the two streams (no host
  *   synchronisation inside).  vis_dev = sum over blocks (first block overwrites).  The result
  *   stays on the device.  Returns after enqueueing; the caller synchronises
@@ -200,8 +218,9 @@ int xc_correlate_channels(xc_plan_t* plan, const int8_t* in_dev, int32_t* vis_de
                           void* cuda_stream);
 
 /* xc_correlate_host -- the integrated run with HOST buffers (Fig. 7: host->device copy,
- *   X-engine, device->host copy of the result): copies in_host (xc_in_bytes(), pinned for full speed) to
- *   in_dev_scratch, correlates, copies the result into vis_host (xc_vis_bytes(), pinned for full speed) and
+ *   X-engine, device->host copy of the result): copies in_host (dense, 4*N*F*T bytes, pinned for full speed) to
+ *   in_dev_scratch (xc_scratch_in_bytes(), 16-byte aligned; rows are re-pitched to 128-byte multiples on the device, so any N -- N % 4 != 0
+ *   included -- goes through the channel-range pipeline), correlates, copies the result into vis_host (xc_vis_bytes(), pinned for full speed) and
  *   synchronises the stream before returning.  Blocks of 8 MiB and more are cut into up to 16 channel ranges so
  *   that the copy-in of range c+1, the X-engine on range c and the copy-out of range c-1 overlap; the copies then
  *   run on two plan-owned streams ordered against cuda_stream by events (the only place the library uses streams
@@ -214,11 +233,12 @@ int xc_correlate_host(xc_plan_t* plan, const int8_t* in_host, int32_t* vis_host,
 int xc_correlate_host_i4(xc_plan_t* plan, const uint8_t* in4_host, int32_t* vis_host, uint8_t* in4_dev_scratch,
                          int32_t* vis_dev_scratch, void* cuda_stream);
 
-/* PROFILING ONLY: trace_dev = device buffer of 3*256*4 + 4 int64 (or NULL to switch off); CTA 0 of the
- * tensor-core kernel writes clock64() stamps of its first 256 pipeline iterations per warp role
- * (0 = TMA producer, 1 = MMA issuer, 2 = epilogue) into it (CTA-pair kernel only), and every tensor-core kernel
- * writes {clock64, globaltimer} at its start and end into the last 4 words (effective SM clock of the launch). */
+#ifdef XC_PROFILE
+/* PROFILING BUILD ONLY (-DXC_PROFILE; libxc_profile.so): trace_dev = device buffer of 3*256*4 int64 (or NULL to switch
+ * off); CTA 0 of the tensor-core kernel writes clock64() stamps of its first 256 pipeline iterations per warp role
+ * (0 = TMA producer, 1 = MMA issuer, 2 = epilogue) into it. */
 int xc_debug_set_trace(xc_plan_t* plan, void* trace_dev);
+#endif
 
 /* Tile schedule introspection (for tests of the triangular map).
  *   xc_tile_count: number of scheduled tiles per channel for the integer path.
@@ -226,6 +246,8 @@ int xc_debug_set_trace(xc_plan_t* plan, void* trace_dev);
  *                  the tile's extent in stations (si stations on the i side, sj on the j side). */
 int xc_tile_count(const xc_plan_t* plan);
 int xc_tile_get(const xc_plan_t* plan, int k, int* bi, int* bj, int* si, int* sj);
+/* T-split factor (1 or 2) used by the last integer compute call on this plan (see XC_OPT_TSPLIT). */
+int xc_t_split(const xc_plan_t* plan);
 
 /* The paper's closed-form triangular map and its inverse:
  *   g = by(by+1)/2 + bx,  by = floor(-1/2 + sqrt(1/4 + 2g)),  bx = g - by(by+1)/2,

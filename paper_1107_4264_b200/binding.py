@@ -10,22 +10,26 @@ import os
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libxc.so")
+LIB_PROFILE_PATH = os.path.join(HERE, "libxc_profile.so")
 
 MAX_T = 65535
-TRACE_WORDS = 3 * 256 * 4 + 4
+TIMING_WORDS = 6          # uint64 words of the xc_set_timing_buffer buffer
+TRACE_WORDS = 3 * 256 * 4  # int64 words of the profiling build's trace buffer
 I8_KERNEL_AUTO, I8_KERNEL_TC, I8_KERNEL_SIMT = 0, 1, 2
-OPT_I8_KERNEL, OPT_MAX_CTAS, OPT_FORCE_STAGE, OPT_DEBUG_SKIP, OPT_TILE, OPT_EPILOGUE, OPT_BK, OPT_PDL = 0, 1, 2, 3, 4, 5, 6, 7
-EPI_AUTO, EPI_DIRECT, EPI_STAGED = 0, 1, 2
-TILE_AUTO, TILE_1CTA_128x128, TILE_1CTA_128x256, TILE_2CTA_256x256, TILE_SPLIT, TILE_MIXED = 0, 1, 2, 3, 4, 5
+OPT_I8_KERNEL, OPT_MAX_CTAS, OPT_FORCE_STAGE, OPT_DEBUG_SKIP, OPT_TILE, OPT_PDL, OPT_TSPLIT = 0, 1, 2, 3, 4, 7, 8
+TILE_AUTO, TILE_1CTA_128x128, TILE_2CTA_256x256 = 0, 1, 3
 
 # every symbol include/xc.h declares
 EXPORTED_SYMBOLS = (
     "xc_plan", "xc_destroy", "xc_in_bytes", "xc_in_bytes_f32", "xc_vis_bytes", "xc_n_baselines",
     "xc_workspace_bytes", "xc_set_workspace", "xc_set_option", "xc_correlate", "xc_correlate_acc",
-    "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_integrate", "xc_correlate_i4", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get",
-    "xc_debug_set_trace", "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error",
-    "xc_version",
+    "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_integrate",
+    "xc_correlate_i4", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get", "xc_t_split",
+    "xc_set_in_pitch", "xc_in_pitch", "xc_scratch_pitch", "xc_scratch_in_bytes", "xc_set_timing_buffer",
+    "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error", "xc_version",
 )
+# additionally exported by the profiling build only (libxc_profile.so, -DXC_PROFILE)
+PROFILE_SYMBOLS = ("xc_debug_set_trace",)
 
 
 class XcError(RuntimeError):
@@ -65,7 +69,10 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_correlate_pipelined": (i, [p, p, i, p, p, p, p]),
         "xc_correlate_host": (i, [p, p, p, p, p, p]),
         "xc_correlate_host_i4": (i, [p, p, p, p, p, p]),
-        "xc_debug_set_trace": (i, [p, p]),
+        "xc_set_in_pitch": (i, [p, sz]), "xc_in_pitch": (sz, [p]),
+        "xc_scratch_pitch": (sz, [p]), "xc_scratch_in_bytes": (sz, [p]),
+        "xc_set_timing_buffer": (i, [p, p]),
+        "xc_t_split": (i, [p]),
         "xc_tile_count": (i, [p]),
         "xc_tile_get": (i, [p, i, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i)]),
         "xc_tri_index": (i64, [i64, i64]),
@@ -75,6 +82,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_last_cuda_error": (ctypes.c_char_p, [p]),
         "xc_version": (ctypes.c_char_p, []),
     }
+    if hasattr(L, "xc_debug_set_trace"):      # profiling build
+        sig["xc_debug_set_trace"] = (i, [p, p])
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
         fn.restype = res
@@ -190,16 +199,53 @@ class Plan:
         return out
 
     def set_trace(self, buf) -> None:
-        """PROFILING ONLY: buf = int64 CUDA tensor of TRACE_WORDS elements (or None): see xc_debug_set_trace."""
+        """PROFILING BUILD ONLY (load_library(LIB_PROFILE_PATH)): buf = int64 CUDA tensor of TRACE_WORDS elements or None."""
+        if not hasattr(lib(), "xc_debug_set_trace"):
+            raise RuntimeError("xc_debug_set_trace exists only in libxc_profile.so (build with --profile)")
         self._check(lib().xc_debug_set_trace(self._h, ctypes.c_void_p(buf.data_ptr() if buf is not None else 0)),
                     "xc_debug_set_trace")
         self._trace = buf
 
+    def set_timing_buffer(self, buf) -> None:
+        """buf = CUDA tensor of TIMING_WORDS 64-bit words (or None): see xc_set_timing_buffer.  Preset buf[0] = max, buf[1] = 0
+        before each launch; afterwards buf[1] - buf[0] is the kernel's duration in ns."""
+        self._check(lib().xc_set_timing_buffer(self._h, ctypes.c_void_p(buf.data_ptr() if buf is not None else 0)),
+                    "xc_set_timing_buffer")
+        self._stamps = buf
+
+    def set_in_pitch(self, row_pitch_bytes: int) -> None:
+        self._check(lib().xc_set_in_pitch(self._h, row_pitch_bytes), "xc_set_in_pitch")
+
+    @property
+    def in_pitch(self) -> int:
+        return int(lib().xc_in_pitch(self._h))
+
+    @property
+    def scratch_pitch(self) -> int:
+        return int(lib().xc_scratch_pitch(self._h))
+
+    @property
+    def scratch_in_bytes(self) -> int:
+        return int(lib().xc_scratch_in_bytes(self._h))
+
+    @property
+    def t_split(self) -> int:
+        return int(lib().xc_t_split(self._h))
+
+    def new_scratch(self, n: int = 1, device="cuda"):
+        """Device scratch for the host-buffer calls: n * scratch_in_bytes int8 (rows re-pitched to 128-byte multiples)."""
+        import torch
+        return torch.empty(n * self.scratch_in_bytes, dtype=torch.int8, device=device)
+
     # compute -------------------------------------------------------------------------------
     def _chk_in(self, x, dtype):
         import torch
-        if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == dtype and x.is_contiguous()
-                and tuple(x.shape) == self.in_shape()):
+        ok = isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == dtype and x.is_contiguous()
+        if ok and dtype == torch.int8 and tuple(x.shape) == (self.T, self.F, self.in_pitch):
+            return                                     # block given as [T][F][row pitch in bytes] (xc_set_in_pitch)
+        if ok and dtype == torch.int8 and self.in_pitch != 4 * self.N:
+            raise ValueError(f"pitched input must be a contiguous CUDA int8 tensor of shape {(self.T, self.F, self.in_pitch)}")
+        if not (ok and tuple(x.shape) == self.in_shape()):
             raise ValueError(f"input must be a contiguous CUDA {dtype} tensor of shape {self.in_shape()}")
 
     def _chk_vis(self, v, dtype):
@@ -267,12 +313,12 @@ class Plan:
 
     def correlate_pipelined(self, blocks_host, dev_buf2, vis, compute_stream, copy_stream):
         """blocks_host: pinned CPU int8 tensor [n_blocks][T][F][N][2][2]; dev_buf2: CUDA int8 tensor of
-        2 * in_bytes; vis: CUDA int32.  Enqueues Algorithm 1 and returns; sync compute_stream."""
+        2 * scratch_in_bytes; vis: CUDA int32.  Enqueues Algorithm 1 and returns; sync compute_stream."""
         import torch
         if not (blocks_host.dtype == torch.int8 and blocks_host.is_contiguous() and not blocks_host.is_cuda
                 and tuple(blocks_host.shape[1:]) == self.in_shape()):
             raise ValueError("blocks_host must be a contiguous CPU int8 tensor [n_blocks][T][F][N][2][2]")
-        if dev_buf2.numel() * dev_buf2.element_size() < 2 * self.in_bytes:
+        if dev_buf2.numel() * dev_buf2.element_size() < 2 * self.scratch_in_bytes:
             raise ValueError("dev_buf2 too small")
         self._chk_vis(vis, torch.int32)
         self._check(lib().xc_correlate_pipelined(
@@ -289,7 +335,7 @@ class Plan:
         if not (blocks_host.dtype == torch.int8 and blocks_host.is_contiguous() and not blocks_host.is_cuda
                 and tuple(blocks_host.shape[1:]) == self.in_shape()):
             raise ValueError("blocks_host must be a contiguous CPU int8 tensor [n_blocks][T][F][N][2][2]")
-        if dev_buf2.numel() * dev_buf2.element_size() < 2 * self.in_bytes:
+        if dev_buf2.numel() * dev_buf2.element_size() < 2 * self.scratch_in_bytes:
             raise ValueError("dev_buf2 too small")
         self._chk_vis(vis32, torch.int32)
         self._chk_vis(vis64, torch.int64)
@@ -312,7 +358,10 @@ class Plan:
         return vis_host
 
     def correlate_host(self, x_host, vis_host, in_dev, vis_dev, stream=None):
-        """End to end with HOST buffers (H2D copy, X-engine, D2H copy, stream sync)."""
+        """End to end with HOST buffers (H2D copy, X-engine, D2H copy, stream sync).  in_dev: device scratch of at least
+        scratch_in_bytes (new_scratch())."""
+        if in_dev.numel() * in_dev.element_size() < self.scratch_in_bytes:
+            raise ValueError("in_dev scratch smaller than scratch_in_bytes")
         self._check(lib().xc_correlate_host(
             self._h, ctypes.c_void_p(x_host.data_ptr()), ctypes.c_void_p(vis_host.data_ptr()),
             ctypes.c_void_p(in_dev.data_ptr()), ctypes.c_void_p(vis_dev.data_ptr()), _stream_handle(stream)),

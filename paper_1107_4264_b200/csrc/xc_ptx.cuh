@@ -88,6 +88,45 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
     asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
 }
+// Release at cluster scope: this thread's (and, after __syncwarp, its warp's) earlier st.shared::cluster stores are
+// visible to whoever acquires the barrier's phase at cluster scope (T-split hand-over of partial accumulators).
+__device__ __forceinline__ void mbar_arrive_release_cluster(uint32_t cluster_bar) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+// mbar_wait with acquire semantics at cluster scope (pairs with mbar_arrive_release_cluster from another CTA).
+__device__ __forceinline__ void mbar_wait_acquire_cluster(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p, q;\n\t"
+        ".reg .u32 n;\n\t"
+        "mov.u32 n, 0;\n\t"
+        "XC_WAITC:\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra XC_DONEC;\n\t"
+        "add.u32 n, n, 1;\n\t"
+        "setp.gt.u32 q, n, %2;\n\t"
+        "@q trap;\n\t"
+        "bra XC_WAITC;\n\t"
+        "XC_DONEC:\n\t"
+        "}" ::"r"(bar),
+        "r"(parity), "n"(XC_SPIN_LIMIT)
+        : "memory");
+}
+// 16-byte store into the shared memory of another CTA of the cluster (address from mapa_u32)
+__device__ __forceinline__ void st_shared_cluster_v4(uint32_t cluster_addr, int4 v) {
+    asm volatile("st.shared::cluster.v4.s32 [%0], {%1, %2, %3, %4};" ::"r"(cluster_addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w)
+                 : "memory");
+}
+__device__ __forceinline__ int4 ld_shared_v4(uint32_t addr) {
+    int4 v;
+    asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 __device__ __forceinline__ uint32_t elect_one() {
     uint32_t pred;
     asm volatile(
@@ -128,29 +167,6 @@ __device__ __forceinline__ void tma_load_3d_2sm(uint32_t dst_smem, const CUtenso
         "%5}], [%2];" ::"r"(dst_smem),
         "l"(reinterpret_cast<uint64_t>(tmap)), "r"(cluster_bar), "r"(c0), "r"(c1), "r"(c2)
         : "memory");
-}
-
-// ---- bulk stores shared -> global (TMA store engine, no tensor map) ------------------------------
-// Generic-proxy writes to shared memory must be made visible to the async proxy before it reads them.
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void bulk_store(void* gdst, uint32_t ssrc, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(ssrc), "r"(bytes) : "memory");
-}
-// global[i] += shared[i] (int32), element-wise, performed in L2
-__device__ __forceinline__ void bulk_reduce_add_s32(void* gdst, uint32_t ssrc, uint32_t bytes) {
-    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.s32 [%0], [%1], %2;" ::"l"(gdst), "r"(ssrc),
-                 "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-// all bulk groups of this thread have finished READING shared memory (the source may be overwritten)
-__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
-__device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads) {
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-__device__ __forceinline__ void st_shared_v4(uint32_t addr, int4 v) {
-    asm volatile("st.shared.v4.s32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
 // ---- tcgen05 / TMEM -------------------------------------------------------------------------

@@ -17,6 +17,7 @@ constexpr int SIMT_B = 16;  // stations per block edge
 struct SimtParams {
     int N, F, T;
     long long NB;
+    long long pitch;      // bytes between consecutive (t, f) rows of `in`
     const int8_t* in;
     int32_t* vis;
     int accumulate;
@@ -42,7 +43,7 @@ __global__ void __launch_bounds__(SIMT_B* SIMT_B) xc_i8_simt_kernel(const SimtPa
     if (i > j || j >= p.N) return;  // super-diagonal threads exit
     int acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     for (int t = 0; t < p.T; ++t) {
-        const int8_t* x = p.in + (static_cast<long long>(t) * p.F + f) * p.N * 4;
+        const int8_t* x = p.in + (static_cast<long long>(t) * p.F + f) * p.pitch;
         int a[4], b[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
@@ -62,10 +63,11 @@ __global__ void __launch_bounds__(SIMT_B* SIMT_B) xc_i8_simt_kernel(const SimtPa
     for (int k = 0; k < 8; ++k) dst[k] = p.accumulate ? dst[k] + acc[k] : acc[k];
 }
 
-// (b) Staging: rows of 4N bytes -> rows of 4*Npad bytes (Npad = N rounded up to 4), zero padded,
-// written to a 128-byte-aligned workspace.  One thread per destination station (4 bytes).
+// (b) Staging: rows of 4N bytes, `pitch` bytes apart -> rows of 4*Npad bytes (the plan's 128-byte-multiple pitch), zero
+// padded, written to a 128-byte-aligned workspace.  One thread per destination station (4 bytes).  Needed only when the
+// input cannot be read by TMA in place: a base or row pitch that is not a multiple of 16 bytes (N % 4 != 0).
 __global__ void xc_stage_pad_kernel(const int8_t* __restrict__ in, uint32_t* __restrict__ out, long long rows, int N,
-                                    int Npad) {
+                                    long long pitch, int Npad) {
     const long long total = rows * Npad;
     for (long long k = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; k < total;
          k += static_cast<long long>(gridDim.x) * blockDim.x) {
@@ -73,7 +75,7 @@ __global__ void xc_stage_pad_kernel(const int8_t* __restrict__ in, uint32_t* __r
         const int s = static_cast<int>(k - r * Npad);
         uint32_t v = 0;
         if (s < N) {
-            const uint8_t* src = reinterpret_cast<const uint8_t*>(in) + (r * N + s) * 4;
+            const uint8_t* src = reinterpret_cast<const uint8_t*>(in) + r * pitch + s * 4;
             v = static_cast<uint32_t>(src[0]) | (static_cast<uint32_t>(src[1]) << 8) |
                 (static_cast<uint32_t>(src[2]) << 16) | (static_cast<uint32_t>(src[3]) << 24);
         }
@@ -81,16 +83,34 @@ __global__ void xc_stage_pad_kernel(const int8_t* __restrict__ in, uint32_t* __r
     }
 }
 
-// Same, 16 bytes (4 stations) per thread, for N % 4 == 0 and a 16-byte aligned input: only reached with
-// XC_OPT_FORCE_STAGE (a plain copy into the workspace, for testing S0 on aligned shapes).
+// Same, 16 bytes (4 stations) per thread, for N % 4 == 0, a 16-byte aligned input and a 16-byte-multiple pitch: only
+// reached with XC_OPT_FORCE_STAGE (a re-pitching copy into the workspace, for testing S0 on aligned shapes).
 __global__ void xc_stage_pad16_kernel(const uint4* __restrict__ in, uint4* __restrict__ out, long long rows, int n4,
-                                      int npad4) {
+                                      int pitch16, int npad4) {
     const long long total = rows * npad4;
     for (long long k = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; k < total;
          k += static_cast<long long>(gridDim.x) * blockDim.x) {
         const long long r = k / npad4;
         const int c = static_cast<int>(k - r * npad4);
-        out[k] = (c < n4) ? __ldcs(in + r * n4 + c) : make_uint4(0u, 0u, 0u, 0u);
+        out[k] = (c < n4) ? __ldcs(in + r * pitch16 + c) : make_uint4(0u, 0u, 0u, 0u);
+    }
+}
+
+// (b') Re-pitching for the host-buffer calls: the H2D copy lands dense rows (4N bytes: the copy engine moves dense blocks at
+// full PCIe rate, a pitched 2-D copy of 2000-byte rows measured 4x slower), and this pass spreads channels [f0, f0 + nf) of
+// every time sample to the plan's 128-byte-multiple pitch.  W bytes per thread: 16 when 4N is a multiple of 16, else 4.
+template <typename W>
+__global__ void xc_repitch_kernel(const W* __restrict__ in, W* __restrict__ out, int T, int F, int f0, int nf, int n_w,
+                                  long long out_pitch_w) {
+    const long long per_t = static_cast<long long>(nf) * n_w;
+    const long long total = per_t * T;
+    for (long long k = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; k < total;
+         k += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long t = k / per_t;
+        const long long rem = k - t * per_t;
+        const long long row = t * F + f0 + rem / n_w;
+        const long long c = rem % n_w;
+        out[row * out_pitch_w + c] = in[row * n_w + c];
     }
 }
 
@@ -124,24 +144,25 @@ __global__ void xc_unpack_i4_kernel(const uint8_t* __restrict__ in4, uint32_t* _
         out[r * Npad + s] = o0;
     }
 }
-// N % 8 == 0 and a 16-byte aligned input: 16 packed bytes (8 stations) -> 32 int8 per thread; n8 = N / 8
+// N % 8 == 0 and a 16-byte aligned input: 16 packed bytes (8 stations) -> 32 int8 per thread; n8 = N / 8, npad8 = Npad / 8
 __global__ void xc_unpack_i4x8_kernel(const uint4* __restrict__ in4, uint4* __restrict__ out, int T, int F, int f0, int nf,
-                                      int n8) {
+                                      int n8, int npad8) {
     const long long per_t = static_cast<long long>(nf) * n8;
     const long long total = per_t * T;
     for (long long k = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; k < total;
          k += static_cast<long long>(gridDim.x) * blockDim.x) {
         const long long t = k / per_t;
         const long long rem = k - t * per_t;
-        const long long idx = (t * F + f0 + rem / n8) * n8 + rem % n8;
-        const uint4 w = __ldcs(in4 + idx);
+        const long long row = t * F + f0 + rem / n8;
+        const long long c = rem % n8;
+        const uint4 w = __ldcs(in4 + row * n8 + c);
         uint4 a, b;
         unpack_i4_word(w.x, &a.x, &a.y);
         unpack_i4_word(w.y, &a.z, &a.w);
         unpack_i4_word(w.z, &b.x, &b.y);
         unpack_i4_word(w.w, &b.z, &b.w);
-        out[2 * idx] = a;
-        out[2 * idx + 1] = b;
+        out[2 * (row * npad8 + c)] = a;       // workspace rows are npad8 * 32 bytes apart (bytes beyond 4N are never read)
+        out[2 * (row * npad8 + c) + 1] = b;
     }
 }
 

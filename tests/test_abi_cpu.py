@@ -23,11 +23,18 @@ def _built():
 def test_exports_every_declared_symbol():
     hdr = open(os.path.join(ROOT, "include", "xc.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    # declarations inside #ifdef XC_PROFILE belong to the profiling build only
+    prof = "".join(re.findall(r"#ifdef XC_PROFILE(.*?)#endif", hdr, flags=re.S))
+    hdr = re.sub(r"#ifdef XC_PROFILE.*?#endif", "", hdr, flags=re.S)
     declared = set(re.findall(r"\b(xc_[a-z0-9_]+)\s*\(", hdr))
     assert declared == set(xcb.EXPORTED_SYMBOLS)
+    assert set(re.findall(r"\b(xc_[a-z0-9_]+)\s*\(", prof)) == set(xcb.PROFILE_SYMBOLS)
     L = ctypes.CDLL(xcb.binding.LIB_PATH)
     for name in declared:
         assert hasattr(L, name), name
+    for name in xcb.PROFILE_SYMBOLS:                        # the product build carries no profiling hooks
+        assert not hasattr(L, name), name
+    assert L.xc_set_option(xcb.Plan(8, 2, 16)._h, xcb.OPT_DEBUG_SKIP, 1) == -1
 
 
 def test_no_oracle_or_cpu_path_in_product():
@@ -49,6 +56,10 @@ def test_plan_argument_validation():
     assert L.xc_in_bytes_f32(h) == 16 * 16 * 4 * 256
     assert L.xc_n_baselines(h) == 136                      # BASELINE.json configs[0]
     assert L.xc_vis_bytes(h) == 32 * 136 * 4
+    assert L.xc_in_pitch(h) == 64 and L.xc_scratch_pitch(h) == 128 and L.xc_scratch_in_bytes(h) == (128 + 64) * 4 * 256 and L.xc_workspace_bytes(h) == 128 * 4 * 256
+    assert L.xc_set_in_pitch(h, 63) == -1 and L.xc_set_in_pitch(h, 256) == 0
+    assert L.xc_in_pitch(h) == 256 and L.xc_in_bytes(h) == 256 * 4 * 256
+    assert L.xc_set_in_pitch(h, 0) == 0 and L.xc_in_pitch(h) == 64
     L.xc_destroy(h)
     for args, code in [((0, 2, 4, 8, 0), -1), ((4, 2, 0, 8, 0), -1), ((4, 2, 4, 0, 0), -1),
                        ((4, 1, 4, 8, 0), -2), ((4, 2, 4, 8, 7), -2), ((4, 2, 4, 65536, 0), -3)]:
@@ -74,7 +85,7 @@ def test_compute_without_gpu_fails_loudly():
     assert rc in (-5, -2)
 
 
-@pytest.mark.parametrize("mode", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("mode", [0, 1, 3])
 @pytest.mark.parametrize("N", [1, 2, 3, 5, 16, 31, 32, 33, 64, 65, 100, 128, 129, 256, 500, 512, 1024])
 def test_tile_schedule_covers_triangle_exactly_once(N, mode):
     p = xcb.Plan(N, 1, 8)
@@ -99,12 +110,12 @@ def test_tile_schedule_covers_triangle_exactly_once(N, mode):
 
 def test_tile_counts_match_survey_table():
     """S1: nb(nb+1)/2 square 256x256 tiles per channel, nb = ceil(4N/256) -> 1, 3, 10, 36, 136
-    for N = 64 ... 1024 (CTA-pair tiles); 6 / 20 / 72 / 272 single-CTA 128x256 tiles."""
-    for N, n2, n1 in [(64, 1, 2), (128, 3, 6), (256, 10, 20), (512, 36, 72), (1024, 136, 272)]:
+    for N = 64 ... 1024 (CTA-pair tiles); the same formula with nb = ceil(4N/128) for single-CTA 128x128 tiles."""
+    for N, n2, n1 in [(64, 1, 3), (128, 3, 10), (256, 10, 36), (512, 36, 136), (1024, 136, 528)]:
         p = xcb.Plan(N, 1, 8)
         p.set_option(xcb.OPT_TILE, xcb.TILE_2CTA_256x256)
         assert len(p.tiles()) == n2
-        p.set_option(xcb.OPT_TILE, xcb.TILE_1CTA_128x256)
+        p.set_option(xcb.OPT_TILE, xcb.TILE_1CTA_128x128)
         assert len(p.tiles()) == n1
 
 
@@ -136,16 +147,16 @@ def test_option_validation():
     """xc_set_option rejects values outside each option's range and unknown options (no device needed)."""
     p = xcb.Plan(64, 4, 128)
     L, h = xcb.lib(), p._h
-    ok = [(xcb.OPT_I8_KERNEL, 2), (xcb.OPT_MAX_CTAS, 0), (xcb.OPT_MAX_CTAS, 37), (xcb.OPT_FORCE_STAGE, 1), (xcb.OPT_TILE, 5),
-          (xcb.OPT_TILE, 0), (xcb.OPT_EPILOGUE, 2), (xcb.OPT_BK, 256), (xcb.OPT_BK, 0), (xcb.OPT_PDL, 0), (xcb.OPT_PDL, 1)]
-    bad = [(xcb.OPT_I8_KERNEL, 3), (xcb.OPT_MAX_CTAS, -1), (xcb.OPT_TILE, 6), (xcb.OPT_TILE, -1), (xcb.OPT_EPILOGUE, 3),
-           (xcb.OPT_BK, 96), (99, 0)]
+    ok = [(xcb.OPT_I8_KERNEL, 2), (xcb.OPT_MAX_CTAS, 0), (xcb.OPT_MAX_CTAS, 37), (xcb.OPT_FORCE_STAGE, 1), (xcb.OPT_TILE, 3),
+          (xcb.OPT_TILE, 0), (xcb.OPT_TSPLIT, 2), (xcb.OPT_TSPLIT, 0), (xcb.OPT_PDL, 0), (xcb.OPT_PDL, 1)]
+    bad = [(xcb.OPT_I8_KERNEL, 3), (xcb.OPT_MAX_CTAS, -1), (xcb.OPT_TILE, 2), (xcb.OPT_TILE, 4), (xcb.OPT_TILE, -1),
+           (xcb.OPT_TSPLIT, 3), (5, 0), (6, 0), (99, 0)]   # 5 / 6: round 1's epilogue / stage-size options are gone
     for opt, val in ok:
         assert L.xc_set_option(h, opt, val) == 0, (opt, val)
     for opt, val in bad:
         assert L.xc_set_option(h, opt, val) == -1, (opt, val)
     assert L.xc_set_option(None, xcb.OPT_TILE, 0) == -1
     # every tile mode keeps an exact-cover schedule after switching back and forth
-    for mode in (5, 3, 4, 1, 0):
+    for mode in (3, 1, 0):
         p.set_option(xcb.OPT_TILE, mode)
         assert len(p.tiles()) >= 1
