@@ -414,7 +414,7 @@ def main():
 
     # ---- other denominators for "% of int8 tensor peak": measured cuBLAS int8 GEMM, nominal -----------
     denominators = {"bf16_burst_x2": i8_burst, "bf16_sustained_x2": i8_sustained, "nominal_dense_int8": NOMINAL_I8_TOPS}
-    if rank == 0:
+    if rank == 0 and not args.no_sweep:
         denominators.update(bench_legs.cublas_int8_peak(stream))
     roof["denominators_tops"] = denominators
     if denominators.get("cublas_int8_burst"):

@@ -80,7 +80,30 @@ def f32_leg(stream, clocks, F=None, launches=5):
     p3.close()
     del x3, v3
     torch.cuda.empty_cache()
+    if F is None:
+        out["fma_issue_probe"] = fma_probe()
     return out
+
+
+def fma_probe(iters=100000):
+    """Pure-register FFMA2 / FFMA streams (csrc/xc_probe.cu, built as libxc_probe.so): what the fp32 pipe delivers for the
+    kernel's operand pattern with no memory traffic at all -- the practical ceiling next to which the kernel's rate is read."""
+    import ctypes
+    from paper_1107_4264_b200 import build as xc_build
+    names = ["kernel statement order (ptxas schedule)", "scalar FFMA", "FFMA2, all operands re-used", "FFMA2 pair x pair",
+             "FFMA2 a-stationary (pinned)", "FFMA2 b-stationary (pinned)"]
+    try:
+        L = ctypes.CDLL(xc_build.build_probe())
+        L.xc_probe_fma.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+        res = {}
+        for mode, nm in enumerate(names):
+            o = (ctypes.c_double * 4)()
+            rc = L.xc_probe_fma(mode, iters, o)
+            res[nm] = {"rc": rc} if rc else {"ms": o[0], "fma_per_clk_per_sm": o[1], "sm_mhz": o[2], "tflops": o[3]}
+        res["how"] = "2 x 256 threads per SM, 64 accumulators per thread, no memory traffic; fma_per_clk_per_sm from the SM cycle counter (peak 128)"
+        return res
+    except Exception as e:  # noqa: BLE001
+        return {"unavailable": repr(e)}
 
 
 def only_leg(which, workload, stream):
@@ -207,4 +230,45 @@ def extras(stream, clocks, sampler, peaks):
 
     # ---- F-engine + corner turn, and the FX chain ----------------------------------------------------------
     out["fx"] = fengine_leg(stream, "cfg3")
+    return out
+
+
+def _fx_leg(stream, workload, launches, with_fx):
+    """F-engine (+ FX chain) on the shape of `workload`: volt int8 [N][2][T*F][2] -> cube -> vis.  Roofline: the F-engine
+    moves 4NFT bytes in and 4NFT bytes out (algorithmic; HBM) and needs about 5 F log2 F real operations per spectrum on
+    the fp32 CUDA cores (non-FMA: 128 lanes / clk / SM) -- whichever takes longer bounds it."""
+    import numpy as np
+    import torch
+    import paper_1107_4264_b200 as xcb
+    import xc_workloads as wl
+    from bench import load_peaks
+    w = wl.CONFIGS[workload]
+    N, F, T = w.N, w.F, w.T
+    volt = torch.from_numpy(wl.voltages(N, F, T, seed=w.seed + 500)).cuda()
+    scale = wl.fengine_scale(F)
+    p = xcb.Plan(N, F, T)
+    cube = p.new_cube()
+    ms = _timed(lambda: p.fengine(volt, scale, cube, stream=stream), stream, launches)
+    peaks = load_peaks()
+    alg_bytes = 8.0 * N * F * T
+    flops = 5.0 * F * max(np.log2(F), 1.0) * 2 * N * T
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    alu_peak = sms * 128 * 1965e6 / 1e12                     # T non-FMA fp32 operations / s at clocks.max.sm
+    t_hbm, t_alu = alg_bytes / (peaks["hbm_gbs"] * 1e9), flops / (alu_peak * 1e12)
+    gbs = alg_bytes / (ms * 1e-3) / 1e9
+    out = {"workload": f"{workload} shape: N={N}, F={F}-point transforms, T={T} time blocks, int8 complex voltages (Gaussian sigma 16 + 2 tones)",
+           "fengine_ms": ms, "bound": "hbm" if t_hbm >= t_alu else "alu", "achieved_gbs": gbs, "hbm_peak_gbs": peaks["hbm_gbs"],
+           "frac_hbm": gbs / peaks["hbm_gbs"], "algorithmic_bytes": alg_bytes, "fft_flops_5NlogN": flops,
+           "achieved_tflops": flops / (ms * 1e-3) / 1e12, "alu_peak_tops_non_fma": alu_peak,
+           "frac_alu": flops / (ms * 1e-3) / 1e12 / alu_peak, "roof_ms": 1e3 * max(t_hbm, t_alu)}
+    if with_fx:
+        vis = p.new_vis()
+        ms_fx = _timed(lambda: p.fx(volt, scale, cube, vis, stream=stream), stream, launches)
+        p.set_in_pitch(p.scratch_pitch)
+        ms_x = _timed(lambda: p.correlate(cube, vis, stream=stream), stream, launches)
+        out.update({"fx_ms": ms_fx, "xengine_alone_ms": ms_x, "fx_tops": w.ops / (ms_fx * 1e-3) / 1e12,
+                    "launches_per_fx": 2})
+    p.close()
+    del volt, cube
+    torch.cuda.empty_cache()
     return out

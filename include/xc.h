@@ -94,8 +94,8 @@ typedef enum {
     XC_OPT_PDL = 7,        /* 1 (default) = launch the tensor-core kernels with programmatic stream            */
                            /* serialization: the prologue overlaps the previous kernel's tail; 0 = plain launch */
     XC_OPT_TSPLIT = 8      /* T-split of the single-CTA tile over a cluster of 2 (the paper's small-N future    */
-                           /* work): 0 = auto (on when 2 * tiles * F <= SM count), 1 = off,   */
-                           /* 2 = on whenever T allows it.  Results are identical either way.                   */
+                           /* work): 0 = auto (on when 2 * tiles * F <= SM count and T >= 8192: */
+                           /* the hand-over costs ~3 us), 1 = off, 2 = on whenever T allows it.  Same bits either way. */
 #ifdef XC_PROFILE
     , XC_OPT_DEBUG_SKIP = 3 /* PROFILING BUILD ONLY (-DXC_PROFILE), results become meaningless: bit 0 = no TMA */
                             /* loads after the first ring fill, bit 1 = no MMAs, bit 2 = no stores, bit 3 =    */
@@ -232,6 +232,33 @@ int xc_correlate_host(xc_plan_t* plan, const int8_t* in_host, int32_t* vis_host,
  *   xc_in_bytes_i4() bytes; half the host->device bytes of the int8 call, same result cube. */
 int xc_correlate_host_i4(xc_plan_t* plan, const uint8_t* in4_host, int32_t* vis_host, uint8_t* in4_dev_scratch,
                          int32_t* vis_dev_scratch, void* cuda_stream);
+
+/* ---- F-engine + corner turn in front of the X-engine ("the next step is to develop
+ * this into a full FX correlator") ------------------------------------------------------------------------------------
+ * xc_fengine -- for every station s, polarisation p and time block t < T the F-point Fourier transform
+ *        X[t][f][s][p] = sum_{k<F} volt[s][p][t*F + k] * exp(-2 pi i f k / F)       ("X_i(nu) = int A_i(tau)
+ *   e^{-i 2 pi nu tau}"; "N (fast) Fourier transforms of length F ... once every F samples"),
+ *   quantised to int8 as q = clip(rint(X * scale), -127, 127) per real component (round-half-even, decided in fp32;
+ *   four to eight bits suffice) and written in the X-engine's input order [t][f][station][pol][re,im]
+ *    -- the corner turn is this kernel's store pattern.
+ *   volt_dev: int8 [N][2 pol][T*F samples][2 re,im], station-major time series (2-byte aligned); xc_volt_bytes().
+ *   cube_dev: int8 rows (t, f) of 4N valid bytes, cube_pitch bytes apart (a multiple of 4, >= 4N; 0 = xc_scratch_pitch(),
+ *   the 128-byte multiple the X-engine reads fastest; xc_cube_bytes() is the size at that pitch); 4-byte aligned.
+ *   F must be a power of two <= 4096, else XC_ERR_UNSUPPORTED.  fp32 arithmetic (Stockham FFT, radix <= 16): the
+ *   spectrum agrees with an fp64 DFT to about 1e-6 relative to sqrt(F) * max|volt|, so a quantised sample can differ by one
+ *   step from an exact evaluation only where X * scale lies within that distance of a rounding boundary k + 1/2; the
+ *   bins f = 0, F/4, F/2, 3F/4 of integer input are exact, ties included.
+ * xc_fengine_f32 -- the same spectra unquantised and unscaled, float [T][F][N][2][2] (dense; 8-byte aligned): for checking
+ *   the transform itself against an fp64 DFT.  Strided stores: a testing aid, not a fast path.
+ * xc_fx -- the FX correlator: xc_fengine into cube_scratch_dev (xc_cube_bytes(), 16-byte aligned, pitch
+ *   xc_scratch_pitch()), then the X-engine on it: vis (+)= sum_t X X^H.  Two launches on the caller's stream; the
+ *   X-engine's prologue overlaps the F-engine's tail (programmatic dependent launch). */
+size_t xc_volt_bytes(const xc_plan_t* plan);   /* 4*N*F*T */
+size_t xc_cube_bytes(const xc_plan_t* plan);   /* xc_scratch_pitch()*F*T */
+int xc_fengine(xc_plan_t* plan, const int8_t* volt_dev, float scale, int8_t* cube_dev, size_t cube_pitch, void* cuda_stream);
+int xc_fengine_f32(xc_plan_t* plan, const int8_t* volt_dev, float* spec_dev, void* cuda_stream);
+int xc_fx(xc_plan_t* plan, const int8_t* volt_dev, float scale, int8_t* cube_scratch_dev, int32_t* vis_dev, int accumulate,
+          void* cuda_stream);
 
 #ifdef XC_PROFILE
 /* PROFILING BUILD ONLY (-DXC_PROFILE; libxc_profile.so): trace_dev = device buffer of 3*256*4 int64 (or NULL to switch

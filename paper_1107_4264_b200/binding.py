@@ -26,6 +26,7 @@ EXPORTED_SYMBOLS = (
     "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_integrate",
     "xc_correlate_i4", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get", "xc_t_split",
     "xc_set_in_pitch", "xc_in_pitch", "xc_scratch_pitch", "xc_scratch_in_bytes", "xc_set_timing_buffer",
+    "xc_volt_bytes", "xc_cube_bytes", "xc_fengine", "xc_fengine_f32", "xc_fx",
     "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error", "xc_version",
 )
 # additionally exported by the profiling build only (libxc_profile.so, -DXC_PROFILE)
@@ -73,6 +74,10 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_scratch_pitch": (sz, [p]), "xc_scratch_in_bytes": (sz, [p]),
         "xc_set_timing_buffer": (i, [p, p]),
         "xc_t_split": (i, [p]),
+        "xc_volt_bytes": (sz, [p]), "xc_cube_bytes": (sz, [p]),
+        "xc_fengine": (i, [p, p, ctypes.c_float, p, sz, p]),
+        "xc_fengine_f32": (i, [p, p, p, p]),
+        "xc_fx": (i, [p, p, ctypes.c_float, p, p, i, p]),
         "xc_tile_count": (i, [p]),
         "xc_tile_get": (i, [p, i, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i)]),
         "xc_tri_index": (i64, [i64, i64]),
@@ -348,6 +353,59 @@ class Plan:
             ctypes.c_void_p(vis64_host.data_ptr() if vis64_host is not None else 0),
             ctypes.c_void_p(compute_stream.cuda_stream), ctypes.c_void_p(copy_stream.cuda_stream)), "xc_integrate")
         return vis64
+
+    # F-engine + FX chain ---------------------------------------------------------------------
+    def volt_shape(self):
+        return (self.N, 2, self.T * self.F, 2)
+
+    def _chk_volt(self, volt):
+        import torch
+        if not (isinstance(volt, torch.Tensor) and volt.is_cuda and volt.dtype == torch.int8 and volt.is_contiguous()
+                and tuple(volt.shape) == self.volt_shape()):
+            raise ValueError(f"volt must be a contiguous CUDA int8 tensor of shape {self.volt_shape()}")
+
+    def new_cube(self, device="cuda"):
+        """int8 [T][F][scratch_pitch]: the F-engine's output / the X-engine's pitched input."""
+        import torch
+        return torch.empty((self.T, self.F, self.scratch_pitch), dtype=torch.int8, device=device)
+
+    def fengine(self, volt, scale: float, cube=None, stream=None):
+        """cube = quantise(FFT_F(volt) * scale) in the X-engine's order.  cube: int8 CUDA [T][F][pitch] (pitch % 4 == 0,
+        >= 4N; default new_cube()).  Returns the cube."""
+        self._chk_volt(volt)
+        if cube is None:
+            cube = self.new_cube(volt.device)
+        if not (cube.is_cuda and cube.is_contiguous() and cube.dim() == 3 and tuple(cube.shape[:2]) == (self.T, self.F)
+                and cube.element_size() == 1):
+            raise ValueError("cube must be a contiguous CUDA int8 tensor [T][F][pitch]")
+        self._check(lib().xc_fengine(self._h, ctypes.c_void_p(volt.data_ptr()), ctypes.c_float(scale),
+                                     ctypes.c_void_p(cube.data_ptr()), int(cube.shape[2]), _stream_handle(stream)), "xc_fengine")
+        return cube
+
+    def fengine_f32(self, volt, spec=None, stream=None):
+        """Unquantised fp32 spectra, float CUDA [T][F][N][2][2]."""
+        import torch
+        self._chk_volt(volt)
+        if spec is None:
+            spec = torch.empty(self.in_shape(), dtype=torch.float32, device=volt.device)
+        self._chk_in(spec, torch.float32)
+        self._check(lib().xc_fengine_f32(self._h, ctypes.c_void_p(volt.data_ptr()), ctypes.c_void_p(spec.data_ptr()),
+                                         _stream_handle(stream)), "xc_fengine_f32")
+        return spec
+
+    def fx(self, volt, scale: float, cube_scratch, vis=None, accumulate=False, stream=None):
+        """vis (+)= X-engine(F-engine(volt)).  cube_scratch: new_cube()."""
+        import torch
+        self._chk_volt(volt)
+        if tuple(cube_scratch.shape) != (self.T, self.F, self.scratch_pitch) or not cube_scratch.is_contiguous():
+            raise ValueError("cube_scratch must be new_cube()")
+        if vis is None:
+            vis = self.new_vis(torch.int32, volt.device)
+        self._chk_vis(vis, torch.int32)
+        self._check(lib().xc_fx(self._h, ctypes.c_void_p(volt.data_ptr()), ctypes.c_float(scale),
+                                ctypes.c_void_p(cube_scratch.data_ptr()), ctypes.c_void_p(vis.data_ptr()),
+                                1 if accumulate else 0, _stream_handle(stream)), "xc_fx")
+        return vis
 
     def correlate_host_i4(self, x4_host, vis_host, in4_dev, vis_dev, stream=None):
         """End to end with HOST buffers for 4-bit samples (uint8 [T][F][N][2])."""

@@ -15,6 +15,7 @@
 #include <vector>
 
 #include "xc_f32.cuh"
+#include "xc_fengine.cuh"
 #include "xc_i8_tc.cuh"
 #include "xc_simt.cuh"
 
@@ -55,6 +56,8 @@ struct xc_plan_s {
     int device = -1, sm_count = 0;
     uint32_t* d_tiles_tc = nullptr;
     uint32_t* d_tiles_f32 = nullptr;
+    float2* d_twiddle = nullptr;                         // F-engine: exp(-2 pi i m / F), m < F (F a power of two <= 4096)
+    int logf = -1;                                       // log2 F, or -1 when the F-engine cannot serve this F
     PFN_encodeTiled encode = nullptr;
     void* ws = nullptr;
     size_t ws_bytes = 0;
@@ -96,15 +99,19 @@ void tile_shape(int mode, int* si, int* sj) {
     *si = *sj = (mode == XC_TILE_2CTA_256x256) ? 64 : 32;
 }
 
-// T-split (single-CTA tile only): two CTAs of a cluster share one tile's time axis when that leaves no SM without
-// work it could have had, i.e. when even the doubled unit count fits the machine in one wave.  Each rank needs at
-// least one sample; a share is a whole multiple of the MMA's K = 32.
+// T-split (single-CTA tile only): two CTAs of a cluster share one tile's time axis.  Worth it when (a) it leaves no SM
+// without work it could have had, i.e. even the doubled unit count fits the machine in one wave, and (b) the tensor work
+// it takes off the critical path -- T tensor-core cycles, half of a 128 x 128 tile's 2T -- exceeds what the cluster launch,
+// the DSMEM hand-over of 64 KB of partial sums and its release/acquire pair cost: measured ~3.3 us ~ 6000 cycles
+// (N = 32, F = 64: 7.0 us with the split against 5.0 us without at T = 2048), hence T >= 8192.
+// Each rank needs at least one sample; a share is a whole multiple of the MMA's K = 32.
+constexpr int kTSplitMinT = 8192;
 int pick_t_split(const xc_plan_t* p, int nf, int sms) {
     if (p->tile_mode != XC_TILE_1CTA_128x128 || p->opt_tsplit == 1) return 1;
     const int share = ((p->T + 1) / 2 + 31) & ~31;
     if (share >= p->T) return 1;
     if (p->opt_tsplit == 2) return 2;
-    return (static_cast<long long>(p->tiles_tc.size()) * nf * 2 <= sms) ? 2 : 1;
+    return (p->T >= kTSplitMinT && static_cast<long long>(p->tiles_tc.size()) * nf * 2 <= sms) ? 2 : 1;
 }
 
 // S1: pick the tensor-core tile and build its per-channel schedule.
@@ -181,6 +188,107 @@ cudaError_t opt_in_smem() {
                                 xc::TcCfg<UMMA_N, CG, BK, TS>::SMEM_BYTES);
 }
 
+// ---- F-engine host side --------------------------------------------------------------------------------
+// exp(-2 pi i m / F) in fp64, then rounded to fp32.  The angle is folded into the first eighth of a turn so that the table
+// is exact at quarter turns (0, +-1) and symmetric at odd eighth turns: integer-valued voltages then give exactly integer
+// spectra in the bins 0, F/4, F/2, 3F/4, whatever the ties of the quantiser are.
+void fe_twiddle(int F, int m, float* re, float* im) {
+    const double kTwoPi = 6.283185307179586476925286766559;
+    int e = static_cast<int>((8LL * m) / F);                     // eighth of the turn, 0..7
+    long long rem = 8LL * m - static_cast<long long>(e) * F;     // in units of 1/(8F) turn, 0 <= rem < F
+    bool mirror = (e & 1) != 0;                                  // odd eighths are reflected: angle = (e + 1) / 8 turn - theta
+    if (mirror) rem = F - rem;
+    const double theta = kTwoPi * static_cast<double>(rem) / (8.0 * static_cast<double>(F));
+    double c = std::cos(theta), s = std::sin(theta);
+    if (rem == 0) { c = 1.0; s = 0.0; }
+    if (rem == F) { c = s = std::sqrt(0.5); }
+    if (mirror) s = -s;
+    const int quarter = ((e + (mirror ? 1 : 0)) / 2) & 3;        // quarter turns to add, exactly
+    double cc = c, ss = s;
+    if (quarter == 1) { cc = -s; ss = c; }
+    else if (quarter == 2) { cc = -c; ss = -s; }
+    else if (quarter == 3) { cc = s; ss = -c; }
+    *re = static_cast<float>(cc);
+    *im = static_cast<float>(-ss);
+}
+
+template <int LOGF>
+cudaError_t fe_opt_in() {
+    return cudaFuncSetAttribute(xc::xc_fengine_kernel<LOGF>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+}
+template <int LOGF>
+void fe_launch_one(const xc::FeParams& fp, unsigned grid, size_t smem, cudaStream_t st) {
+    xc::xc_fengine_kernel<LOGF><<<grid, xc::FE_THREADS, smem, st>>>(fp);
+}
+template <int LOGF>
+size_t fe_extra_smem() { return xc::FeCfg<LOGF>::WORK_BYTES + xc::FeCfg<LOGF>::TW_BYTES; }
+
+#define XC_FE_FOR_ALL(X) X(0) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12)
+
+int fe_prepare(xc_plan_t* p) {
+    p->logf = -1;
+    for (int l = 0; l <= xc::FE_MAX_LOGF; ++l)
+        if ((1 << l) == p->F) p->logf = l;
+    if (p->logf < 0) return XC_OK;            // the F-engine calls will answer XC_ERR_UNSUPPORTED
+    std::vector<float2> tw(p->F);
+    for (int m = 0; m < p->F; ++m) fe_twiddle(p->F, m, &tw[m].x, &tw[m].y);
+    if (!p->d_twiddle) XC_CUDA(p, cudaMalloc(&p->d_twiddle, sizeof(float2) * p->F));
+    XC_CUDA(p, cudaMemcpy(p->d_twiddle, tw.data(), sizeof(float2) * p->F, cudaMemcpyHostToDevice));
+    switch (p->logf) {
+#define X(L) case L: XC_CUDA(p, fe_opt_in<L>()); break;
+        XC_FE_FOR_ALL(X)
+#undef X
+        default: break;
+    }
+    return XC_OK;
+}
+
+int ensure_device(xc_plan_t* p);
+
+// volt -> cube (quantised, rows `pitch` bytes apart) and / or spec (fp32, dense cube order)
+int fengine_launch(xc_plan_t* p, const int8_t* volt, float scale, int8_t* cube, size_t pitch, float* spec, cudaStream_t st) {
+    if (!p || !volt || (!cube && !spec)) return XC_ERR_INVALID_ARG;
+    int rc = ensure_device(p);
+    if (rc != XC_OK) return rc;
+    if (p->logf < 0) {
+        p->last_err = "the F-engine needs F to be a power of two <= 4096";
+        return XC_ERR_UNSUPPORTED;
+    }
+    if ((reinterpret_cast<uintptr_t>(volt) & 1u) || (reinterpret_cast<uintptr_t>(cube) & 3u) || (reinterpret_cast<uintptr_t>(spec) & 7u))
+        return XC_ERR_ALIGNMENT;
+    if (cube && (pitch < static_cast<size_t>(4) * p->N || (pitch & 3u))) return XC_ERR_INVALID_ARG;
+    // stations per CTA: 32 (128-byte rows) while the tile of one time block fits, else 16 or 8; never more than N needs
+    int SB = 32;
+    while (SB > 8 && (static_cast<long long>(SB) * 4 * p->F > xc::FE_TILE_BYTES || SB / 2 >= p->N)) SB /= 2;
+    long long TT = xc::FE_TILE_BYTES / (static_cast<long long>(SB) * 4 * p->F);
+    if (TT < 1) TT = 1;
+    if (TT > p->T) TT = p->T;
+    xc::FeParams fp;
+    fp.N = p->N;
+    fp.T = p->T;
+    fp.SB = SB;
+    fp.TT = static_cast<int>(TT);
+    fp.nsb = (p->N + SB - 1) / SB;
+    fp.pitch = static_cast<long long>(pitch);
+    fp.volt = volt;
+    fp.cube = cube;
+    fp.spec = spec;
+    fp.tw = p->d_twiddle;
+    fp.scale = scale;
+    const long long grid = static_cast<long long>(fp.nsb) * ((p->T + TT - 1) / TT);
+    if (grid > 0x7FFFFFFFLL) return XC_ERR_UNSUPPORTED;
+    const size_t tile = (static_cast<size_t>(SB) * 4 * p->F * TT + 15) & ~static_cast<size_t>(15);
+    switch (p->logf) {
+#define X(L) case L: fe_launch_one<L>(fp, static_cast<unsigned>(grid), tile + fe_extra_smem<L>(), st); break;
+        XC_FE_FOR_ALL(X)
+#undef X
+        default: return XC_ERR_UNSUPPORTED;
+    }
+    XC_CUDA(p, cudaGetLastError());
+    p->last_launches = 1;
+    return XC_OK;
+}
+
 int ensure_device(xc_plan_t* p) {
     int dev = 0;
     XC_CUDA(p, cudaGetDevice(&dev));
@@ -224,6 +332,8 @@ int ensure_device(xc_plan_t* p) {
     XC_CUDA(p, (opt_in_smem<256, 2, 128, 1>()));
     XC_CUDA(p, (opt_in_smem<128, 1, 256, 1>()));
     XC_CUDA(p, (opt_in_smem<128, 1, 256, 2>()));
+    int rc_fe = fe_prepare(p);
+    if (rc_fe != XC_OK) return rc_fe;
     p->dev_ready = true;
     return XC_OK;
 }
@@ -418,6 +528,7 @@ void xc_destroy(xc_plan_t* p) {
     if (!p) return;
     if (p->d_tiles_tc) cudaFree(p->d_tiles_tc);
     if (p->d_tiles_f32) cudaFree(p->d_tiles_f32);
+    if (p->d_twiddle) cudaFree(p->d_twiddle);
     if (p->ws && p->ws_owned) cudaFree(p->ws);
     for (int k = 0; k < 2; ++k) {
         if (p->ev_copied[k]) cudaEventDestroy(p->ev_copied[k]);
@@ -440,7 +551,7 @@ size_t xc_n_baselines(const xc_plan_t* p) { return p ? static_cast<size_t>(p->NB
 size_t xc_scratch_pitch(const xc_plan_t* p) { return p ? p->pad_pitch : 0; }
 size_t xc_scratch_in_bytes(const xc_plan_t* p) {
     if (!p) return 0;
-    const size_t dense = static_cast<size_t>(4) * p->N * p->F * p->T;
+    const size_t dense = (static_cast<size_t>(4) * p->N * p->F * p->T + 127) & ~static_cast<size_t>(127);   // halves of dev_buf2 stay aligned
     return p->pad_pitch * p->F * p->T + (p->pad_pitch == static_cast<size_t>(4) * p->N ? 0 : dense);
 }
 size_t xc_workspace_bytes(const xc_plan_t* p) { return p ? p->pad_pitch * p->F * p->T : 0; }
@@ -748,6 +859,31 @@ int xc_debug_set_trace(xc_plan_t* p, void* trace_dev) {
     return XC_OK;
 }
 #endif
+
+size_t xc_volt_bytes(const xc_plan_t* p) { return p ? static_cast<size_t>(4) * p->N * p->F * p->T : 0; }
+size_t xc_cube_bytes(const xc_plan_t* p) { return p ? p->pad_pitch * p->F * p->T : 0; }
+
+int xc_fengine(xc_plan_t* p, const int8_t* volt_dev, float scale, int8_t* cube_dev, size_t cube_pitch, void* stream) {
+    if (!p || !cube_dev) return XC_ERR_INVALID_ARG;
+    return fengine_launch(p, volt_dev, scale, cube_dev, cube_pitch ? cube_pitch : p->pad_pitch, nullptr,
+                          static_cast<cudaStream_t>(stream));
+}
+
+int xc_fengine_f32(xc_plan_t* p, const int8_t* volt_dev, float* spec_dev, void* stream) {
+    if (!p || !spec_dev) return XC_ERR_INVALID_ARG;
+    return fengine_launch(p, volt_dev, 1.0f, nullptr, 0, spec_dev, static_cast<cudaStream_t>(stream));
+}
+
+int xc_fx(xc_plan_t* p, const int8_t* volt_dev, float scale, int8_t* cube_scratch_dev, int32_t* vis_dev, int accumulate,
+          void* stream) {
+    if (!p || !cube_scratch_dev || !vis_dev) return XC_ERR_INVALID_ARG;
+    if (reinterpret_cast<uintptr_t>(cube_scratch_dev) & 15u) return XC_ERR_ALIGNMENT;
+    int rc = fengine_launch(p, volt_dev, scale, cube_scratch_dev, p->pad_pitch, nullptr, static_cast<cudaStream_t>(stream));
+    if (rc != XC_OK) return rc;
+    rc = correlate_i8(p, cube_scratch_dev, vis_dev, stream, accumulate ? 1 : 0, 0, -1, 0, p->pad_pitch);
+    if (rc == XC_OK) p->last_launches += 1;
+    return rc;
+}
 
 int xc_tile_count(const xc_plan_t* p) { return p ? static_cast<int>(p->tiles_tc.size()) : 0; }
 

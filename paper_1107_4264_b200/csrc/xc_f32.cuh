@@ -12,7 +12,10 @@
 // owns a 16 x 16-station block and skips the arithmetic when the whole block is above the diagonal,
 // which cuts the paper's wasted work from 32 x 64 to 16 x 16 granularity.
 // Measured variants (B200, config 3 values): stages of 8 / 16 / 32 samples x 2-4 stages and 1 vs 2
-// blocks per SM -- 16 x 3 x 2 is the fastest.
+// blocks per SM -- 16 x 3 x 2 is the fastest.  Round 2 also measured a ring synchronised by per-stage full / empty
+// mbarriers (cp.async.mbarrier.arrive.noinc, refill lagging two iterations) in place of the block-wide barrier per stage,
+// because ncu attributes 17 % of the warp cycles to that barrier: 11.3-11.8 ms against 10.7 ms -- the waiting only moves
+// to the mbarriers (the FMA pipe, not the barrier, is what the warps queue for), so the simple ring stays.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -55,30 +58,38 @@ __device__ __forceinline__ void cp_async_wait() {
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-// Packed fp32 FMA (sm_100 FFMA2): d.lo = a.lo * b.lo + c.lo, d.hi = a.hi * b.hi + c.hi, each rounded once like
-// fmaf.  The SASS instruction takes a scalar-broadcast, a half-swap and per-half negation as operand modifiers, so
-// the (re, im) pair algebra below costs no extra instructions (checked with cuobjdump: FFMA2 ... .F32x2.LO_HI.NP).
-__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {
+// One station i (a = both polarisations) against the thread's four stations j: 32 packed FMAs = 64 of the paper's FMAs
+// (16 per station pair).  acc[n][pi*2+pj] = (re, im) += a_{pi} * conj(b_{n,pj}); per output the order is
+//     re = fma(a.im, b.im, fma(a.re, b.re, re)),  im = fma(-a.re, b.im, fma(a.im, b.re, im)),
+// i.e. (re, im) += (a.re, a.im) * b.re, then (re, im) += (a.im, -a.re) * b.im.
+// The statement order is pinned (asm volatile) and "a-stationary": eight consecutive FFMA2 share their 64-bit a operand
+// and differ in the scalar b and the accumulator.  A pure-register probe of this operand pattern (csrc/xc_probe.cu, bench.py
+// extras.f32.fma_issue_probe) measured 66.3 TFLOPS for this order against 58.1 for the order ptxas picks by itself and 61.4
+// for the b-stationary one: the instruction reads 5 register words (2 + 1 + 2) per two pipe cycles, and holding the pair
+// operand in the re-use latch is what fits the register-file bandwidth.
+__device__ __forceinline__ float2 ffma2_pinned(float2 a, float bs, float2 c) {
     unsigned long long ua, ub, uc, ud;
     asm("mov.b64 %0, {%1, %2};" : "=l"(ua) : "f"(a.x), "f"(a.y));
-    asm("mov.b64 %0, {%1, %2};" : "=l"(ub) : "f"(b.x), "f"(b.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ub) : "f"(bs), "f"(bs));
     asm("mov.b64 %0, {%1, %2};" : "=l"(uc) : "f"(c.x), "f"(c.y));
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(ud) : "l"(ua), "l"(ub), "l"(uc));
+    asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(ud) : "l"(ua), "l"(ub), "l"(uc));
     float2 d;
     asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(ud));
     return d;
 }
-
-// acc[pi*2+pj] = (re, im) += a_{pi} * conj(b_{pj}): 16 FMAs as 8 packed ones.  Per output the order
-// is  re = fma(a.im, b.im, fma(a.re, b.re, re)),  im = fma(-a.re, b.im, fma(a.im, b.re, im)).
-__device__ __forceinline__ void cmac4(float2 (&acc)[4], const float4& a, const float4& b) {
-    // pi = 0: (a.x, a.y); pi = 1: (a.z, a.w); pj = 0: (b.x, b.y); pj = 1: (b.z, b.w)
-    const float2 a0 = make_float2(a.x, a.y), a0s = make_float2(a.y, -a.x);
-    const float2 a1 = make_float2(a.z, a.w), a1s = make_float2(a.w, -a.z);
-    acc[0] = ffma2(a0, make_float2(b.x, b.x), acc[0]); acc[0] = ffma2(a0s, make_float2(b.y, b.y), acc[0]);
-    acc[1] = ffma2(a0, make_float2(b.z, b.z), acc[1]); acc[1] = ffma2(a0s, make_float2(b.w, b.w), acc[1]);
-    acc[2] = ffma2(a1, make_float2(b.x, b.x), acc[2]); acc[2] = ffma2(a1s, make_float2(b.y, b.y), acc[2]);
-    acc[3] = ffma2(a1, make_float2(b.z, b.z), acc[3]); acc[3] = ffma2(a1s, make_float2(b.w, b.w), acc[3]);
+__device__ __forceinline__ void cmac_row(float2 (&acc)[4][4], const float4& a, const float4& b0, const float4& b1,
+                                         const float4& b2, const float4& b3) {
+    const float bre[8] = {b0.x, b0.z, b1.x, b1.z, b2.x, b2.z, b3.x, b3.z};      // b_{n,pj}.re, index 2n + pj
+    const float bim[8] = {b0.y, b0.w, b1.y, b1.w, b2.y, b2.w, b3.y, b3.w};
+#pragma unroll
+    for (int pi = 0; pi < 2; ++pi) {
+        const float2 ap = pi ? make_float2(a.z, a.w) : make_float2(a.x, a.y);
+        const float2 as = pi ? make_float2(a.w, -a.z) : make_float2(a.y, -a.x);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc[k >> 1][pi * 2 + (k & 1)] = ffma2_pinned(ap, bre[k], acc[k >> 1][pi * 2 + (k & 1)]);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc[k >> 1][pi * 2 + (k & 1)] = ffma2_pinned(as, bim[k], acc[k >> 1][pi * 2 + (k & 1)]);
+    }
 }
 
 __global__ void __launch_bounds__(F32_THREADS, XC_F32_MINB) xc_f32_kernel(const F32Params p) {
@@ -148,8 +159,8 @@ __global__ void __launch_bounds__(F32_THREADS, XC_F32_MINB) xc_f32_kernel(const 
             const float4 a0 = row[ti], a1 = row[ti + 8];
             const float4 b0 = row[F32_SI + tj], b1 = row[F32_SI + tj + 4];
             const float4 b2 = row[F32_SI + tj + 8], b3 = row[F32_SI + tj + 12];
-            cmac4(acc[0][0], a0, b0); cmac4(acc[0][1], a0, b1); cmac4(acc[0][2], a0, b2); cmac4(acc[0][3], a0, b3);
-            cmac4(acc[1][0], a1, b0); cmac4(acc[1][1], a1, b1); cmac4(acc[1][2], a1, b2); cmac4(acc[1][3], a1, b3);
+            cmac_row(acc[0], a0, b0, b1, b2, b3);
+            cmac_row(acc[1], a1, b0, b1, b2, b3);
         }
     }
     cp_async_wait<0>();
