@@ -214,14 +214,16 @@ void fe_twiddle(int F, int m, float* re, float* im) {
 
 template <int LOGF>
 cudaError_t fe_opt_in() {
-    return cudaFuncSetAttribute(xc::xc_fengine_kernel<LOGF>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(xc::xc_fengine_kernel<LOGF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(xc::xc_fengine_kernel<LOGF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
 }
 template <int LOGF>
-void fe_launch_one(const xc::FeParams& fp, unsigned grid, size_t smem, cudaStream_t st) {
-    xc::xc_fengine_kernel<LOGF><<<grid, xc::FE_THREADS, smem, st>>>(fp);
+void fe_launch_one(const xc::FeParams& fp, unsigned grid, size_t tile, cudaStream_t st) {
+    const size_t extra = xc::FeCfg<LOGF>::WORK_BYTES + xc::FeCfg<LOGF>::TW_BYTES;
+    if (fp.spec) xc::xc_fengine_kernel<LOGF, true><<<grid, xc::FE_THREADS, extra, st>>>(fp);
+    else xc::xc_fengine_kernel<LOGF, false><<<grid, xc::FE_THREADS, tile + extra, st>>>(fp);
 }
-template <int LOGF>
-size_t fe_extra_smem() { return xc::FeCfg<LOGF>::WORK_BYTES + xc::FeCfg<LOGF>::TW_BYTES; }
 
 #define XC_FE_FOR_ALL(X) X(0) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12)
 
@@ -230,10 +232,26 @@ int fe_prepare(xc_plan_t* p) {
     for (int l = 0; l <= xc::FE_MAX_LOGF; ++l)
         if ((1 << l) == p->F) p->logf = l;
     if (p->logf < 0) return XC_OK;            // the F-engine calls will answer XC_ERR_UNSUPPORTED
-    std::vector<float2> tw(p->F);
-    for (int m = 0; m < p->F; ++m) fe_twiddle(p->F, m, &tw[m].x, &tw[m].y);
-    if (!p->d_twiddle) XC_CUDA(p, cudaMalloc(&p->d_twiddle, sizeof(float2) * p->F));
-    XC_CUDA(p, cudaMemcpy(p->d_twiddle, tw.data(), sizeof(float2) * p->F, cudaMemcpyHostToDevice));
+    // Per-pass tables in the order the kernel reads them (xc_fengine.cuh, FeCfg): the log2 F bits are split over
+    // NP = ceil(log2 F / 4) passes, the first (log2 F mod NP) passes one bit wider; pass i >= 1 with radix R_i on
+    // sub-transforms of length NS_i multiplies leg r of butterfly k by exp(-2 pi i k r / (NS_i R_i)): entry [k][r - 1].
+    std::vector<float2> tw;
+    const int L = p->logf, NP = (L + 3) / 4;
+    int ns = 1;
+    for (int i = 0; i < NP; ++i) {
+        const int R = 1 << (L / NP + (i < L % NP ? 1 : 0));
+        if (i >= 1)
+            for (int k = 0; k < ns; ++k)
+                for (int r = 1; r < R; ++r) {
+                    float2 w;
+                    fe_twiddle(p->F, k * r * (p->F / (ns * R)), &w.x, &w.y);
+                    tw.push_back(w);
+                }
+        ns *= R;
+    }
+    if (tw.empty()) tw.push_back(make_float2(1.f, 0.f));
+    if (!p->d_twiddle) XC_CUDA(p, cudaMalloc(&p->d_twiddle, sizeof(float2) * tw.size()));
+    XC_CUDA(p, cudaMemcpy(p->d_twiddle, tw.data(), sizeof(float2) * tw.size(), cudaMemcpyHostToDevice));
     switch (p->logf) {
 #define X(L) case L: XC_CUDA(p, fe_opt_in<L>()); break;
         XC_FE_FOR_ALL(X)
@@ -277,9 +295,10 @@ int fengine_launch(xc_plan_t* p, const int8_t* volt, float scale, int8_t* cube, 
     fp.scale = scale;
     const long long grid = static_cast<long long>(fp.nsb) * ((p->T + TT - 1) / TT);
     if (grid > 0x7FFFFFFFLL) return XC_ERR_UNSUPPORTED;
-    const size_t tile = (static_cast<size_t>(SB) * 4 * p->F * TT + 15) & ~static_cast<size_t>(15);
+    // output tile: 2 SB columns (signals) of TT * F two-byte samples, 4 bytes of padding per column
+    const size_t tile = (static_cast<size_t>(2) * SB * (static_cast<size_t>(TT) * p->F * 2 + 4) + 15) & ~static_cast<size_t>(15);
     switch (p->logf) {
-#define X(L) case L: fe_launch_one<L>(fp, static_cast<unsigned>(grid), tile + fe_extra_smem<L>(), st); break;
+#define X(L) case L: fe_launch_one<L>(fp, static_cast<unsigned>(grid), tile, st); break;
         XC_FE_FOR_ALL(X)
 #undef X
         default: return XC_ERR_UNSUPPORTED;

@@ -14,15 +14,17 @@
 // polarisations x TT time blocks.  Its 256 threads transform G = 256 / (F / RMAX) signals at a time with a Stockham
 // autosort FFT: ceil(log2 F / 4) passes of radix <= 16, every pass a register-resident butterfly per thread, passes
 // exchanged through a shared-memory work buffer; the first pass reads the int8 samples straight from global memory, the
-// last pass scales, rounds and drops its 2-byte results into a shared-memory tile [tt][f][SB x 4 bytes] whose rows are
-// rotated by their row index (bank-conflict-free 2-byte column writes).  When all signals are done the tile is streamed
-// out: every (t, f) row of the CTA is one contiguous run of SB x 4 bytes of the cube.
-// Twiddles come from a table exp(-2 pi i m / F) computed in fp64 on the host (exact at eighth turns) and kept in shared
-// memory.  Rounding = round-half-even in fp32 (cvt.rni), symmetric clip.
-// Two things the first ncu capture asked for (profiles/r2_ncu_fengine.md): the work buffer and the twiddle table are padded
-// by one complex slot per 16 (the Stockham scatter writes with a stride of R slots: 57 % of all shared-memory wavefronts
-// were bank conflicts), and all complex arithmetic is packed fp32x2 (add/sub/mul/fma.f32x2: one instruction per complex
-// add, two per complex multiply).
+// last pass scales, rounds and drops its 2-byte results into a shared-memory tile [signal][tt * F + f] (column-major: a
+// thread's outputs sit at compile-time offsets from one base; columns are padded by 4 bytes so that the row-wise read-out
+// is conflict-free).  When all signals are done the tile is streamed out: every (t, f) row of the CTA is one contiguous run
+// of SB x 4 bytes of the cube.
+// Twiddles are computed in fp64 on the host (exact at eighth turns), stored per pass in the order the pass reads them
+// ([k][r - 1] = exp(-2 pi i k r / (NS R))) and kept in shared memory.  Rounding = round-half-even in fp32, symmetric clip.
+// What the ncu captures asked for, in order (profiles/r2_ncu_fengine.md): (1) the work buffer is padded by one complex slot
+// per 16 (the Stockham scatter writes with a stride of R slots: 57 % of all shared-memory wavefronts were bank conflicts);
+// (2) all complex arithmetic is packed fp32x2 (one instruction per complex add, two per complex multiply); (3) int8 <-> fp32
+// conversions avoid the 16-lane conversion unit; (4) every shared-memory address of a pass is one per-thread base plus
+// compile-time offsets (45 % of the instructions were integer address arithmetic).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -41,7 +43,7 @@ struct FeParams {
     const int8_t* volt;       // [N][2][T*F][2]
     int8_t* cube;             // quantised output (or null)
     float* spec;              // unquantised fp32 spectra [T][F][N][2][2] (or null); testing aid, strided stores
-    const float2* tw;         // exp(-2 pi i m / F), m < F
+    const float2* tw;         // per-pass twiddle tables (fe_twiddle_layout), F - RMAX entries
     float scale;
 };
 
@@ -55,8 +57,10 @@ struct FeCfg {
     static constexpr int G = FE_THREADS / TPS;                               // signals per sub-batch
     static constexpr int FPAD = F + (F >> 4);                                // one padding slot per 16 complex slots
     static constexpr int WORK_BYTES = (NP > 1) ? G * FPAD * 8 : 0;           // [G][FPAD] float2
-    static constexpr int TW_BYTES = (NP > 1) ? FPAD * 8 : 0;
+    static constexpr int TW_N = (NP > 1) ? F - RMAX : 0;                     // sum over passes i >= 1 of NS_i (R_i - 1)
+    static constexpr int TW_BYTES = TW_N * 8;
     static constexpr int ns(int i) { return i == 0 ? 1 : ns(i - 1) << bits(i - 1); }   // product of the radices before pass i
+    static constexpr int tw_off(int i) { return i <= 1 ? 0 : tw_off(i - 1) + ns(i - 1) * ((1 << bits(i - 1)) - 1); }
     static_assert(TPS <= FE_THREADS && TPS >= 1, "threads per signal");
 };
 
@@ -189,17 +193,6 @@ __device__ __forceinline__ uint32_t fe_quant2(float2 y) {
     return __byte_perm(__float_as_uint(t.x), __float_as_uint(t.y), 0x7740) & 0xFFFFu;
 }
 
-// Byte offset inside the CTA's output tile of the 2-byte sample (row rho = tt * F + f, signal column sp) when rows hold RB
-// bytes: the tile is a sequence of 128-byte lines of m = 128 / RB rows; each line is rotated by (line % 32) words so that
-// threads writing one column of 32 consecutive rows hit 32 different banks.
-// lrb = log2 RB (5, 6 or 7), so m = 1 << (7 - lrb).
-__device__ __forceinline__ uint32_t fe_tile_off(uint32_t rho, uint32_t sp, uint32_t lrb) {
-    const uint32_t lm = 7u - lrb;
-    const uint32_t line = rho >> lm;
-    const uint32_t o = ((rho & ((1u << lm) - 1u)) << lrb) + sp * 2u;
-    return line * 128u + ((o + 4u * (line & 31u)) & 127u);
-}
-
 // One pass of the Stockham FFT for this thread's butterflies.  v[b][r]: butterfly b (j = tid_in_signal + b * TPS), leg r.
 template <int LOGF, int PASS>
 struct FePass {
@@ -208,6 +201,7 @@ struct FePass {
     static constexpr int NB = C::RMAX / R;                // butterflies per thread
     static constexpr int NS = C::ns(PASS);                // length of the sub-transforms done so far
     static constexpr int STRIDE = C::F / R;               // distance of a butterfly's legs in the input of the pass
+    static constexpr int TW_OFF = C::tw_off(PASS);        // where this pass's twiddle table starts
 
     static __host__ __device__ constexpr int padc(int c) { return c + (c >> 4); }     // fe_pad of a compile-time offset
     // fe_pad(x + c) = fe_pad(x) + padc(c) whenever x % 16 + c % 16 < 16, which holds for every (x, c) used below: c is a
@@ -237,9 +231,9 @@ struct FePass {
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
             if (NS > 1) {
-                const int kc = ((ts + b * C::TPS) & (NS - 1)) * (C::F / (NS * R));
+                const float2* tk = tw + TW_OFF + ((ts + b * C::TPS) & (NS - 1)) * (R - 1);  // row k of this pass's table
 #pragma unroll
-                for (int r = 1; r < R; ++r) v[b][r] = cmul(v[b][r], tw[fe_pad(kc * r)]);
+                for (int r = 1; r < R; ++r) v[b][r] = cmul(v[b][r], tk[r - 1]);
             }
             Dft<R>::run(v[b]);
         }
@@ -283,23 +277,26 @@ struct FeRun {
     }
 };
 
-template <int LOGF>
+// SPEC = false: the product kernel (quantised cube).  SPEC = true: the fp32 spectra for the transform's own parity test.
+template <int LOGF, bool SPEC>
 __global__ void __launch_bounds__(FE_THREADS) xc_fengine_kernel(const FeParams p) {
     using C = FeCfg<LOGF>;
     constexpr int F = C::F;
     extern __shared__ __align__(16) uint8_t fe_smem[];
-    uint8_t* tile = fe_smem;                                                          // [TT][F] rows of RB bytes, rotated
-    const uint32_t RB = static_cast<uint32_t>(p.SB) * 4u;           // 32, 64 or 128
-    const uint32_t lrb = 31u - __clz(RB);
-    const uint32_t tile_bytes = RB * F * p.TT;
-    float2* work = reinterpret_cast<float2*>(fe_smem + ((tile_bytes + 15u) & ~15u));   // [G][FPAD]
+    // output tile, column-major: column sp (signal) holds the TT * F samples of the CTA's time blocks, 2 bytes each, columns
+    // CS bytes apart (+4: the read-out below walks along sp)
+    const int lsb = 32 - __clz(p.SB);                               // log2(2 SB): SB is 8, 16 or 32
+    const uint32_t CS = static_cast<uint32_t>(p.TT) * F * 2u + 4u;
+    const uint32_t tile_bytes = SPEC ? 0u : (2u * p.SB * CS + 15u) & ~15u;
+    uint8_t* tile = fe_smem;
+    float2* work = reinterpret_cast<float2*>(fe_smem + tile_bytes);                    // [G][FPAD]
     float2* tw = reinterpret_cast<float2*>(reinterpret_cast<uint8_t*>(work) + C::WORK_BYTES);
 
     const int tid = threadIdx.x;
     const int s0 = static_cast<int>(blockIdx.x % p.nsb) * p.SB;       // station groups fastest: neighbouring CTAs complete
     const int t0 = static_cast<int>(blockIdx.x / p.nsb) * p.TT;       // each other's 128-byte lines in L2
     if (C::NP > 1) {
-        for (int m = tid; m < F; m += FE_THREADS) tw[fe_pad(m)] = __ldg(p.tw + m);
+        for (int m = tid; m < C::TW_N; m += FE_THREADS) tw[m] = __ldg(p.tw + m);
         __syncthreads();
     }
     const int g = tid / C::TPS;             // signal of the sub-batch this thread works on
@@ -310,8 +307,8 @@ __global__ void __launch_bounds__(FE_THREADS) xc_fengine_kernel(const FeParams p
 
     // (signal, time block) q of the CTA -> where its F samples start and whether it exists
     auto locate = [&](int q, int& sp, int& tt, int& s, int& pol, int& t) {
-        sp = q % (2 * p.SB);
-        tt = q / (2 * p.SB);
+        sp = q & (2 * p.SB - 1);
+        tt = q >> lsb;
         s = s0 + (sp >> 1);
         pol = sp & 1;
         t = t0 + tt;
@@ -337,33 +334,41 @@ __global__ void __launch_bounds__(FE_THREADS) xc_fengine_kernel(const FeParams p
             const bool ok2 = locate(q0 + C::G + g, sp2, tt2, s2, pol2, t2);
             P0::load_raw(raw, p.volt + ((static_cast<long long>(s2) * 2 + pol2) * TF + static_cast<long long>(t2) * F) * 2, ts, ok2);
         }
-        auto sink = [&](int f, float2 X) {
-            if (!ok) return;
-            if (p.spec) {
-                float2* dst = reinterpret_cast<float2*>(p.spec) + ((static_cast<long long>(t) * F + f) * p.N + s) * 2 + pol;
-                *dst = X;
-            }
-            if (p.cube) {
-                const float2 y = mul2(X, make_float2(p.scale, p.scale));      // one rounding per component, like __fmul_rn
-                const uint32_t off = fe_tile_off(static_cast<uint32_t>(tt) * F + f, sp, lrb);
-                *reinterpret_cast<uint16_t*>(tile + off) = static_cast<uint16_t>(fe_quant2(y));
-            }
-        };
-        FeRun<LOGF, 0>::run(cur, buf, tw, ts, sink);
+        if constexpr (SPEC) {
+            float2* dst = reinterpret_cast<float2*>(p.spec) + (static_cast<long long>(t) * F * p.N + s) * 2 + pol;
+            const long long fstride = static_cast<long long>(p.N) * 2;
+            auto sink = [&](int f, float2 X) {
+                if (ok) dst[f * fstride] = X;
+            };
+            FeRun<LOGF, 0>::run(cur, buf, tw, ts, sink);
+        } else {
+            // column sp, row tt * F: the thread's outputs f = j + r * NS land at compile-time offsets from here
+            uint16_t* col = reinterpret_cast<uint16_t*>(tile + static_cast<uint32_t>(sp) * CS) + tt * F;
+            const float2 sc2 = make_float2(p.scale, p.scale);
+            const bool inq = (q0 + g) < nq;       // columns of stations >= N / blocks >= T exist in the tile and are masked at read-out
+            auto sink = [&](int f, float2 X) {
+                if (inq) col[f] = static_cast<uint16_t>(fe_quant2(mul2(X, sc2)));      // one rounding per component, like __fmul_rn
+            };
+            FeRun<LOGF, 0>::run(cur, buf, tw, ts, sink);
+        }
     }
-    if (!p.cube) return;
+    if constexpr (SPEC) return;
     __syncthreads();
-    // Stream the tile out, one 128-byte line (128 / RB rows of the cube) per warp instruction: lane = word of the line.
-    const uint32_t lm = 7u - lrb, lw = lrb - 2u;                  // log2 of rows per line, of words per row
-    const uint32_t nlines = (static_cast<uint32_t>(p.TT) * F + (1u << lm) - 1u) >> lm;
+    // Stream the tile out: one warp instruction writes 128 contiguous... bytes per cube row segment -- lane = (row, station)
+    // with 128 / RB rows per instruction; a lane gathers its station's two polarisations (two 2-byte columns) into one word.
+    const uint32_t lrb = static_cast<uint32_t>(lsb) + 1u;         // log2 of RB = 4 SB bytes per row segment
+    const uint32_t lm = 7u - lrb, lw = lrb - 2u;                  // log2 of rows per instruction, of words (stations) per row
+    const uint32_t nrows = static_cast<uint32_t>(p.TT) * F;
     const uint32_t lane = tid & 31, warp = tid >> 5;
-    for (uint32_t line = warp; line < nlines; line += FE_THREADS / 32) {
-        const uint32_t rho = (line << lm) + (lane >> lw);         // row of the tile: tt * F + f
-        const uint32_t cw = lane & ((1u << lw) - 1u);             // word of the row = station s0 + cw
+    const uint32_t cw = lane & ((1u << lw) - 1u);                 // station s0 + cw
+    const uint16_t* c0 = reinterpret_cast<const uint16_t*>(tile + (2u * cw) * CS);
+    const uint16_t* c1 = reinterpret_cast<const uint16_t*>(tile + (2u * cw + 1u) * CS);
+    const int s = s0 + static_cast<int>(cw);
+    for (uint32_t rho = (warp << lm) + (lane >> lw); rho < nrows; rho += (FE_THREADS / 32) << lm) {
         const uint32_t tt = rho >> LOGF, f = rho & (F - 1);
-        const int t = t0 + static_cast<int>(tt), s = s0 + static_cast<int>(cw);
-        if (tt < static_cast<uint32_t>(p.TT) && t < p.T && s < p.N) {
-            const uint32_t w = *reinterpret_cast<const uint32_t*>(tile + line * 128u + (((lane + line) & 31u) << 2));
+        const int t = t0 + static_cast<int>(tt);
+        if (t < p.T && s < p.N) {
+            const uint32_t w = static_cast<uint32_t>(c0[rho]) | (static_cast<uint32_t>(c1[rho]) << 16);
             int8_t* row = p.cube + (static_cast<long long>(t) * F + f) * p.pitch;
             __stcs(reinterpret_cast<uint32_t*>(row) + s, w);
         }
