@@ -163,27 +163,34 @@ def cpu_sample(w, x, target_s=12.0):
 
 
 def run_reference(args, rank):
-    """--impl reference: the CPU oracle as it stands, on the host cores (rank 0 only)."""
+    """--impl reference: the CPU oracle as it stands, on the host cores (rank 0 only).  A step = a bounded sample of the
+    workload: `cores` channels (the oracle parallelises over channels only) and as many time samples as the oracle does in
+    about 2 s, so that the driver's --steps 20 --warmup 5 ends within a few minutes at every N."""
     if rank != 0:
         return
     import xc_workloads as wl
     from oracle import xo
     w = wl.CONFIGS[args.workload]
     cores = xo.num_threads()
-    per_ch = w.T * w.N * (2 * w.N + 1)
-    # a step = `nch` channels of the workload (bounded sample; channels are independent)
     nch = max(1, min(w.F, cores))
-    sub = wl.Workload(w.name, w.N, nch, w.T, w.kind, w.sigma, w.seed)
-    x = wl.make_input(sub)
     sel = list(range(nch))
+    per_sample = nch * w.N * (2 * w.N + 1)                         # cMACs per time sample of the step
+    t_cal = min(w.T, 32)
+    x_cal = wl.make_input(wl.Workload(w.name, w.N, nch, t_cal, w.kind, w.sigma, w.seed))
+    xo.channels_i8(x_cal, sel)
+    t0 = time.perf_counter()
+    xo.channels_i8(x_cal, sel)
+    rate = t_cal * per_sample / (time.perf_counter() - t0)
+    T_s = int(max(1, min(w.T, 2.0 * rate / per_sample)))
+    x = wl.make_input(wl.Workload(w.name, w.N, nch, T_s, w.kind, w.sigma, w.seed))
     for _ in range(args.warmup):
         xo.channels_i8(x, sel)
     t0 = time.perf_counter()
     for _ in range(args.steps):
         xo.channels_i8(x, sel)
     dt = time.perf_counter() - t0
-    tops = 8.0 * args.steps * nch * per_ch / dt / 1e12
-    sample = f"{nch} of {w.F} channels of {w.name} per step, all baselines"
+    tops = 8.0 * args.steps * T_s * per_sample / dt / 1e12
+    sample = f"{nch} of {w.F} channels x {T_s} of {w.T} time samples of {w.name} per step, all baselines"
     print(json.dumps({
         "impl": "reference", "metric": "X-engine Tops/s (8 ops per cMAC)", "value": tops, "unit": "Tops/s",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,

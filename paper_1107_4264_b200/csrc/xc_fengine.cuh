@@ -31,6 +31,9 @@
 
 namespace xc {
 
+#ifndef XC_FE_RADIX32
+#define XC_FE_RADIX32 1
+#endif
 constexpr int FE_THREADS = 256;
 constexpr int FE_MAX_LOGF = 12;            // F <= 4096
 constexpr int FE_TILE_BYTES = 32768;       // target size of the CTA's output tile (53 KB per CTA at F = 512: 4 CTAs per SM)
@@ -47,10 +50,19 @@ struct FeParams {
     float scale;
 };
 
+// number of passes for F = 2^logf (host mirror of FeCfg<LOGF>::NP, for the twiddle-table layout)
+inline int fe_num_passes(int logf) {
+    const int maxb = (XC_FE_RADIX32 && (logf == 5 || logf == 9 || logf == 10)) ? 5 : 4;
+    return (logf + maxb - 1) / maxb;
+}
+
 template <int LOGF>
 struct FeCfg {
     static constexpr int F = 1 << LOGF;
-    static constexpr int NP = (LOGF + 3) / 4;                               // passes (0 for F = 1)
+    // bits per pass: at most 4 (radix 16), except that F = 32, 512 and 1024 use radix 32 so that they need one pass less
+    // (the kernel is bound by the shared-memory traffic of the passes, profiles/r2_ncu_fengine.md)
+    static constexpr int MAXB = (XC_FE_RADIX32 && (LOGF == 5 || LOGF == 9 || LOGF == 10)) ? 5 : 4;
+    static constexpr int NP = (LOGF + MAXB - 1) / MAXB;                      // passes (0 for F = 1)
     static constexpr int bits(int i) { return NP ? LOGF / NP + (i < LOGF % NP ? 1 : 0) : 0; }
     static constexpr int RMAX = 1 << bits(0);                                // points per thread
     static constexpr int TPS = F / RMAX;                                     // threads per signal
@@ -172,6 +184,40 @@ template <> struct Dft<16> {
         for (int k = 0; k < 8; ++k) {
             v[k] = cadd(e[k], o[k]);
             v[k + 8] = csub(e[k], o[k]);
+        }
+    }
+};
+
+template <> struct Dft<32> {
+    static __device__ __forceinline__ void run(float2 (&v)[32]) {
+        float2 e[16], o[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            e[k] = v[2 * k];
+            o[k] = v[2 * k + 1];
+        }
+        Dft<16>::run(e);
+        Dft<16>::run(o);
+        // o[k] *= exp(-2 pi i k / 32)
+        o[1] = cmul(o[1], make_float2(0.98078528040323043058f, -0.19509032201612824808f));
+        o[2] = cmul(o[2], make_float2(0.92387953251128673848f, -0.38268343236508978178f));
+        o[3] = cmul(o[3], make_float2(0.83146961230254523567f, -0.55557023301960217765f));
+        o[4] = mul_w8_1(o[4]);
+        o[5] = cmul(o[5], make_float2(0.55557023301960228867f, -0.83146961230254523567f));
+        o[6] = cmul(o[6], make_float2(0.38268343236508983729f, -0.92387953251128673848f));
+        o[7] = cmul(o[7], make_float2(0.19509032201612833135f, -0.98078528040323043058f));
+        o[8] = mul_mi(o[8]);
+        o[9] = cmul(o[9], make_float2(-0.19509032201612819257f, -0.98078528040323043058f));
+        o[10] = cmul(o[10], make_float2(-0.38268343236508972627f, -0.92387953251128673848f));
+        o[11] = cmul(o[11], make_float2(-0.55557023301960195560f, -0.83146961230254545772f));
+        o[12] = mul_w8_3(o[12]);
+        o[13] = cmul(o[13], make_float2(-0.83146961230254534669f, -0.55557023301960217765f));
+        o[14] = cmul(o[14], make_float2(-0.92387953251128673848f, -0.38268343236508989280f));
+        o[15] = cmul(o[15], make_float2(-0.98078528040323043058f, -0.19509032201612860891f));
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            v[k] = cadd(e[k], o[k]);
+            v[k + 16] = csub(e[k], o[k]);
         }
     }
 };
