@@ -233,7 +233,7 @@ int fe_prepare(xc_plan_t* p) {
         if ((1 << l) == p->F) p->logf = l;
     if (p->logf < 0) return XC_OK;            // the F-engine calls will answer XC_ERR_UNSUPPORTED
     // Per-pass tables in the order the kernel reads them (xc_fengine.cuh, FeCfg): the log2 F bits are split over
-    // NP passes (radix <= 16, or <= 32 for F = 32, 512, 1024), the first (log2 F mod NP) passes one bit wider; pass i >= 1 with radix R_i on
+    // NP passes (radix <= 16, or <= 32 for F = 512, 1024), the first (log2 F mod NP) passes one bit wider; pass i >= 1 with radix R_i on
     // sub-transforms of length NS_i multiplies leg r of butterfly k by exp(-2 pi i k r / (NS_i R_i)): entry [k][r - 1].
     std::vector<float2> tw;
     const int L = p->logf, NP = xc::fe_num_passes(L);

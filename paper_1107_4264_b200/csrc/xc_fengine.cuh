@@ -52,16 +52,17 @@ struct FeParams {
 
 // number of passes for F = 2^logf (host mirror of FeCfg<LOGF>::NP, for the twiddle-table layout)
 inline int fe_num_passes(int logf) {
-    const int maxb = (XC_FE_RADIX32 && (logf == 5 || logf == 9 || logf == 10)) ? 5 : 4;
+    const int maxb = (XC_FE_RADIX32 && (logf == 9 || logf == 10)) ? 5 : 4;
     return (logf + maxb - 1) / maxb;
 }
 
 template <int LOGF>
 struct FeCfg {
     static constexpr int F = 1 << LOGF;
-    // bits per pass: at most 4 (radix 16), except that F = 32, 512 and 1024 use radix 32 so that they need one pass less
-    // (the kernel is bound by the shared-memory traffic of the passes, profiles/r2_ncu_fengine.md)
-    static constexpr int MAXB = (XC_FE_RADIX32 && (LOGF == 5 || LOGF == 9 || LOGF == 10)) ? 5 : 4;
+    // bits per pass: at most 4 (radix 16), except that F = 512 and 1024 use radix 32 so that they need two passes instead of
+    // three (the kernel is bound by the shared-memory traffic of the passes, profiles/r2_ncu_fengine.md): measured 0.624
+    // against 0.648 ms (F = 512) and 0.623 against 0.645 ms (F = 1024); F = 32 in one radix-32 pass was slower (0.56 vs 0.32 ms).
+    static constexpr int MAXB = (XC_FE_RADIX32 && (LOGF == 9 || LOGF == 10)) ? 5 : 4;
     static constexpr int NP = (LOGF + MAXB - 1) / MAXB;                      // passes (0 for F = 1)
     static constexpr int bits(int i) { return NP ? LOGF / NP + (i < LOGF % NP ? 1 : 0) : 0; }
     static constexpr int RMAX = 1 << bits(0);                                // points per thread
