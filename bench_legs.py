@@ -228,9 +228,35 @@ def extras(stream, clocks, sampler, peaks):
     del host, dev2, v5
     torch.cuda.empty_cache()
 
+    # ---- T-split of the single-CTA tile (small N, long integration), off / on / what AUTO picks -----------
+    out["t_split"] = t_split_leg(stream)
+
     # ---- F-engine + corner turn, and the FX chain ----------------------------------------------------------
     out["fx"] = fengine_leg(stream, "cfg3")
     return out
+
+
+def t_split_leg(stream):
+    """The paper's small-N future work (PAPER.md:311-313): one 128 x 128 tile per channel leaves SMs idle and walks T serially;
+    the T-split halves that walk over a cluster of 2.  Two shapes: config 5's N = 32 (T = 2048, where the hand-over costs more
+    than it saves and AUTO keeps it off) and a long integration N = 32, F = 32, T = 16384 (where AUTO turns it on)."""
+    import torch
+    import paper_1107_4264_b200 as xcb
+    import xc_workloads as wl
+    from bench import kernel_durations
+    res = {}
+    for name, (N, F, T) in {"cfg5_N32 (F=64, T=2048)": (32, 64, 2048), "long integration (N=32, F=32, T=16384)": (32, 32, 16384)}.items():
+        x = torch.from_numpy(wl.gaussian(N, F, T, seed=77, sigma=4.0)).cuda()
+        row = {}
+        for label, ts in (("off", 1), ("on", 2), ("auto", 0)):
+            p = xcb.Plan(N, F, T)
+            p.set_option(xcb.OPT_TSPLIT, ts)
+            v = p.new_vis()
+            km, em, _ = kernel_durations(p, x, v, stream, 10)
+            row[label] = {"kernel_us": km * 1e3, "t_split_used": p.t_split}
+            p.close()
+        res[name] = row
+    return res
 
 
 def _fx_leg(stream, workload, launches, with_fx):

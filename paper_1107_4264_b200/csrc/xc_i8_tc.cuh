@@ -439,9 +439,10 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
         }
     }
 
-    // Teardown: nobody leaves (or frees TMEM) while a peer may still signal into this CTA.
+    // Teardown: nobody leaves (or frees TMEM) while a peer may still signal into this CTA (execution ordering only: the
+    // kernel's end makes the global stores visible, a release here would only wait for them).
     tc_fence_before();
-    if (CLUSTER) cluster_sync_all(); else __syncthreads();
+    if (CLUSTER) cluster_sync_relaxed(); else __syncthreads();
     if (warp == 1) {
         __syncwarp();
         tc_fence_after();

@@ -74,6 +74,13 @@ __device__ __forceinline__ uint32_t cluster_ctarank() {
 __device__ __forceinline__ void cluster_sync_all() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
+// Execution-only rendezvous of the cluster: nobody passes before everybody has arrived, but no memory ordering is
+// asked for.  Used at teardown, where the only purpose is to keep shared memory / TMEM alive while peers may still
+// signal into this CTA: the .release form compiles to MEMBAR.ALL.GPU, i.e. it first waits until every global store
+// of the epilogue has been acknowledged (measured ~2300 cycles = 1.3 us at the end of every launch).
+__device__ __forceinline__ void cluster_sync_relaxed() {
+    asm volatile("barrier.cluster.arrive.relaxed.aligned;\n\tbarrier.cluster.wait.aligned;" ::: "memory");
+}
 // shared::cta address -> shared::cluster address of the same variable in CTA `rank` of the cluster
 __device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {
     uint32_t r;
