@@ -106,8 +106,59 @@ def fma_probe(iters=100000):
         return {"unavailable": repr(e)}
 
 
+def trace_leg(workload, stream):
+    """Pipeline timeline of CTA 0 of xc_i8_tc_kernel from the PROFILING build (libxc_profile.so, -DXC_PROFILE): clock64 stamps
+    of the TMA producer, the MMA issuer and one epilogue warp, relative to the CTA's start, for the first tiles of `workload`.
+    Returns per-role lists of cycle stamps and the derived per-stage periods."""
+    import torch
+    import paper_1107_4264_b200 as xcb
+    import xc_workloads as wl
+    from paper_1107_4264_b200 import build as xc_build
+    xcb.load_library(xc_build.build(profile=True))
+    w = wl.CONFIGS[workload]
+    x = torch.from_numpy(wl.make_input(w)).cuda()
+    p = xcb.Plan(w.N, w.F, w.T)
+    v = p.new_vis()
+    tr = torch.zeros(xcb.TRACE_WORDS, dtype=torch.int64, device="cuda")
+    st = torch.zeros(xcb.TIMING_WORDS, dtype=torch.int64, device="cuda")
+    with torch.cuda.stream(stream):
+        for _ in range(5):
+            p.correlate(x, v, stream=stream)
+        stream.synchronize()
+        p.set_trace(tr)
+        p.set_timing_buffer(st)
+        st[0] = 2 ** 62
+        stream.synchronize()
+        p.correlate(x, v, stream=stream)
+        stream.synchronize()
+    t = tr.cpu().view(3, 256, 4)
+    s6 = st.tolist()
+    c0 = s6[2]
+    tile = p.tiles()[0][2]
+    bk = 128 if tile == 64 else 256
+    kb = (w.T + bk - 1) // bk
+    n = min(256, 3 * kb)
+    rel = lambda a: [int(q - c0) if q else None for q in a]
+    mma = [rel(t[1, i].tolist()) for i in range(n) if t[1, i, 0]]
+    prod = [rel(t[0, i, :3].tolist()) for i in range(n) if t[0, i, 0]]
+    epi = [rel(t[2, i, :3].tolist()) for i in range(4) if t[2, i, 0]]
+    per = [mma[i + 1][0] - mma[i][0] for i in range(len(mma) - 1)]
+    out = {"workload": workload, "tile_stations": tile, "stages_per_tile": kb, "samples_per_stage": bk,
+           "kernel_ns": s6[1] - s6[0], "cta0_cycles": s6[4] - s6[2], "sm_mhz": (s6[4] - s6[2]) / max(1, s6[5] - s6[3]) * 1e3,
+           "producer_first_issue_cycle": prod[0][2] if prod else None, "first_data_ready_cycle": mma[0][1] if mma else None,
+           "mma_stage_period_cycles_tile0": per[:kb - 1], "mma_stage_period_cycles_tile1": per[kb:2 * kb - 1],
+           "mma_stage_breakdown_first8 (wait_start, data_ready, mmas_issued, committed)": mma[:8],
+           "epilogue_tiles (start, accumulator_ready, done)": epi,
+           "ideal_tensor_cycles_per_stage": 512}
+    p.close()
+    xcb.load_library()
+    return out
+
+
 def only_leg(which, workload, stream):
     """Profiling aid for ncu captures: a few launches of one secondary kernel."""
+    if which == "trace":
+        return {"only": "trace", **trace_leg(workload, stream)}
     if which == "f32":
         return {"only": "f32", **f32_leg(stream, None, F=32, launches=3)}
     if which == "fengine":
