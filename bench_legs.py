@@ -106,7 +106,7 @@ def fma_probe(iters=100000):
         return {"unavailable": repr(e)}
 
 
-def trace_leg(workload, stream):
+def trace_leg(workload, stream, debug_skip=0):
     """Pipeline timeline of CTA 0 of xc_i8_tc_kernel from the PROFILING build (libxc_profile.so, -DXC_PROFILE): clock64 stamps
     of the TMA producer, the MMA issuer and one epilogue warp, relative to the CTA's start, for the first tiles of `workload`.
     Returns per-role lists of cycle stamps and the derived per-stage periods."""
@@ -118,6 +118,7 @@ def trace_leg(workload, stream):
     w = wl.CONFIGS[workload]
     x = torch.from_numpy(wl.make_input(w)).cuda()
     p = xcb.Plan(w.N, w.F, w.T)
+    p.set_option(xcb.OPT_DEBUG_SKIP, debug_skip)      # profiling build only: 1 no TMA loads, 2 no MMAs, 4 no stores, 8 stores to an 8 MB window
     v = p.new_vis()
     tr = torch.zeros(xcb.TRACE_WORDS, dtype=torch.int64, device="cuda")
     st = torch.zeros(xcb.TIMING_WORDS, dtype=torch.int64, device="cuda")
@@ -143,7 +144,7 @@ def trace_leg(workload, stream):
     prod = [rel(t[0, i, :3].tolist()) for i in range(n) if t[0, i, 0]]
     epi = [rel(t[2, i, :3].tolist()) for i in range(4) if t[2, i, 0]]
     per = [mma[i + 1][0] - mma[i][0] for i in range(len(mma) - 1)]
-    out = {"workload": workload, "tile_stations": tile, "stages_per_tile": kb, "samples_per_stage": bk,
+    out = {"workload": workload, "debug_skip": debug_skip, "tile_stations": tile, "stages_per_tile": kb, "samples_per_stage": bk,
            "kernel_ns": s6[1] - s6[0], "cta0_cycles": s6[4] - s6[2], "sm_mhz": (s6[4] - s6[2]) / max(1, s6[5] - s6[3]) * 1e3,
            "producer_first_issue_cycle": prod[0][2] if prod else None, "first_data_ready_cycle": mma[0][1] if mma else None,
            "mma_stage_period_cycles_tile0": per[:kb - 1], "mma_stage_period_cycles_tile1": per[kb:2 * kb - 1],
@@ -158,7 +159,8 @@ def trace_leg(workload, stream):
 def only_leg(which, workload, stream):
     """Profiling aid for ncu captures: a few launches of one secondary kernel."""
     if which == "trace":
-        return {"only": "trace", **trace_leg(workload, stream)}
+        import os
+        return {"only": "trace", **trace_leg(workload, stream, int(os.environ.get("XC_TRACE_SKIP", "0")))}
     if which == "f32":
         return {"only": "f32", **f32_leg(stream, None, F=32, launches=3)}
     if which == "fengine":
