@@ -160,3 +160,23 @@ def test_option_validation():
     for mode in (3, 1, 0):
         p.set_option(xcb.OPT_TILE, mode)
         assert len(p.tiles()) >= 1
+
+
+def test_tracked_ncu_exports_feed_the_bench_roofline():
+    """bench.py reads `roofline.traffic` and the tensor-pipe figure from the tracked ncu exports under profiles/ (nothing is
+    hard-coded in bench.py): every export of this round parses, names the X-engine kernel, and its DRAM traffic is within 12 %
+    of the algorithmic bytes of its workload (input read once, output written once -- no wasted re-reads)."""
+    import sys
+    sys.path.insert(0, ROOT)
+    import bench
+    import xc_workloads as wl
+    seen = 0
+    for name in ("cfg2", "cfg3", "cfg4", "cfg5_N500", "cfg5_N1024"):
+        prof = bench.ncu_profile(name)
+        assert prof and prof["launches"] >= 1, name
+        w = wl.CONFIGS[name]
+        assert 0.88 <= prof["dram_bytes"] / (w.in_bytes + w.vis_bytes) <= 1.12, (name, prof["dram_bytes"])
+        assert 40.0 < prof["tensor_pipe_active_pct"] <= 100.0
+        seen += 1
+    assert seen == 5
+    assert bench.ncu_profile("no_such_workload") == {}

@@ -193,3 +193,27 @@ def test_fx_chain_config3_shape_sampled():
     assert nbad <= 3
     p.set_in_pitch(p.scratch_pitch)
     assert torch.equal(p.correlate(cube), vis)
+
+
+@pytest.mark.parametrize("N,F,T", [(128, 1024, 24), (1024, 64, 40), (500, 64, 33)])
+def test_cube_other_config_shapes_sampled(N, F, T):
+    """The other BASELINE shape classes (config 2: 1024-point transforms, radix 32 x 32; config 5: N = 1024 and the ragged
+    N = 500 with 64-point transforms), a few time blocks each: sampled spectra of the cube against the oracle (near-tie rule)."""
+    volt = wl.voltages(N, F, T, seed=N + F, tones=1)
+    scale = wl.fengine_scale(F)
+    p = xcb.Plan(N, F, T)
+    got = gpu_cube(p, volt, scale)
+    rng = np.random.default_rng(N)
+    sel = [(0, 0, 0), (N - 1, 1, T - 1)] + [(int(rng.integers(N)), int(rng.integers(2)), int(rng.integers(T))) for _ in range(22)]
+    X = fo.spectra(volt, F, sel)
+    nbad = 0
+    for (s, pol, t), Xs in zip(sel, X):
+        for c, part in enumerate((Xs.real, Xs.imag)):
+            y = part * np.float64(np.float32(scale))
+            ref = fo.quantise(part, scale)
+            m = np.abs(y - np.floor(y) - 0.5)
+            d = got[t, :, s, pol, c].astype(int) - ref.astype(int)
+            assert (d[m > scale * tol(F)] == 0).all() and np.abs(d).max() <= 1, (s, pol, t, c)
+            nbad += int((d != 0).sum())
+    assert nbad <= 3
+    p.close()
