@@ -204,14 +204,23 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
         mbar_init(pfree_bar, TC_EPI_WARPS);
         fence_barrier_init();
     }
+    // Rendezvous 1 (CTA or cluster): the barriers exist.  Threads only ARRIVE here; the TMEM allocation (several hundred
+    // cycles) happens between arrive and wait, and the TMA producer, which needs no TMEM, leaves as soon as everybody has
+    // arrived -- its first loads are in flight while warp 1 still allocates (-0.3 us on the microsecond-scale launches).
+    if (CLUSTER) cluster_arrive_relaxed(); else __syncthreads();
     if (warp == 1) {
         tmem_alloc<CG>(smem_u32(tmem_slot), TMEM_COLS);
         tmem_relinquish<CG>();
+        tc_fence_before();
     }
-    tc_fence_before();
-    if (CLUSTER) cluster_sync_all(); else __syncthreads();
-    tc_fence_after();
-    const uint32_t tmem_base = *tmem_slot;
+    if (CLUSTER) cluster_wait();
+    uint32_t tmem_base = 0;
+    if (warp != 0) {
+        // Rendezvous 2 (MMA issuer + epilogue warps of this CTA): the TMEM base address is in shared memory
+        named_bar_sync(1, TC_THREADS - 32);
+        tc_fence_after();
+        tmem_base = *tmem_slot;
+    }
     // Programmatic dependent launch: everything above (barrier init, TMEM allocation, descriptor prefetch) touched no
     // global memory that a predecessor writes and may overlap the tail of the previous kernel in the stream; from here
     // on this kernel reads the input / tile table and writes vis, so it first waits for that kernel to complete.  The
