@@ -499,6 +499,25 @@ def main():
                 s_tops = ww.ops / (s["ms_per_launch"] * 1e-3) / 1e12
                 ent["sustained"] = {"ms_per_launch": s["ms_per_launch"], "tops": s_tops, "frac": s_tops / i8_sustained, "nvml": s["nvml"]}
             per_config[name] = ent
+            if name == "cfg5_N500":
+                # the same values in a block whose rows are xc_scratch_pitch() = 2048 bytes apart (xc_set_in_pitch): what the
+                # F-engine and the host-buffer calls hand to the X-engine (line-aligned rows)
+                pitch = pp.scratch_pitch
+                xp = torch.zeros((ww.T, ww.F, pitch), dtype=torch.int8, device="cuda")
+                xp[:, :, :4 * ww.N] = xx.view(ww.T, ww.F, 4 * ww.N)
+                pp.set_in_pitch(pitch)
+                km2, em2, mhz2 = kernel_durations(pp, xp, vv, stream, 10)
+                ent2 = roofline_entry(ww, km2, peaks, i8_burst, ncu_profile(name + "_p2048"))
+                ent2.pop("ncu", None)
+                ent2.update({"N": ww.N, "F": ww.F, "T": ww.T, "row_pitch_bytes": pitch, "event_ms": em2, "sm_mhz_in_kernel": mhz2,
+                             "back_to_back_ms": back_to_back(pp, xp, vv, stream, 20),
+                             "tensor_pipe_active_ncu_pct": ncu_profile(name + "_p2048").get("tensor_pipe_active_pct")})
+                if not args.no_sustained:
+                    s = sustained_leg(pp, xp, vv, stream, sampler, min(args.sustained_seconds, 1.5), km2)
+                    s_tops = ww.ops / (s["ms_per_launch"] * 1e-3) / 1e12
+                    ent2["sustained"] = {"ms_per_launch": s["ms_per_launch"], "tops": s_tops, "frac": s_tops / i8_sustained, "nvml": s["nvml"]}
+                per_config["cfg5_N500_pitch2048"] = ent2
+                del xp
             pp.close()
             del xx, vv
             torch.cuda.empty_cache()

@@ -398,7 +398,7 @@ int stage_if_needed(xc_plan_t* p, const int8_t* in_dev, cudaStream_t st, const v
             xc::xc_unpack_i4_kernel<<<grid(units), 256, 0, st>>>(
                 reinterpret_cast<const uint8_t*>(in_dev), static_cast<uint32_t*>(p->ws), p->T, p->F, f0, nf, p->N, npad);
         }
-    } else if (p->in_pitch % 16 == 0 && !(reinterpret_cast<uintptr_t>(in_dev) & 15u)) {
+    } else if (p->N % 4 == 0 && p->in_pitch % 16 == 0 && !(reinterpret_cast<uintptr_t>(in_dev) & 15u)) {
         xc::xc_stage_pad16_kernel<<<grid(rows * (npad / 4)), 256, 0, st>>>(
             reinterpret_cast<const uint4*>(in_dev), static_cast<uint4*>(p->ws), rows, p->N / 4,
             static_cast<int>(p->in_pitch / 16), npad / 4);

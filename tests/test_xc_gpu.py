@@ -513,6 +513,10 @@ def test_pitched_device_input(N, F, T, pitch):
             assert np.array_equal(vis.cpu().numpy()[F - 1], ref[F - 1])
         p.set_option(xcb.OPT_I8_KERNEL, xcb.I8_KERNEL_SIMT)
         assert np.array_equal(p.correlate(xd).cpu().numpy(), ref)
+        p.set_option(xcb.OPT_I8_KERNEL, xcb.I8_KERNEL_AUTO)
+        p.set_option(xcb.OPT_FORCE_STAGE, 1)                    # the staging kernels read pitched rows too (any N)
+        assert np.array_equal(p.correlate(xd).cpu().numpy(), ref)
+        assert p.last_launches == 2
         p.close()
 
 
