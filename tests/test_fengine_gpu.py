@@ -216,4 +216,11 @@ def test_cube_other_config_shapes_sampled(N, F, T):
             assert (d[m > scale * tol(F)] == 0).all() and np.abs(d).max() <= 1, (s, pol, t, c)
             nbad += int((d != 0).sum())
     assert nbad <= 3
+    # the chain: xc_fx's cube is the one xc_fengine writes, and its visibilities are the X-engine's on that very cube
+    cube = p.new_cube()
+    vis = p.fx(torch.from_numpy(volt).cuda(), scale, cube)
+    torch.cuda.synchronize()
+    assert np.array_equal(cube.cpu().numpy()[:, :, :4 * N].reshape(T, F, N, 2, 2), got)
+    p.set_in_pitch(p.scratch_pitch)
+    assert torch.equal(p.correlate(cube), vis)
     p.close()
