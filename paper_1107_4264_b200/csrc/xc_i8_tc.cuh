@@ -182,11 +182,14 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
     constexpr uint32_t TMEM_COLS = 2 * UMMA_N;                         // 512 or 256: a power of two >= 32
     constexpr bool CLUSTER = (CG == 2 || TS == 2);
 
-    if (p.stamps && threadIdx.x == 0) {
+    // timing stamps are taken by the last epilogue warp, which has nothing to do until the first accumulator is complete:
+    // reading %globaltimer takes several hundred cycles and must not sit in the producer's or the issuer's path
+    if (p.stamps && threadIdx.x == TC_THREADS - 32) {
+        const unsigned long long c = static_cast<unsigned long long>(clock64());
         const unsigned long long gt = globaltimer_ns();
         atomicMin(p.stamps + 0, gt);
         if (blockIdx.x == 0) {
-            p.stamps[2] = static_cast<unsigned long long>(clock64());
+            p.stamps[2] = c;
             p.stamps[3] = gt;
         }
     }
@@ -457,11 +460,12 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
         tc_fence_after();
         tmem_dealloc<CG>(tmem_base, TMEM_COLS);
     }
-    if (p.stamps && threadIdx.x == 0) {
+    if (p.stamps && threadIdx.x == TC_THREADS - 32) {
+        const unsigned long long c = static_cast<unsigned long long>(clock64());
         const unsigned long long gt = globaltimer_ns();
         atomicMax(p.stamps + 1, gt);
         if (blockIdx.x == 0) {
-            p.stamps[4] = static_cast<unsigned long long>(clock64());
+            p.stamps[4] = c;
             p.stamps[5] = gt;
         }
     }
