@@ -244,7 +244,7 @@ int xc_correlate_host_i4(xc_plan_t* plan, const uint8_t* in4_host, int32_t* vis_
  *   volt_dev: int8 [N][2 pol][T*F samples][2 re,im], station-major time series (2-byte aligned); xc_volt_bytes().
  *   cube_dev: int8 rows (t, f) of 4N valid bytes, cube_pitch bytes apart (a multiple of 4, >= 4N; 0 = xc_scratch_pitch(),
  *   the 128-byte multiple the X-engine reads fastest; xc_cube_bytes() is the size at that pitch); 4-byte aligned.
- *   F must be a power of two <= 4096, else XC_ERR_UNSUPPORTED.  fp32 arithmetic (Stockham FFT, radix <= 16): the
+ *   F must be a power of two <= 4096, else XC_ERR_UNSUPPORTED.  fp32 arithmetic (Stockham FFT, radix <= 32): the
  *   spectrum agrees with an fp64 DFT to about 1e-6 relative to sqrt(F) * max|volt|, so a quantised sample can differ by one
  *   step from an exact evaluation only where X * scale lies within that distance of a rounding boundary k + 1/2; the
  *   bins f = 0, F/4, F/2, 3F/4 of integer input are exact, ties included.

@@ -12,7 +12,8 @@
 //
 // How: the work is bandwidth- and ALU-shaped, not a dense contraction -- CUDA cores, fp32.  One CTA owns SB stations x 2
 // polarisations x TT time blocks.  Its 256 threads transform G = 256 / (F / RMAX) signals at a time with a Stockham
-// autosort FFT: ceil(log2 F / 4) passes of radix <= 16, every pass a register-resident butterfly per thread, passes
+// autosort FFT: ceil(log2 F / 4) passes of radix <= 16 (F = 512, 1024: two passes, the first of radix 32), every pass a
+// register-resident butterfly per thread, passes
 // exchanged through a shared-memory work buffer; the first pass reads the int8 samples straight from global memory, the
 // last pass scales, rounds and drops its 2-byte results into a shared-memory tile [signal][tt * F + f] (column-major: a
 // thread's outputs sit at compile-time offsets from one base; columns are padded by 4 bytes so that the row-wise read-out
