@@ -239,7 +239,7 @@ int fe_prepare(xc_plan_t* p) {
     const int L = p->logf, NP = xc::fe_num_passes(L);
     int ns = 1;
     for (int i = 0; i < NP; ++i) {
-        const int R = 1 << (L / NP + (i < L % NP ? 1 : 0));
+        const int R = 1 << xc::fe_pass_bits(L, i);
         if (i >= 1)
             for (int k = 0; k < ns; ++k)
                 for (int r = 1; r < R; ++r) {

@@ -51,21 +51,23 @@ struct FeParams {
     float scale;
 };
 
-// number of passes for F = 2^logf (host mirror of FeCfg<LOGF>::NP, for the twiddle-table layout)
-inline int fe_num_passes(int logf) {
-    const int maxb = (XC_FE_RADIX32 && (logf == 9 || logf == 10)) ? 5 : 4;
-    return (logf + maxb - 1) / maxb;
+// How log2 F bits are split over the passes (one table for the kernel templates and for the host's twiddle layout):
+// at most 4 bits per pass (radix 16), balanced, the first passes one bit wider -- except that F = 512 and 1024 use a radix-32
+// first pass so that they need two passes instead of three (the kernel is bound by the shared-memory traffic of the passes,
+// profiles/r2_ncu_fengine.md): measured 0.624 against 0.648 ms (F = 512) and 0.623 against 0.645 ms (F = 1024); F = 32 in one
+// radix-32 pass was slower (0.56 vs 0.32 ms), and F = 64 as 16 x 4 instead of 8 x 8 too (0.62 vs 0.59 ms at N = 1024, T = 2048).
+__host__ __device__ constexpr int fe_num_passes(int logf) {
+    return (logf + ((XC_FE_RADIX32 && (logf == 9 || logf == 10)) ? 5 : 4) - 1) / ((XC_FE_RADIX32 && (logf == 9 || logf == 10)) ? 5 : 4);
+}
+__host__ __device__ constexpr int fe_pass_bits(int logf, int i) {
+    return fe_num_passes(logf) ? logf / fe_num_passes(logf) + (i < logf % fe_num_passes(logf) ? 1 : 0) : 0;
 }
 
 template <int LOGF>
 struct FeCfg {
     static constexpr int F = 1 << LOGF;
-    // bits per pass: at most 4 (radix 16), except that F = 512 and 1024 use radix 32 so that they need two passes instead of
-    // three (the kernel is bound by the shared-memory traffic of the passes, profiles/r2_ncu_fengine.md): measured 0.624
-    // against 0.648 ms (F = 512) and 0.623 against 0.645 ms (F = 1024); F = 32 in one radix-32 pass was slower (0.56 vs 0.32 ms).
-    static constexpr int MAXB = (XC_FE_RADIX32 && (LOGF == 9 || LOGF == 10)) ? 5 : 4;
-    static constexpr int NP = (LOGF + MAXB - 1) / MAXB;                      // passes (0 for F = 1)
-    static constexpr int bits(int i) { return NP ? LOGF / NP + (i < LOGF % NP ? 1 : 0) : 0; }
+    static constexpr int NP = fe_num_passes(LOGF);                           // passes (0 for F = 1)
+    static constexpr int bits(int i) { return fe_pass_bits(LOGF, i); }
     static constexpr int RMAX = 1 << bits(0);                                // points per thread
     static constexpr int TPS = F / RMAX;                                     // threads per signal
     static constexpr int G = FE_THREADS / TPS;                               // signals per sub-batch
