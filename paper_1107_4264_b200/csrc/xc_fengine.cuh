@@ -77,6 +77,14 @@ struct FeCfg {
     static constexpr int TW_BYTES = TW_N * 8;
     static constexpr int ns(int i) { return i == 0 ? 1 : ns(i - 1) << bits(i - 1); }   // product of the radices before pass i
     static constexpr int tw_off(int i) { return i <= 1 ? 0 : tw_off(i - 1) + ns(i - 1) * ((1 << bits(i - 1)) - 1); }
+    // Two-pass transforms whose second pass needs at most 16 twiddles per thread keep them in registers for the CTA's whole
+    // life (they depend on the thread only, not on the signal): a quarter of the kernel's shared-memory wavefronts were
+    // twiddle loads (profiles/r2_ncu_fengine.md).  Measured: F = 64 0.595 -> 0.550 ms, F = 32 0.648 -> 0.605, F = 256
+    // 0.533 -> 0.523; F = 128 (14 twiddles, 98 registers) got slower (0.558 -> 0.591) and F = 512 / 1024 would need 60.
+    static constexpr int R1 = 1 << bits(1);
+    static constexpr int NB1 = RMAX / R1;
+    static constexpr bool TW_REGS = (NP == 2) && (NB1 * (R1 - 1) <= 8 || LOGF == 8);
+    static constexpr int TWR_B = TW_REGS ? NB1 : 1, TWR_R = TW_REGS ? R1 - 1 : 1;
     static_assert(TPS <= FE_THREADS && TPS >= 1, "threads per signal");
 };
 
@@ -277,10 +285,15 @@ struct FePass {
             for (int r = 0; r < R; ++r) v[b][r] = pb[padc(r * STRIDE)];
         }
     }
-    static __device__ __forceinline__ void compute(float2 (&v)[NB][R], const float2* tw, int ts) {
+    // twr: this thread's twiddles of pass 1 in registers (FeCfg::TW_REGS), else unused
+    static __device__ __forceinline__ void compute(float2 (&v)[NB][R], const float2* tw, int ts,
+                                                   const float2 (&twr)[C::TWR_B][C::TWR_R]) {
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-            if (NS > 1) {
+            if constexpr (C::TW_REGS && PASS == 1) {
+#pragma unroll
+                for (int r = 1; r < R; ++r) v[b][r] = cmul(v[b][r], twr[b][r - 1]);
+            } else if (NS > 1) {
                 const float2* tk = tw + TW_OFF + ((ts + b * C::TPS) & (NS - 1)) * (R - 1);  // row k of this pass's table
 #pragma unroll
                 for (int r = 1; r < R; ++r) v[b][r] = cmul(v[b][r], tk[r - 1]);
@@ -307,11 +320,12 @@ struct FeRun {
     // Runs passes PASS .. NP-1 for this thread; `sink(f, value)` takes the final spectrum samples.
     // `raw`: pass 0's samples, fetched one sub-batch ahead by the caller (unused by the later passes)
     template <typename Raw, typename Sink>
-    static __device__ __forceinline__ void run(const Raw& raw, float2* buf, const float2* tw, int ts, Sink&& sink) {
+    static __device__ __forceinline__ void run(const Raw& raw, float2* buf, const float2* tw, int ts,
+                                               const float2 (&twr)[C::TWR_B][C::TWR_R], Sink&& sink) {
         float2 v[P::NB][P::R];
         if constexpr (PASS == 0) P::convert(v, raw);
         else P::load_smem(v, buf, ts);
-        P::compute(v, tw, ts);
+        P::compute(v, tw, ts, twr);
         if constexpr (PASS >= C::NP - 1) {        // (>=: F = 1 has no pass at all and is its own spectrum)
 #pragma unroll
             for (int b = 0; b < P::NB; ++b)
@@ -322,7 +336,7 @@ struct FeRun {
             if (PASS > 0) __syncthreads();         // everybody has read the buffer
             P::store_smem(v, buf, ts);
             __syncthreads();
-            FeRun<LOGF, PASS + 1>::run(raw, buf, tw, ts, sink);
+            FeRun<LOGF, PASS + 1>::run(raw, buf, tw, ts, twr, sink);
         }
     }
 };
@@ -364,6 +378,16 @@ __global__ void __launch_bounds__(FE_THREADS) xc_fengine_kernel(const FeParams p
         t = t0 + tt;
         return (q < nq) && (s < p.N) && (t < p.T);
     };
+    float2 twr[C::TWR_B][C::TWR_R];
+    if constexpr (C::TW_REGS) {
+        using P1 = FePass<LOGF, 1>;
+#pragma unroll
+        for (int b = 0; b < C::NB1; ++b)
+#pragma unroll
+            for (int r = 1; r < C::R1; ++r) twr[b][r - 1] = tw[P1::TW_OFF + ((ts + b * C::TPS) & (P1::NS - 1)) * (C::R1 - 1) + r - 1];
+    } else {
+        twr[0][0] = make_float2(0.f, 0.f);
+    }
     using P0 = FePass<LOGF, 0>;
     uint32_t raw[P0::NB][P0::R];            // pass 0's samples of the NEXT sub-batch: their latency hides behind this one
     {
@@ -390,7 +414,7 @@ __global__ void __launch_bounds__(FE_THREADS) xc_fengine_kernel(const FeParams p
             auto sink = [&](int f, float2 X) {
                 if (ok) dst[f * fstride] = X;
             };
-            FeRun<LOGF, 0>::run(cur, buf, tw, ts, sink);
+            FeRun<LOGF, 0>::run(cur, buf, tw, ts, twr, sink);
         } else {
             // column sp, row tt * F: the thread's outputs f = j + r * NS land at compile-time offsets from here
             uint16_t* col = reinterpret_cast<uint16_t*>(tile + static_cast<uint32_t>(sp) * CS) + tt * F;
@@ -399,7 +423,7 @@ __global__ void __launch_bounds__(FE_THREADS) xc_fengine_kernel(const FeParams p
             auto sink = [&](int f, float2 X) {
                 if (inq) col[f] = static_cast<uint16_t>(fe_quant2(mul2(X, sc2)));      // one rounding per component, like __fmul_rn
             };
-            FeRun<LOGF, 0>::run(cur, buf, tw, ts, sink);
+            FeRun<LOGF, 0>::run(cur, buf, tw, ts, twr, sink);
         }
     }
     if constexpr (SPEC) return;
