@@ -224,3 +224,27 @@ def test_cube_other_config_shapes_sampled(N, F, T):
     p.set_in_pitch(p.scratch_pitch)
     assert torch.equal(p.correlate(cube), vis)
     p.close()
+
+
+def test_random_shapes_fengine_and_fx():
+    """Seeded sweep of ragged shapes (N, power-of-two F, T, cube pitch): the cube against the oracle (near-tie rule), and the
+    X-engine run on that cube equal to xc_fx's visibilities."""
+    rng = np.random.default_rng(20261105)
+    for _ in range(14):
+        N = int(rng.integers(1, 140))
+        F = 1 << int(rng.integers(0, 10))
+        T = int(rng.integers(1, max(2, 3000 // F)))
+        volt = wl.voltages(N, F, T, seed=int(rng.integers(1 << 30)), tones=int(rng.integers(0, 3)), full_range_mix=True)
+        scale = wl.fengine_scale(F) * float(rng.choice([0.5, 1.0, 4.0]))
+        ref_cube, margin = fo.fengine(volt, F, scale)
+        p = xcb.Plan(N, F, T)
+        pitch = p.scratch_pitch if rng.integers(2) else ((4 * N + 15) // 16) * 16
+        check_cube(gpu_cube(p, volt, scale, pitch), ref_cube, margin, F, scale)
+        cube = p.new_cube()
+        vis = p.fx(torch.from_numpy(volt).cuda(), scale, cube)
+        p.set_in_pitch(p.scratch_pitch)
+        assert torch.equal(p.correlate(cube), vis), (N, F, T)
+        got = cube.cpu().numpy()[:, :, :4 * N].reshape(T, F, N, 2, 2)
+        if np.array_equal(got, ref_cube):                     # no near-tie flipped: then the chain must match the oracles bit for bit
+            assert np.array_equal(vis.cpu().numpy(), xo.correlate_i8(ref_cube)), (N, F, T)
+        p.close()
