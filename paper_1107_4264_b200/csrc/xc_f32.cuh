@@ -22,8 +22,16 @@
 
 namespace xc {
 
-constexpr int F32_SI = 32;       // stations per tile on the i side
-constexpr int F32_SJ = 64;       // stations per tile on the j side
+#ifndef XC_F32_TI
+#define XC_F32_TI 2
+#endif
+constexpr int F32_TI = XC_F32_TI;            // stations per thread on the i side (x 4 on the j side)
+constexpr int F32_LI = 16 / F32_TI;          // lanes of a warp along i; the warp's block is 16 stations tall
+constexpr int F32_LJ = 32 / F32_LI;          // lanes along j
+constexpr int F32_WBJ = 4 * F32_LJ;          // stations of a warp's block along j
+constexpr int F32_SI = 16 * F32_TI;          // stations per tile on the i side
+constexpr int F32_SJ = 64;                   // stations per tile on the j side
+constexpr int F32_WI = F32_SI / 16;          // warps along i
 #ifndef XC_F32_BK
 #define XC_F32_BK 16
 #endif
@@ -31,7 +39,7 @@ constexpr int F32_SJ = 64;       // stations per tile on the j side
 #define XC_F32_STAGES 3
 #endif
 #ifndef XC_F32_MINB
-#define XC_F32_MINB 2
+#define XC_F32_MINB (XC_F32_TI == 2 ? 2 : 1)
 #endif
 constexpr int F32_BK = XC_F32_BK;       // samples per ring stage
 constexpr int F32_STAGES = XC_F32_STAGES;
@@ -100,8 +108,8 @@ __global__ void __launch_bounds__(F32_THREADS, XC_F32_MINB) xc_f32_kernel(const 
     // i > j) or beyond N skips the arithmetic -- it still loads and synchronises -- so diagonal tiles cost what
     // they store at 16-station granularity, and the co-resident CTA's warps take the freed issue slots.
     const int warp = tid >> 5, lane = tid & 31;
-    const int ti = 16 * (warp & 1) + (lane & 7);    // stations i0 + ti, i0 + ti + 8
-    const int tj = 16 * (warp >> 1) + (lane >> 3);  // stations j0 + tj + 4 n, n = 0..3
+    const int ti = 16 * (warp % F32_WI) + (lane % F32_LI);       // stations i0 + ti + F32_LI a, a < F32_TI
+    const int tj = F32_WBJ * (warp / F32_WI) + (lane / F32_LI);  // stations j0 + tj + F32_LJ n, n = 0..3
 
     const long long w = blockIdx.x;
     const int f = static_cast<int>(w / p.tiles_per_f);
@@ -128,9 +136,9 @@ __global__ void __launch_bounds__(F32_THREADS, XC_F32_MINB) xc_f32_kernel(const 
         }
     };
 
-    float2 acc[2][4][4];
+    float2 acc[F32_TI][4][4];
 #pragma unroll
-    for (int a = 0; a < 2; ++a)
+    for (int a = 0; a < F32_TI; ++a)
 #pragma unroll
         for (int b = 0; b < 4; ++b)
 #pragma unroll
@@ -143,8 +151,8 @@ __global__ void __launch_bounds__(F32_THREADS, XC_F32_MINB) xc_f32_kernel(const 
     }
 
     // warp-uniform: does this warp's 16 x 16 block hold any stored pair (i <= j < N)?
-    const int wi0 = i0 + 16 * (warp & 1), wj0 = j0 + 16 * (warp >> 1);
-    const bool active = (wi0 <= wj0 + 15) && (wi0 < p.N) && (wj0 < p.N);
+    const int wi0 = i0 + 16 * (warp % F32_WI), wj0 = j0 + F32_WBJ * (warp / F32_WI);
+    const bool active = (wi0 <= wj0 + F32_WBJ - 1) && (wi0 < p.N) && (wj0 < p.N);
 
     for (int kb = 0; kb < KB; ++kb) {
         cp_async_wait<F32_STAGES - 2>();
@@ -156,11 +164,10 @@ __global__ void __launch_bounds__(F32_THREADS, XC_F32_MINB) xc_f32_kernel(const 
 #pragma unroll
         for (int k = 0; k < F32_BK; ++k) {
             const float4* row = sA + k * (F32_SI + F32_SJ);
-            const float4 a0 = row[ti], a1 = row[ti + 8];
-            const float4 b0 = row[F32_SI + tj], b1 = row[F32_SI + tj + 4];
-            const float4 b2 = row[F32_SI + tj + 8], b3 = row[F32_SI + tj + 12];
-            cmac_row(acc[0], a0, b0, b1, b2, b3);
-            cmac_row(acc[1], a1, b0, b1, b2, b3);
+            const float4 b0 = row[F32_SI + tj], b1 = row[F32_SI + tj + F32_LJ];
+            const float4 b2 = row[F32_SI + tj + 2 * F32_LJ], b3 = row[F32_SI + tj + 3 * F32_LJ];
+#pragma unroll
+            for (int a = 0; a < F32_TI; ++a) cmac_row(acc[a], row[ti + F32_LI * a], b0, b1, b2, b3);
         }
     }
     cp_async_wait<0>();
@@ -168,10 +175,10 @@ __global__ void __launch_bounds__(F32_THREADS, XC_F32_MINB) xc_f32_kernel(const 
     float* visf = p.vis + static_cast<long long>(f) * p.NB * 8;
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
-        const int j = j0 + tj + 4 * b;
+        const int j = j0 + tj + F32_LJ * b;
 #pragma unroll
-        for (int a = 0; a < 2; ++a) {
-            const int i = i0 + ti + 8 * a;
+        for (int a = 0; a < F32_TI; ++a) {
+            const int i = i0 + ti + F32_LI * a;
             if (i <= j && j < p.N) {
                 float4* dst = reinterpret_cast<float4*>(visf + (static_cast<long long>(j) * (j + 1) / 2 + i) * 8);
                 float4 lo = make_float4(acc[a][b][0].x, acc[a][b][0].y, acc[a][b][1].x, acc[a][b][1].y);
