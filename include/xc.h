@@ -96,6 +96,10 @@ typedef enum {
     XC_OPT_TSPLIT = 8      /* T-split of the single-CTA tile over a cluster of 2 (the paper's small-N future    */
                            /* work): 0 = auto (on when 2 * tiles * F <= SM count and T >= 8192: */
                            /* the hand-over costs ~3 us), 1 = off, 2 = on whenever T allows it.  Same bits either way. */
+    , XC_OPT_ORIGIN_SHIFT = 9 /* 1 (default) = when the rows of the block are not 128 bytes apart (dense N % 32 != 0) but */
+                           /* row pitch x F is, move every channel's tile grid left by the offset of its rows inside   */
+                           /* their 128-byte line, so that TMA fetches whole lines ("rows aligned to   */
+                           /* the memory line"); 0 = off (for comparison).  Same bits either way.                       */
 #ifdef XC_PROFILE
     , XC_OPT_DEBUG_SKIP = 3 /* PROFILING BUILD ONLY (-DXC_PROFILE), results become meaningless: bit 0 = no TMA */
                             /* loads after the first ring fill, bit 1 = no MMAs, bit 2 = no stores, bit 3 =    */
@@ -275,6 +279,11 @@ int xc_tile_count(const xc_plan_t* plan);
 int xc_tile_get(const xc_plan_t* plan, int k, int* bi, int* bj, int* si, int* sj);
 /* T-split factor (1 or 2) used by the last integer compute call on this plan (see XC_OPT_TSPLIT). */
 int xc_t_split(const xc_plan_t* plan);
+/* Origin shift used by the last integer compute call on this plan (see XC_OPT_ORIGIN_SHIFT): returns the period P (1, 2,
+ * 4 or 8 channels; 0 for a null plan) and fills, for c < P, shift_bytes[c] (grid of channels f = c mod P moved left by so
+ * many bytes = 4 x stations; 0 = not moved) and tiles[c] (tiles scheduled for such a channel).  Either array may be NULL,
+ * else it holds 8 ints. */
+int xc_origin_shift(const xc_plan_t* plan, int* shift_bytes, int* tiles);
 
 /* The paper's closed-form triangular map and its inverse:
  *   g = by(by+1)/2 + bx,  by = floor(-1/2 + sqrt(1/4 + 2g)),  bx = g - by(by+1)/2,

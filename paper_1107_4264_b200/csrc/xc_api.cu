@@ -51,6 +51,8 @@ struct xc_plan_s {
     int tile_mode = 0;      // XC_TILE_*: shape of the tensor-core tile actually in use
     int t_split = 1;        // CTAs sharing one tile's time axis (single-CTA tile only): 1 or 2
     std::vector<uint32_t> tiles_tc, tiles_f32;
+    std::vector<uint32_t> tiles_tc_ext;                  // the same schedule with one more block row (origin shift): tiles_tc is its prefix
+    int shift_period = 1, shift_bytes[8] = {0, 0, 0, 0, 0, 0, 0, 0}, shift_tiles[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // what the last call used
     // device state (created lazily on the device current at first compute call)
     bool dev_ready = false, tiles_uploaded = false;
     int device = -1, sm_count = 0;
@@ -64,7 +66,7 @@ struct xc_plan_s {
     bool ws_owned = false;
     cudaEvent_t ev_ws = nullptr;                         // recorded after the last consumer of the staging workspace
     int opt_kernel = XC_I8_KERNEL_AUTO, opt_max_ctas = 0, opt_force_stage = 0, opt_pdl = 1, opt_tsplit = 0;
-    int opt_tile = XC_TILE_AUTO;
+    int opt_tile = XC_TILE_AUTO, opt_origin_shift = 1;
     unsigned long long* stamps = nullptr;                // xc_set_timing_buffer
 #ifdef XC_PROFILE
     int opt_debug_skip = 0;
@@ -133,6 +135,7 @@ void set_tile_mode(xc_plan_t* p, int mode) {
     tile_shape(mode, &si, &sj);
     p->tile_mode = mode;
     p->tiles_tc = build_tiles(p->N, si, sj);
+    p->tiles_tc_ext = build_tiles(p->N + si, si, sj);    // square tiles: block row bj holds bi = 0 .. bj, so tiles_tc is a prefix
     p->tiles_uploaded = false;
 }
 
@@ -147,7 +150,7 @@ int upload_table(xc_plan_t* p, uint32_t** dst, const std::vector<uint32_t>& src)
 
 int upload_tiles(xc_plan_t* p) {
     if (p->tiles_uploaded) return XC_OK;
-    int rc = upload_table(p, &p->d_tiles_tc, p->tiles_tc);
+    int rc = upload_table(p, &p->d_tiles_tc, p->tiles_tc_ext);
     if (rc != XC_OK) return rc;
     p->tiles_uploaded = true;
     return XC_OK;
@@ -439,6 +442,51 @@ int encode_tmap(xc_plan_t* p, const void* src, size_t pitch, int bk, int nf) {
     return XC_OK;
 }
 
+// Origin shift ("rows aligned to the memory line").  Rows of the block TMA reads start at
+// base + f pitch + t pitch F.  When pitch F is a multiple of 128 bytes the offset of a row inside its 128-byte line depends
+// on f only, with a period of at most 8 channels (base and pitch are multiples of 16).  A box row that starts `shift` bytes
+// into a line straddles two lines (two L2 requests, 5 sectors instead of 4: N = 500 ran 31 % slower than with padded
+// rows); moving channel f's whole tile grid `shift` bytes to the left makes every box row exactly one line.  The price is
+// that a class whose 4N + shift bytes need one more block row has more tiles; such a class keeps the unshifted grid when
+// the extra tiles would cost more than the misaligned loads do (x 1.25, measured at N = 500).
+// Fills the per-class fields of tp and the plan's record of them; returns the number of tiles of the nf channels.
+long long plan_origin_shift(xc_plan_t* p, xc::TcParams* tp, const void* base, size_t pitch, int nf) {
+    int si, sj;
+    tile_shape(p->tile_mode, &si, &sj);
+    const int mbytes = 4 * si;                                    // Gram rows (= bytes of a row) per tile
+    const int n0 = (4 * p->N + mbytes - 1) / mbytes;
+    const uintptr_t b = reinterpret_cast<uintptr_t>(base);
+    int per = 1;
+    const bool can = p->opt_origin_shift && ((pitch * static_cast<size_t>(p->F)) % 128u == 0);
+    if (can && (pitch % 128u)) {
+        per = 8;
+        while (per > 1 && ((pitch * static_cast<size_t>(per / 2)) % 128u == 0)) per /= 2;
+    }
+    long long cum = 0;
+    tp->per_n = per;
+    tp->tiles_per_f = 0;
+    tp->per_cum[0] = 0;
+    for (int c = 0; c < 8; ++c) p->shift_bytes[c] = p->shift_tiles[c] = 0;
+    for (int c = 0; c < per; ++c) {
+        int shift = can ? static_cast<int>((b + static_cast<uintptr_t>(c) * pitch) & 127u) : 0;
+        int n = (4 * p->N + shift + mbytes - 1) / mbytes;
+        if (n > n0 && 4LL * n * (n + 1) > 5LL * n0 * (n0 + 1)) {   // more than 1.25 x the tiles: keep the unshifted grid
+            shift = 0;
+            n = n0;
+        }
+        const int tiles = n * (n + 1) / 2;
+        tp->per_shift[c] = static_cast<uint8_t>(shift);
+        cum += tiles;
+        tp->per_cum[c + 1] = static_cast<uint32_t>(cum);
+        if (tiles > tp->tiles_per_f) tp->tiles_per_f = tiles;
+        p->shift_bytes[c] = shift;
+        p->shift_tiles[c] = tiles;
+    }
+    tp->per_total = static_cast<int>(cum);
+    p->shift_period = per;
+    return static_cast<long long>(nf / per) * cum + tp->per_cum[nf % per];
+}
+
 // X-engine on channels [f0, f0 + nf) of the block at in_dev / the cube at vis_dev (both addressed with the plan's F).
 // pitch_override != 0: in_dev is a device block with that row pitch (the host paths' re-pitched scratch, the F-engine's cube).
 int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* stream, int accumulate, int f0 = 0,
@@ -496,12 +544,12 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     tp.debug_skip = p->opt_debug_skip;
     tp.trace = p->trace;
 #endif
-    tp.tiles_per_f = static_cast<int>(p->tiles_tc.size());
+    const long long total = plan_origin_shift(p, &tp, static_cast<const int8_t*>(src) + pitch * static_cast<size_t>(f0), pitch, nf);
     tp.tiles = p->d_tiles_tc;
     if (tp.tiles_per_f <= xc::TC_INLINE_TILES)
-        for (int k = 0; k < tp.tiles_per_f; ++k) tp.tiles_inline[k] = p->tiles_tc[k];
-    if (static_cast<long long>(nf) * tp.tiles_per_f > 0x7FFFFFFFLL) return XC_ERR_UNSUPPORTED;
-    tp.total_tiles = nf * tp.tiles_per_f;
+        for (int k = 0; k < tp.tiles_per_f; ++k) tp.tiles_inline[k] = p->tiles_tc_ext[k];
+    if (total > 0x7FFFFFFFLL) return XC_ERR_UNSUPPORTED;
+    tp.total_tiles = static_cast<int>(total);
     p->t_split = pick_t_split(p, nf, p->opt_max_ctas > 0 ? p->opt_max_ctas : p->sm_count);
     tp.t_split = p->t_split == 2 ? (((p->T + 1) / 2 + 31) & ~31) : p->T;
     if (pair) rc = launch_tc<256, 2, 128, 1>(p, tp, st);
@@ -628,6 +676,9 @@ int xc_set_option(xc_plan_t* p, int option, int value) {
             return XC_OK;
         case XC_OPT_PDL:
             p->opt_pdl = value ? 1 : 0;
+            return XC_OK;
+        case XC_OPT_ORIGIN_SHIFT:
+            p->opt_origin_shift = value ? 1 : 0;
             return XC_OK;
 #ifdef XC_PROFILE
         case XC_OPT_DEBUG_SKIP:
@@ -919,6 +970,15 @@ int xc_tile_get(const xc_plan_t* p, int k, int* bi, int* bj, int* si, int* sj) {
 }
 
 int xc_t_split(const xc_plan_t* p) { return p ? p->t_split : 0; }
+
+int xc_origin_shift(const xc_plan_t* p, int* shift_bytes, int* tiles) {
+    if (!p) return 0;
+    for (int c = 0; c < p->shift_period; ++c) {
+        if (shift_bytes) shift_bytes[c] = p->shift_bytes[c];
+        if (tiles) tiles[c] = p->shift_tiles[c];
+    }
+    return p->shift_period;
+}
 
 int64_t xc_tri_index(int64_t bx, int64_t by) { return by * (by + 1) / 2 + bx; }
 

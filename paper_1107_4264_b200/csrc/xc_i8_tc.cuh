@@ -72,8 +72,16 @@ struct TcCfg {
 
 struct TcParams {
     int N, F, T;
-    int tiles_per_f;          // entries of the tile table per channel
-    int total_tiles;          // F * tiles_per_f
+    int tiles_per_f;          // entries of the tile table (the largest per-channel count of any alignment class)
+    int total_tiles;          // sum over the F channels of their tile counts
+    // Origin shift: when the rows of the block are not 128 bytes apart, channel f's rows start `shift` bytes
+    // past a 128-byte line; its tile grid is then moved `shift` bytes (shift / 4 stations) to the left, so that every box row
+    // is one whole L2 line (coordinates below 0 are TMA zero fill, masked in the epilogue).  The shift depends on
+    // f mod per_n only; class c has per_cum[c + 1] - per_cum[c] tiles (a prefix of the table).
+    int per_n;                // channels per alignment period: 1, 2, 4 or 8
+    int per_total;            // tiles of one period = per_cum[per_n]
+    uint32_t per_cum[9];
+    uint8_t per_shift[8];     // bytes, multiples of 16, < 128
     int t_split;              // T-split: samples per rank (a multiple of 32); T when TS == 1
     long long NB;             // N(N+1)/2
     const uint32_t* tiles;    // device: bi | (bj << 16), in units of (SI, SJ) stations (used if tiles_per_f > TC_INLINE_TILES)
@@ -104,6 +112,21 @@ constexpr int TC_TRACE_ITERS = 256;   // pipeline iterations traced; layout: [3 
 __device__ __forceinline__ int walk(int n, int unit, int nunits, int total) {
     const long long w = static_cast<long long>(unit) + static_cast<long long>(n) * nunits;
     return w < total ? static_cast<int>(w) : -1;
+}
+// Entry w of the tile list -> channel, index into the tile table, origin shift of that channel (in bytes).
+struct TcWork {
+    int f, k, shift;
+};
+__device__ __forceinline__ TcWork tc_locate(const TcParams& p, int w) {
+    TcWork r;
+    const int per = w / p.per_total;
+    const int rem = w - per * p.per_total;
+    int c = 0;
+    while (c + 1 < p.per_n && rem >= static_cast<int>(p.per_cum[c + 1])) ++c;
+    r.f = per * p.per_n + c;
+    r.k = rem - static_cast<int>(p.per_cum[c]);
+    r.shift = static_cast<int>(p.per_shift[c]);
+    return r;
 }
 // Tile table entry k of a channel: from the kernel parameters (constant bank: no global-memory latency in front of the
 // first TMA load, which matters for microsecond-scale launches) or, for long tables, from global memory.
@@ -142,7 +165,7 @@ __device__ __forceinline__ void epi_chunk(const uint32_t (&v)[32], int32_t* __re
         out.z = R2 + I3;   // Re [pi][1]
         out.w = I2 - R3;   // Im [pi][1]
         const int j = jbase + 2 * jp + ci;
-        if ((!MASKED || (i <= j && j < N)) && !NOSTORE) {
+        if ((!MASKED || (i >= 0 && i <= j && j < N)) && !NOSTORE) {
             long long off = (static_cast<long long>(j) * (j + 1) / 2 + i) * 8 + slot;
             if (WRAP) off &= (1 << 21) - 1;   // profiling: keep all stores inside an 8 MB window (L2 resident)
             int4* dst = reinterpret_cast<int4*>(visf + off);
@@ -243,15 +266,19 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
         uint32_t stage = 0, phase = 0;
         int it = 0;
         int w_next = walk(0, unit, nunits, p.total_tiles);
-        uint32_t tb_next = (w_next >= 0) ? tile_at(p, w_next % p.tiles_per_f) : 0u;
+        TcWork wk_next = tc_locate(p, w_next >= 0 ? w_next : 0);
+        uint32_t tb_next = (w_next >= 0) ? tile_at(p, wk_next.k) : 0u;
         for (int n = 0; w_next >= 0; ++n) {
-            const int f = w_next / p.tiles_per_f;
+            const int f = wk_next.f, shift = wk_next.shift;
             const uint32_t tb = __shfl_sync(0xffffffffu, tb_next, 0);
             // the next tile's table entry is fetched now so that its latency hides behind this tile's k loop
             w_next = walk(n + 1, unit, nunits, p.total_tiles);
-            if (w_next >= 0) tb_next = tile_at(p, w_next % p.tiles_per_f);
-            const int m_a = static_cast<int>(tb & 0xFFFFu) * Cfg::M + ((CG == 2) ? 128 * static_cast<int>(rank) : 0);
-            const int m_b = static_cast<int>(tb >> 16) * UMMA_N + ((CG == 2) ? 128 * static_cast<int>(rank) : 0);
+            if (w_next >= 0) {
+                wk_next = tc_locate(p, w_next);
+                tb_next = tile_at(p, wk_next.k);
+            }
+            const int m_a = static_cast<int>(tb & 0xFFFFu) * Cfg::M + ((CG == 2) ? 128 * static_cast<int>(rank) : 0) - shift;
+            const int m_b = static_cast<int>(tb >> 16) * UMMA_N + ((CG == 2) ? 128 * static_cast<int>(rank) : 0) - shift;
             const bool a_in_b = (m_a == m_b);     // diagonal tile: this CTA's A rows are its B rows -- one box serves both
             // A diagonal tile of the single-CTA kernel puts TWO consecutive time slices of its one box into the stage's two
             // slots (2 x BK samples per stage), so that a stage holds 512 tensor cycles like every other tile.
@@ -302,11 +329,11 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
             uint32_t stage = 0, phase = 0, buf = 0, tphase = 0;   // tphase bit b = phase of accumulator b
             int it = 0;
             int w_next = walk(0, unit, nunits, p.total_tiles);
-            uint32_t tb_next = (w_next >= 0) ? tile_at(p, w_next % p.tiles_per_f) : 0u;
+            uint32_t tb_next = (w_next >= 0) ? tile_at(p, tc_locate(p, w_next).k) : 0u;
             for (int n = 0; w_next >= 0; ++n) {
                 const uint32_t tb = __shfl_sync(0xffffffffu, tb_next, 0);
                 w_next = walk(n + 1, unit, nunits, p.total_tiles);
-                if (w_next >= 0) tb_next = tile_at(p, w_next % p.tiles_per_f);
+                if (w_next >= 0) tb_next = tile_at(p, tc_locate(p, w_next).k);
                 const bool a_in_b = ((tb & 0xFFFFu) * Cfg::M == (tb >> 16) * UMMA_N);
                 const uint32_t h0 = (CG == 1 && a_in_b) ? 1u : 0u;
                 // byte offset of the A operand inside a stage: its own box (slot 0), or -- pair kernel on the diagonal -- the B box
@@ -364,16 +391,21 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
         // T-split: this warp's slice of the reduction buffer, [chunk][8 x int4][32 lanes]: a warp access is 512 contiguous bytes
         const uint32_t red_w = red0 + static_cast<uint32_t>(((warp - 2) * CHUNKS) * 4096 + lane * 16);
         int w_next = walk(0, unit, nunits, p.total_tiles);
-        uint32_t tb_next = (w_next >= 0) ? tile_at(p, w_next % p.tiles_per_f) : 0u;
+        TcWork wk_next = tc_locate(p, w_next >= 0 ? w_next : 0);
+        uint32_t tb_next = (w_next >= 0) ? tile_at(p, wk_next.k) : 0u;
         for (int n = 0; w_next >= 0; ++n) {
             XC_TRACE_STAMP(p, blockIdx.x == 0 && warp == 2 && lane == 0, 2, it, 0);
-            const int f = w_next / p.tiles_per_f;
+            const int f = wk_next.f;
+            const int ds = wk_next.shift >> 2;                  // origin shift in stations: the tile grid starts at station -ds
             const uint32_t tb = tb_next;
             w_next = walk(n + 1, unit, nunits, p.total_tiles);
-            if (w_next >= 0) tb_next = tile_at(p, w_next % p.tiles_per_f);
-            const int i0 = static_cast<int>(tb & 0xFFFFu) * Cfg::SI + ((CG == 2) ? 32 * static_cast<int>(rank) : 0) + 8 * q;
+            if (w_next >= 0) {
+                wk_next = tc_locate(p, w_next);
+                tb_next = tile_at(p, wk_next.k);
+            }
+            const int i0 = static_cast<int>(tb & 0xFFFFu) * Cfg::SI + ((CG == 2) ? 32 * static_cast<int>(rank) : 0) + 8 * q - ds;
             const int col0 = 32 * CHUNKS * half;                                     // first accumulator column of this warp
-            const int j0 = static_cast<int>(tb >> 16) * Cfg::SJ + col0 / 4;           // first station of this warp's columns
+            const int j0 = static_cast<int>(tb >> 16) * Cfg::SJ + col0 / 4 - ds;      // first station of this warp's columns
             const int i = i0 + (lane >> 2);                     // i0 = first station of this warp's rows
             int32_t* visf = p.vis + static_cast<long long>(f) * p.NB * 8;
 
@@ -407,7 +439,7 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
 #pragma unroll 1
                 for (int cc = 0; cc < CHUNKS; ++cc) {
                     const int jbase = j0 + 8 * cc;
-                    if (jbase >= p.N || jbase + 7 < i0) continue;  // warp-uniform: nothing of this chunk is stored
+                    if (jbase >= p.N || jbase + 7 < i0 || jbase + 7 < 0) continue;  // warp-uniform: nothing of this chunk is stored
                     uint32_t v[32];
                     tmem_ld_32x32(taddr0 + static_cast<uint32_t>(32 * cc), v);
                     tmem_ld_wait();
@@ -421,7 +453,7 @@ __device__ __forceinline__ void tc_body(const CUtensorMap& tmap, const TcParams&
                             v[4 * k + 3] += static_cast<uint32_t>(o.w);
                         }
                     }
-                    const bool full = (i0 + 7 <= jbase) && (jbase + 7 < p.N);  // warp-uniform: no masking needed
+                    const bool full = (i0 >= 0) && (i0 + 7 <= jbase) && (jbase + 7 < p.N);  // warp-uniform: no masking needed
 #ifdef XC_PROFILE
                     if (p.debug_skip & 4) { epi_chunk<true, false, true>(v, visf, i, jbase, p.N, lane); continue; }
                     if (p.debug_skip & 8) { epi_chunk<true, false, false, true>(v, p.vis, i, jbase, p.N, lane); continue; }

@@ -316,6 +316,62 @@ def test_random_shapes_auto_mode():
         p.close()
 
 
+@pytest.mark.parametrize("N,F,T", [(100, 8, 200), (500, 8, 150), (36, 16, 300), (68, 32, 64), (12, 8, 33), (500, 16, 40)])
+def test_origin_shift_unaligned_pitch(N, F, T):
+    """Dense blocks whose rows are not 128 bytes apart while pitch x F is (XC_OPT_ORIGIN_SHIFT; PAPER.md:112,
+    149): every channel's tile grid is moved left by the offset of its rows inside their 128-byte line.  Bit-exact against
+    the oracle in both tile shapes, with and without T-split, overwrite and accumulate, on a channel sub-range (whose base
+    address changes the shifts), every output written; the unshifted schedule gives the same cube."""
+    assert (4 * N) % 128 != 0 and (4 * N * F) % 128 == 0
+    x = wl.full_range(N, F, T, seed=3 * N + F)
+    ref = xo.correlate_i8(x)
+    xd = torch.from_numpy(x).cuda()
+    for tile, ts in [(xcb.TILE_AUTO, 0), (xcb.TILE_2CTA_256x256, 0), (xcb.TILE_1CTA_128x128, 1), (xcb.TILE_1CTA_128x128, 2)]:
+        p = xcb.Plan(N, F, T)
+        p.set_option(xcb.OPT_TILE, tile)
+        p.set_option(xcb.OPT_TSPLIT, ts)
+        vis = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+        p.correlate(xd, vis)
+        used = p.origin_shift
+        assert len(used) > 1 and any(sh for sh, _ in used), used             # the shifted schedule really ran
+        assert all(sh % 16 == 0 and 0 <= sh < 128 for sh, _ in used)
+        assert np.array_equal(vis.cpu().numpy(), ref), (tile, ts)
+        p.correlate_acc(xd, vis)
+        assert np.array_equal(vis.cpu().numpy(), 2 * ref), (tile, ts, "acc")
+        # a channel sub-range starts at another address: other shifts, same numbers
+        if F >= 8:
+            vis.fill_(0x5A5A5A5A)
+            p.correlate_channels(xd, vis, 3, F - 4)
+            got = vis.cpu().numpy()
+            assert np.array_equal(got[3:F - 1], ref[3:F - 1]), (tile, ts, "sub-range")
+            assert (got[:3] == 0x5A5A5A5A).all() and (got[F - 1:] == 0x5A5A5A5A).all()
+        # origin shift off: the round-1 schedule, same cube
+        p.set_option(xcb.OPT_ORIGIN_SHIFT, 0)
+        v0 = p.correlate(xd)
+        assert p.origin_shift == [(0, len(p.tiles()))]
+        assert np.array_equal(v0.cpu().numpy(), ref)
+        p.close()
+
+
+def test_origin_shift_misaligned_base_pointer():
+    """A block whose rows ARE 128 bytes apart but whose base address is not line-aligned: one shift for all channels."""
+    N, F, T = 96, 3, 200         # 384-byte rows: 384 + 112 still fits the pair tile's two block rows
+    x = wl.full_range(N, F, T, seed=77)
+    ref = xo.correlate_i8(x)
+    buf = torch.zeros(x.size + 256, dtype=torch.int8, device="cuda")
+    for off in (16, 48, 112):
+        base = (-buf.data_ptr()) % 128 + off
+        xd = buf[base:base + x.size].view(T, F, N, 2, 2)
+        xd.copy_(torch.from_numpy(x))
+        p = xcb.Plan(N, F, T)
+        p.set_option(xcb.OPT_TILE, xcb.TILE_2CTA_256x256)
+        vis = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+        p.correlate(xd, vis)
+        assert p.origin_shift == [(off, 3)]
+        assert np.array_equal(vis.cpu().numpy(), ref), off
+        p.close()
+
+
 @pytest.mark.parametrize("N,F,T", [(1, 1, 1), (3, 2, 17), (8, 3, 40), (16, 2, 129), (37, 2, 100), (64, 3, 257), (100, 2, 130),
                                    (136, 1, 300)])
 def test_i4_small_shapes(N, F, T):
