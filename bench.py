@@ -322,7 +322,7 @@ def main():
     ap.add_argument("--no-sustained", action="store_true", help="skip the sustained legs")
     ap.add_argument("--sustained-seconds", type=float, default=2.0)
     ap.add_argument("--pitch", type=int, default=0, help="profiling aid: run the workload from a block with this row pitch")
-    ap.add_argument("--only", default="", choices=["", "f32", "fengine", "trace"],
+    ap.add_argument("--only", default="", choices=["", "f32", "f32tc", "fengine", "trace"],
                     help="profiling aid: run only a few launches of that leg (for ncu) and print a short JSON line; trace = pipeline "
                          "timeline of CTA 0 from the -DXC_PROFILE build")
     args = ap.parse_args()

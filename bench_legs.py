@@ -60,7 +60,10 @@ def cublas_int8_peak(stream):
         return {"cublas_int8_burst": None, "cublas_int8_sustained": None, "cublas_int8_how": f"unavailable: {e!r}"}
 
 
-def f32_leg(stream, clocks, F=None, launches=5):
+def f32_leg(stream, clocks, F=None, launches=5, peaks=None, kernel=None):
+    """xc_correlate_f32 on config 3's values as float32: the tensor-core kernel (three TF32 MMAs per product; what AUTO runs at
+    this N) with a tensor roofline, and the CUDA-core kernel (packed FMAs, the paper's scheme) with its ALU roofline.
+    kernel = "tc" / "cuda_cores": only that one (ncu captures)."""
     import torch
     import paper_1107_4264_b200 as xcb
     import xc_workloads as wl
@@ -70,18 +73,34 @@ def f32_leg(stream, clocks, F=None, launches=5):
     x3 = torch.from_numpy(wl.make_input(w3)).cuda().to(torch.float32)
     p3 = xcb.Plan(w3.N, w3.F, w3.T)
     v3 = p3.new_vis(torch.float32)
-    ms = _timed(lambda: p3.correlate_f32(x3, v3, stream=stream), stream, launches)
     sms = torch.cuda.get_device_properties(0).multi_processor_count
-    fp32_peak = sms * 128 * 2 * ((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
-    out = {"workload": f"cfg3 values (N={w3.N}, F={w3.F}, T={w3.T}) as float32 through xc_correlate_f32", "kernel_ms": ms,
-           "tflops": w3.ops / (ms * 1e-3) / 1e12, "bound": "alu", "peak_tflops": fp32_peak,
-           "frac": w3.ops / (ms * 1e-3) / 1e12 / fp32_peak,
-           "peak_source": "SMs x 128 FMA/clk x 2 x clocks.max.sm (derived, DESIGN.md 5.2)"}
+    out = {"workload": f"cfg3 values (N={w3.N}, F={w3.F}, T={w3.T}) as float32 through xc_correlate_f32"}
+    in_bytes, vis_bytes = 16.0 * w3.N * w3.F * w3.T, 32.0 * (w3.N * (w3.N + 1) // 2) * w3.F
+    if kernel in (None, "tc"):
+        p3.set_option(xcb.OPT_F32_KERNEL, xcb.F32_KERNEL_TC)
+        ms = _timed(lambda: p3.correlate_f32(x3, v3, stream=stream), stream, launches)
+        bf16 = (peaks or {}).get("bf16_burst") or 1590.0
+        tf32x3 = bf16 * 0.5 / 3.0
+        out.update({"kernel": "xc_f32_tc_kernel (tcgen05 kind::tf32, hi/lo split: 3 MMAs per product)", "kernel_ms": ms,
+                    "tflops": w3.ops / (ms * 1e-3) / 1e12, "bound": "tensor", "peak_tflops": tf32x3,
+                    "frac": w3.ops / (ms * 1e-3) / 1e12 / tf32x3,
+                    "peak_source": "bf16_tflops (burst, MEASURED_PEAKS.json) x 0.5 (nominal tf32/bf16 ratio) / 3 (MMAs per product): "
+                                   "useful fp32-equivalent flops; NOT a measured tf32 number",
+                    "hbm_gbs": (in_bytes + vis_bytes) / (ms * 1e-3) / 1e9, "algorithmic_bytes": in_bytes + vis_bytes})
+    if kernel in (None, "cuda_cores"):
+        p3.set_option(xcb.OPT_F32_KERNEL, xcb.F32_KERNEL_CUDA_CORES)
+        ms = _timed(lambda: p3.correlate_f32(x3, v3, stream=stream), stream, launches)
+        fp32_peak = sms * 128 * 2 * ((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+        cc = {"kernel": "xc_f32_kernel (CUDA cores, packed fma.rn.f32x2; the paper's register tiling)", "kernel_ms": ms,
+              "tflops": w3.ops / (ms * 1e-3) / 1e12, "bound": "alu", "peak_tflops": fp32_peak,
+              "frac": w3.ops / (ms * 1e-3) / 1e12 / fp32_peak,
+              "peak_source": "SMs x 128 FMA/clk x 2 x clocks.max.sm (derived, DESIGN.md 5.2)"}
+        if F is None:
+            cc["fma_issue_probe"] = fma_probe()
+        out["cuda_cores"] = cc
     p3.close()
     del x3, v3
     torch.cuda.empty_cache()
-    if F is None:
-        out["fma_issue_probe"] = fma_probe()
     return out
 
 
@@ -162,7 +181,9 @@ def only_leg(which, workload, stream):
         import os
         return {"only": "trace", **trace_leg(workload, stream, int(os.environ.get("XC_TRACE_SKIP", "0")))}
     if which == "f32":
-        return {"only": "f32", **f32_leg(stream, None, F=32, launches=3)}
+        return {"only": "f32", **f32_leg(stream, None, F=32, launches=3, kernel="cuda_cores")}
+    if which == "f32tc":
+        return {"only": "f32tc", **f32_leg(stream, None, F=128, launches=3, kernel="tc")}
     if which == "fengine":
         return {"only": "fengine", **fengine_leg(stream, workload, launches=3, with_fx=False)}
     raise ValueError(which)
@@ -182,7 +203,7 @@ def extras(stream, clocks, sampler, peaks):
     import xc_workloads as wl
     out = {}
     # ---- S5: fp32-input variant on config 3's values (BASELINE.json configs[2]); ALU-bound ------------------
-    out["f32"] = f32_leg(stream, clocks)
+    out["f32"] = f32_leg(stream, clocks, peaks=peaks)
 
     # ---- N = 500 from a block with 128-byte-multiple rows (xc_set_in_pitch; what the F-engine / the host paths produce) ----
     w5 = wl.CONFIGS["cfg5_N500"]

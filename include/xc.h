@@ -78,6 +78,12 @@ enum {
     XC_I8_KERNEL_SIMT = 2  /* plain CUDA-core kernel, one thread per baseline: a debugging    */
                            /* aid that shares no device code with the tensor-core kernel     */
 };
+/* Kernels of the fp32 path, xc_set_option(XC_OPT_F32_KERNEL, ...). */
+enum {
+    XC_F32_KERNEL_AUTO = 0,       /* tensor cores for N >= 48, CUDA cores below                                      */
+    XC_F32_KERNEL_CUDA_CORES = 1, /* the paper's own scheme: register tile of station pairs per thread, packed FMAs  */
+    XC_F32_KERNEL_TC = 2          /* tcgen05 kind::tf32, every product from three TF32 MMAs (hi/lo split), fp32 sums */
+};
 /* Tensor-core tile shapes (Gram rows x Gram columns; 4 Gram rows = 1 station), xc_set_option(XC_OPT_TILE, ...).
  * Round 1 also built 128x256 single-CTA tiles, a staged (bulk-store) epilogue, 64/256-sample stages and two
  * diagonal-specialised schedules (SPLIT, MIXED); all measured slower than these two and were removed. */
@@ -100,6 +106,7 @@ typedef enum {
                            /* row pitch x F is, move every channel's tile grid left by the offset of its rows inside   */
                            /* their 128-byte line, so that TMA fetches whole lines ("rows aligned to   */
                            /* the memory line"); 0 = off (for comparison).  Same bits either way.                       */
+    , XC_OPT_F32_KERNEL = 10  /* one of XC_F32_KERNEL_* (xc_correlate_f32)                                               */
 #ifdef XC_PROFILE
     , XC_OPT_DEBUG_SKIP = 3 /* PROFILING BUILD ONLY (-DXC_PROFILE), results become meaningless: bit 0 = no TMA */
                             /* loads after the first ring fill, bit 1 = no MMAs, bit 2 = no stores, bit 3 =    */
@@ -181,13 +188,17 @@ int xc_correlate_acc(xc_plan_t* plan, const int8_t* in_dev, int32_t* vis_dev, vo
  *   the SIMT kernel selected. */
 int xc_correlate_i4(xc_plan_t* plan, const uint8_t* in4_dev, int32_t* vis_dev, int accumulate, void* cuda_stream);
 
-/* xc_correlate_f32 -- same operation on float samples with fp32 FMA arithmetic on the CUDA
- *   cores (the paper's own arithmetic: PAPER.md:75, 16 FMAs per station pair per sample;
- *   warp-level register tiling as in PAPER.md:130-147).  in_dev: float [T][F][N][2][2] (16-byte
- *   aligned); vis_dev: float [F][NB][2][2][2].  accumulate != 0 adds to vis_dev.  Summation
- *   order over t is fixed (ascending, one accumulator per output) so results are
- *   deterministic; they agree with an fp64 evaluation to about T * 2^-24 relative to
- *   sqrt(V_ii V_jj). */
+/* xc_correlate_f32 -- same operation on float samples.  in_dev: float [T][F][N][2][2] (16-byte aligned, dense);
+ *   vis_dev: float [F][NB][2][2][2].  accumulate != 0 adds to vis_dev.  Two kernels (XC_OPT_F32_KERNEL):
+ *   - CUDA cores: fp32 FMA arithmetic (the paper's own: PAPER.md:75, 16 FMAs per station pair per sample; warp-level
+ *     register tiling as in PAPER.md:130-147).  One accumulator per output, ascending t: deterministic, about T * 2^-24
+ *     relative to sqrt(V_ii V_jj) from an fp64 evaluation.
+ *   - tensor cores (default for N >= 48): x x^H is a dense contraction; every sample is split into two TF32 numbers
+ *     (hi = nearest TF32, lo = a - hi) and every product taken as lo hi + hi lo + hi hi into an fp32 accumulator.  The
+ *     dropped parts are below 2^-21 of each product; sums are fp32 in the tensor core's order.  Deterministic (fixed
+ *     schedule); meets north_star's bound 1e-5 sqrt(V_ii V_jj) with the same margin as the FMA kernel (tested);
+ *     integer-valued samples below 2^11 with sums below 2^24 give exact results.
+ *   Errors as xc_correlate. */
 int xc_correlate_f32(xc_plan_t* plan, const float* in_dev, float* vis_dev, int accumulate, void* cuda_stream);
 
 /* xc_correlate_pipelined -- Algorithm 1 read as textbook double
@@ -279,6 +290,8 @@ int xc_tile_count(const xc_plan_t* plan);
 int xc_tile_get(const xc_plan_t* plan, int k, int* bi, int* bj, int* si, int* sj);
 /* T-split factor (1 or 2) used by the last integer compute call on this plan (see XC_OPT_TSPLIT). */
 int xc_t_split(const xc_plan_t* plan);
+/* Kernel (XC_F32_KERNEL_CUDA_CORES or XC_F32_KERNEL_TC) that the last xc_correlate_f32 call on this plan ran; 0 before. */
+int xc_f32_kernel_used(const xc_plan_t* plan);
 /* Origin shift used by the last integer compute call on this plan (see XC_OPT_ORIGIN_SHIFT): returns the period P (1, 2,
  * 4 or 8 channels; 0 for a null plan) and fills, for c < P, shift_bytes[c] (grid of channels f = c mod P moved left by so
  * many bytes = 4 x stations; 0 = not moved) and tiles[c] (tiles scheduled for such a channel).  Either array may be NULL,

@@ -17,7 +17,8 @@ TIMING_WORDS = 6          # uint64 words of the xc_set_timing_buffer buffer
 TRACE_WORDS = 3 * 256 * 4  # int64 words of the profiling build's trace buffer
 I8_KERNEL_AUTO, I8_KERNEL_TC, I8_KERNEL_SIMT = 0, 1, 2
 OPT_I8_KERNEL, OPT_MAX_CTAS, OPT_FORCE_STAGE, OPT_DEBUG_SKIP, OPT_TILE, OPT_PDL, OPT_TSPLIT = 0, 1, 2, 3, 4, 7, 8
-OPT_ORIGIN_SHIFT = 9
+OPT_ORIGIN_SHIFT, OPT_F32_KERNEL = 9, 10
+F32_KERNEL_AUTO, F32_KERNEL_CUDA_CORES, F32_KERNEL_TC = 0, 1, 2
 TILE_AUTO, TILE_1CTA_128x128, TILE_2CTA_256x256 = 0, 1, 3
 
 # every symbol include/xc.h declares
@@ -25,7 +26,7 @@ EXPORTED_SYMBOLS = (
     "xc_plan", "xc_destroy", "xc_in_bytes", "xc_in_bytes_f32", "xc_vis_bytes", "xc_n_baselines",
     "xc_workspace_bytes", "xc_set_workspace", "xc_set_option", "xc_correlate", "xc_correlate_acc",
     "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_integrate",
-    "xc_correlate_i4", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get", "xc_t_split", "xc_origin_shift",
+    "xc_correlate_i4", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get", "xc_t_split", "xc_origin_shift", "xc_f32_kernel_used",
     "xc_set_in_pitch", "xc_in_pitch", "xc_scratch_pitch", "xc_scratch_in_bytes", "xc_set_timing_buffer",
     "xc_volt_bytes", "xc_cube_bytes", "xc_fengine", "xc_fengine_f32", "xc_fx",
     "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error", "xc_version",
@@ -80,6 +81,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_fengine_f32": (i, [p, p, p, p]),
         "xc_fx": (i, [p, p, ctypes.c_float, p, p, i, p]),
         "xc_tile_count": (i, [p]),
+        "xc_f32_kernel_used": (i, [p]),
         "xc_origin_shift": (i, [p, ctypes.POINTER(i), ctypes.POINTER(i)]),
         "xc_tile_get": (i, [p, i, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i)]),
         "xc_tri_index": (i64, [i64, i64]),
@@ -238,6 +240,10 @@ class Plan:
     @property
     def t_split(self) -> int:
         return int(lib().xc_t_split(self._h))
+
+    @property
+    def f32_kernel_used(self) -> int:
+        return int(lib().xc_f32_kernel_used(self._h))
 
     @property
     def origin_shift(self):

@@ -20,7 +20,7 @@ LIB = os.path.join(HERE, "libxc.so")
 LIB_PROFILE = os.path.join(HERE, "libxc_profile.so")
 LIB_PROBE = os.path.join(HERE, "libxc_probe.so")       # measurement aid (csrc/xc_probe.cu), not on the product path
 SOURCES = ["xc_api.cu"]
-HEADERS = ["xc_ptx.cuh", "xc_i8_tc.cuh", "xc_f32.cuh", "xc_fengine.cuh", "xc_simt.cuh", os.path.join("..", "..", "include", "xc.h")]
+HEADERS = ["xc_ptx.cuh", "xc_i8_tc.cuh", "xc_f32.cuh", "xc_f32_tc.cuh", "xc_fengine.cuh", "xc_simt.cuh", os.path.join("..", "..", "include", "xc.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-shared", "-Xcompiler", "-fPIC"]
 
@@ -43,7 +43,8 @@ def build(force: bool = False, verbose: bool = False, profile: bool = False) -> 
     if not force and not stale(lib):
         return lib
     tmp = lib + f".tmp{os.getpid()}"
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-DXC_PROFILE"] if profile else []) + (["-Xptxas", "-v"] if verbose else []) + \
+    cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("XC_NVCC_EXTRA", "").split() + (["-DXC_PROFILE"] if profile else []) + \
+          (["-Xptxas", "-v"] if verbose else []) + \
           ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.check_call(cmd, cwd=CSRC)
     os.replace(tmp, lib)

@@ -15,6 +15,7 @@
 #include <vector>
 
 #include "xc_f32.cuh"
+#include "xc_f32_tc.cuh"
 #include "xc_fengine.cuh"
 #include "xc_i8_tc.cuh"
 #include "xc_simt.cuh"
@@ -51,6 +52,11 @@ struct xc_plan_s {
     int tile_mode = 0;      // XC_TILE_*: shape of the tensor-core tile actually in use
     int t_split = 1;        // CTAs sharing one tile's time axis (single-CTA tile only): 1 or 2
     std::vector<uint32_t> tiles_tc, tiles_f32;
+    std::vector<uint32_t> tiles_f32tc;                   // fp32 tensor-core path: 64 x 64-station pair tiles
+    uint32_t* d_tiles_f32tc = nullptr;
+    CUtensorMap tmap_f32;
+    const void* tmap_f32_src = nullptr;
+    int opt_f32_kernel = XC_F32_KERNEL_AUTO, f32_kernel_used = 0;
     std::vector<uint32_t> tiles_tc_ext;                  // the same schedule with one more block row (origin shift): tiles_tc is its prefix
     int shift_period = 1, shift_bytes[8] = {0, 0, 0, 0, 0, 0, 0, 0}, shift_tiles[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // what the last call used
     // device state (created lazily on the device current at first compute call)
@@ -351,6 +357,12 @@ int ensure_device(xc_plan_t* p) {
     p->encode = reinterpret_cast<PFN_encodeTiled>(fn);
     XC_CUDA(p, cudaFuncSetAttribute(xc::xc_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     xc::F32_SMEM_BYTES));
+    if (!p->d_tiles_f32tc) {
+        XC_CUDA(p, cudaMalloc(&p->d_tiles_f32tc, p->tiles_f32tc.size() * sizeof(uint32_t)));
+        XC_CUDA(p, cudaMemcpy(p->d_tiles_f32tc, p->tiles_f32tc.data(), p->tiles_f32tc.size() * sizeof(uint32_t),
+                              cudaMemcpyHostToDevice));
+    }
+    XC_CUDA(p, cudaFuncSetAttribute(xc::xc_f32_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, xc::FT_SMEM_BYTES));
     XC_CUDA(p, (opt_in_smem<256, 2, 128, 1>()));
     XC_CUDA(p, (opt_in_smem<128, 1, 256, 1>()));
     XC_CUDA(p, (opt_in_smem<128, 1, 256, 2>()));
@@ -559,6 +571,64 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     return rc;
 }
 
+
+// fp32 samples on the tensor cores (xc_f32_tc.cuh): tensor map over the dense float block, persistent CTA pairs.
+int correlate_f32_tc(xc_plan_t* p, const float* in_dev, float* vis_dev, int accumulate, cudaStream_t st) {
+    if (p->tmap_f32_src != in_dev) {
+        const cuuint64_t gdim[3] = {static_cast<cuuint64_t>(4) * p->N, static_cast<cuuint64_t>(p->F), static_cast<cuuint64_t>(p->T)};
+        const cuuint64_t gstride[2] = {static_cast<cuuint64_t>(16) * p->N, static_cast<cuuint64_t>(16) * p->N * p->F};
+        const cuuint32_t box[3] = {32, 1, static_cast<cuuint32_t>(xc::FT_BK)};
+        const cuuint32_t estr[3] = {1, 1, 1};
+        CUresult r = p->encode(&p->tmap_f32, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(in_dev), gdim, gstride, box, estr,
+                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) {
+            char buf[96];
+            snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled (fp32) failed with CUresult %d", static_cast<int>(r));
+            p->last_err = buf;
+            p->tmap_f32_src = nullptr;
+            return XC_ERR_CUDA;
+        }
+        p->tmap_f32_src = in_dev;
+    }
+    xc::F32TcParams tp;
+    memset(&tp, 0, sizeof tp);
+    tp.N = p->N;
+    tp.F = p->F;
+    tp.T = p->T;
+    tp.NB = p->NB;
+    tp.vis = vis_dev;
+    tp.accumulate = accumulate ? 1 : 0;
+    tp.stamps = p->stamps;
+    tp.tiles_per_f = static_cast<int>(p->tiles_f32tc.size());
+    tp.tiles = p->d_tiles_f32tc;
+    if (tp.tiles_per_f <= xc::FT_INLINE_TILES)
+        for (int k = 0; k < tp.tiles_per_f; ++k) tp.tiles_inline[k] = p->tiles_f32tc[k];
+    const long long total = static_cast<long long>(p->F) * tp.tiles_per_f;
+    if (total > 0x7FFFFFFFLL) return XC_ERR_UNSUPPORTED;
+    tp.total_tiles = static_cast<int>(total);
+    long long units = (p->opt_max_ctas > 0 ? p->opt_max_ctas : p->sm_count) / 2;
+    if (units < 1) units = 1;
+    if (units > total) units = total;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(units * 2));
+    cfg.blockDim = dim3(xc::FT_THREADS);
+    cfg.dynamicSmemBytes = xc::FT_SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[2];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = p->opt_pdl ? 2 : 1;
+    XC_CUDA(p, cudaLaunchKernelEx(&cfg, xc::xc_f32_tc_kernel, p->tmap_f32, tp));
+    p->last_launches = 1;
+    return XC_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -586,6 +656,8 @@ int xc_plan(xc_plan_t** out, int N, int P, int F, int T, int layout) {
     p->pad_pitch = (static_cast<size_t>(4) * N + 127) & ~static_cast<size_t>(127);
     set_tile_mode(p, XC_TILE_AUTO);
     p->tiles_f32 = build_tiles(N, xc::F32_SI, xc::F32_SJ);
+    p->tiles_f32tc = build_tiles(N, 64, 64);
+    memset(&p->tmap_f32, 0, sizeof p->tmap_f32);
     memset(&p->tmap, 0, sizeof p->tmap);
     *out = p;
     return XC_OK;
@@ -595,6 +667,7 @@ void xc_destroy(xc_plan_t* p) {
     if (!p) return;
     if (p->d_tiles_tc) cudaFree(p->d_tiles_tc);
     if (p->d_tiles_f32) cudaFree(p->d_tiles_f32);
+    if (p->d_tiles_f32tc) cudaFree(p->d_tiles_f32tc);
     if (p->d_twiddle) cudaFree(p->d_twiddle);
     if (p->ws && p->ws_owned) cudaFree(p->ws);
     for (int k = 0; k < 2; ++k) {
@@ -680,6 +753,10 @@ int xc_set_option(xc_plan_t* p, int option, int value) {
         case XC_OPT_ORIGIN_SHIFT:
             p->opt_origin_shift = value ? 1 : 0;
             return XC_OK;
+        case XC_OPT_F32_KERNEL:
+            if (value < XC_F32_KERNEL_AUTO || value > XC_F32_KERNEL_TC) return XC_ERR_INVALID_ARG;
+            p->opt_f32_kernel = value;
+            return XC_OK;
 #ifdef XC_PROFILE
         case XC_OPT_DEBUG_SKIP:
             p->opt_debug_skip = value & 15;
@@ -708,6 +785,11 @@ int xc_correlate_f32(xc_plan_t* p, const float* in_dev, float* vis_dev, int accu
     int rc = ensure_device(p);
     if (rc != XC_OK) return rc;
     p->last_launches = 0;
+    // Tensor cores (three TF32 MMAs per product, xc_f32_tc.cuh) once a 64-station pair tile is mostly used; the CUDA-core
+    // kernel (xc_f32.cuh, the paper's own register tiling) below that and on request.
+    const bool tc = p->opt_f32_kernel == XC_F32_KERNEL_TC || (p->opt_f32_kernel == XC_F32_KERNEL_AUTO && p->N >= 48);
+    p->f32_kernel_used = tc ? XC_F32_KERNEL_TC : XC_F32_KERNEL_CUDA_CORES;
+    if (tc) return correlate_f32_tc(p, in_dev, vis_dev, accumulate, static_cast<cudaStream_t>(stream));
     xc::F32Params fp;
     fp.N = p->N;
     fp.F = p->F;
@@ -726,6 +808,8 @@ int xc_correlate_f32(xc_plan_t* p, const float* in_dev, float* vis_dev, int accu
     p->last_launches = 1;
     return XC_OK;
 }
+
+int xc_f32_kernel_used(const xc_plan_t* p) { return p ? p->f32_kernel_used : 0; }
 
 }  // extern "C"
 

@@ -704,26 +704,69 @@ def f32_tolerance_check(got, ref64, N):
     return ratio.max()
 
 
+F32_KERNELS = [xcb.F32_KERNEL_CUDA_CORES, xcb.F32_KERNEL_TC]     # fp32 FMAs on the CUDA cores / three TF32 MMAs per product
+
+
+@pytest.mark.parametrize("kern", F32_KERNELS)
 @pytest.mark.parametrize("N,F,T", [(1, 1, 1), (3, 2, 17), (33, 2, 100), (64, 3, 257), (100, 2, 130), (130, 1, 1000)])
-def test_f32_against_fp64_oracle(N, F, T):
+def test_f32_against_fp64_oracle(N, F, T, kern):
     rng = np.random.default_rng(N + T)
     x = rng.standard_normal((T, F, N, 2, 2)).astype(np.float32) * 4.0
     p = xcb.Plan(N, F, T)
+    p.set_option(xcb.OPT_F32_KERNEL, kern)
     vis = torch.full(p.vis_shape(), float("nan"), dtype=torch.float32, device="cuda")
     p.correlate_f32(torch.from_numpy(x).cuda(), vis)
     torch.cuda.synchronize()
+    assert p.f32_kernel_used == kern
     got = vis.cpu().numpy().astype(np.float64)
     assert np.isfinite(got).all()
     f32_tolerance_check(got, xo.channels_f64(x), N)
 
 
-def test_f32_gaussian_floats_N256_sampled_channels():
+@pytest.mark.parametrize("kern", F32_KERNELS)
+def test_f32_long_integration_keeps_the_tolerance(kern):
+    """T = 8192 Gaussian floats: sums of like-signed terms (the autocorrelations) must not drift -- the tensor core adds
+    into its accumulator by truncation, so the tensor-core kernel sums 128-sample chunks there and the chunks in registers."""
+    N, F, T = 70, 1, 8192
+    rng = np.random.default_rng(8192)
+    x = (rng.standard_normal((T, F, N, 2, 2)) * 3.0).astype(np.float32)
+    p = xcb.Plan(N, F, T)
+    p.set_option(xcb.OPT_F32_KERNEL, kern)
+    vis = torch.full(p.vis_shape(), float("nan"), dtype=torch.float32, device="cuda")
+    p.correlate_f32(torch.from_numpy(x).cuda(), vis)
+    torch.cuda.synchronize()
+    got = vis.cpu().numpy().astype(np.float64)
+    worst = f32_tolerance_check(got, xo.channels_f64(x), N)
+    if kern == xcb.F32_KERNEL_TC:
+        assert worst < 3e-6, worst          # the bias of one 128-sample chunk, not of 8192 samples
+
+
+def test_f32_tc_wide_dynamic_range():
+    """The hi/lo split of the tensor-core kernel on samples whose magnitudes span 2^-20 .. 2^20 and whose mantissas are full
+    (a single TF32 product would be off by 2^-11): still inside 1e-5 sqrt(V_ii V_jj) of the fp64 oracle; AUTO picks the
+    tensor-core kernel at this N."""
+    N, F, T = 72, 2, 96
+    rng = np.random.default_rng(4711)
+    x = (rng.standard_normal((T, F, N, 2, 2)) * np.exp2(rng.integers(-20, 21, size=(1, 1, N, 1, 1)))).astype(np.float32)
+    p = xcb.Plan(N, F, T)
+    vis = torch.full(p.vis_shape(), float("nan"), dtype=torch.float32, device="cuda")
+    p.correlate_f32(torch.from_numpy(x).cuda(), vis)
+    torch.cuda.synchronize()
+    assert p.f32_kernel_used == xcb.F32_KERNEL_TC
+    got = vis.cpu().numpy().astype(np.float64)
+    assert np.isfinite(got).all()
+    f32_tolerance_check(got, xo.channels_f64(x), N)
+
+
+@pytest.mark.parametrize("kern", F32_KERNELS)
+def test_f32_gaussian_floats_N256_sampled_channels(kern):
     """Config 3's shape class (N = 256, T = 1000) with genuinely non-integer Gaussian floats: sampled channels (first,
     last, two seeded) against the fp64-accumulating oracle at north_star's tolerance 1e-5 * sqrt(V_ii V_jj)."""
     N, F, T = 256, 24, 1000
     rng = np.random.default_rng(2563)
     x = (rng.standard_normal((T, F, N, 2, 2)) * 4.0 + rng.standard_normal((T, F, 1, 1, 2))).astype(np.float32)
     p = xcb.Plan(N, F, T)
+    p.set_option(xcb.OPT_F32_KERNEL, kern)
     vis = torch.full(p.vis_shape(), float("nan"), dtype=torch.float32, device="cuda")
     p.correlate_f32(torch.from_numpy(x).cuda(), vis)
     torch.cuda.synchronize()
@@ -734,9 +777,11 @@ def test_f32_gaussian_floats_N256_sampled_channels():
     assert worst > 1e-9                                       # the comparison is not vacuous: fp32 rounding is visible
 
 
-def test_f32_random_shapes_exact_on_integer_input_and_accumulate():
-    """The fp32 kernel's 16 x 16-station warp blocks and diagonal skipping at ragged sizes: integer-valued input keeps
-    every fp32 sum exact, so the result must equal the integer oracle bit for bit; accumulate adds exactly."""
+@pytest.mark.parametrize("kern", F32_KERNELS)
+def test_f32_random_shapes_exact_on_integer_input_and_accumulate(kern):
+    """The fp32 kernels at ragged sizes (CUDA cores: 16 x 16-station warp blocks and diagonal skipping; tensor cores: pair
+    tiles, zero-filled edges, lo parts all zero): integer-valued input keeps every fp32 sum exact, so the result must equal
+    the integer oracle bit for bit; accumulate adds exactly."""
     rng = np.random.default_rng(99)
     shapes = [(int(rng.integers(1, 200)), int(rng.integers(1, 4)), int(rng.integers(1, 300))) for _ in range(16)]
     shapes += [(15, 1, 16), (16, 1, 17), (17, 2, 15), (47, 1, 33), (48, 1, 48), (49, 1, 31), (96, 2, 50), (97, 1, 64)]
@@ -744,6 +789,7 @@ def test_f32_random_shapes_exact_on_integer_input_and_accumulate():
         x = wl.full_range(N, F, T, seed=13 * N + T)
         ref = xo.correlate_i8(x).astype(np.float32)
         p = xcb.Plan(N, F, T)
+        p.set_option(xcb.OPT_F32_KERNEL, kern)
         xd = torch.from_numpy(x).cuda().to(torch.float32)
         vis = torch.full(p.vis_shape(), float("nan"), dtype=torch.float32, device="cuda")
         p.correlate_f32(xd, vis)
@@ -753,11 +799,13 @@ def test_f32_random_shapes_exact_on_integer_input_and_accumulate():
         p.close()
 
 
-def test_f32_equals_int8_for_integer_input():
+@pytest.mark.parametrize("kern", F32_KERNELS)
+def test_f32_equals_int8_for_integer_input(kern):
     """Config 3's values as float: all products and sums are exact in fp32 -> identical results."""
     w = wl.Workload("cfg3small", 256, 4, 1000, "gauss_tone", 4.0, 1003)
     x = wl.make_input(w)
     p = xcb.Plan(w.N, w.F, w.T)
+    p.set_option(xcb.OPT_F32_KERNEL, kern)
     xd = torch.from_numpy(x).cuda()
     vi = p.correlate(xd)
     vf = p.correlate_f32(xd.to(torch.float32))
