@@ -80,7 +80,7 @@ enum {
 };
 /* Kernels of the fp32 path, xc_set_option(XC_OPT_F32_KERNEL, ...). */
 enum {
-    XC_F32_KERNEL_AUTO = 0,       /* tensor cores for N >= 48, CUDA cores below                                      */
+    XC_F32_KERNEL_AUTO = 0,       /* = XC_F32_KERNEL_TC (measured faster at every N)                                 */
     XC_F32_KERNEL_CUDA_CORES = 1, /* the paper's own scheme: register tile of station pairs per thread, packed FMAs  */
     XC_F32_KERNEL_TC = 2          /* tcgen05 kind::tf32, every product from three TF32 MMAs (hi/lo split), fp32 sums */
 };
@@ -193,10 +193,11 @@ int xc_correlate_i4(xc_plan_t* plan, const uint8_t* in4_dev, int32_t* vis_dev, i
  *   - CUDA cores: fp32 FMA arithmetic (the paper's own: PAPER.md:75, 16 FMAs per station pair per sample; warp-level
  *     register tiling as in PAPER.md:130-147).  One accumulator per output, ascending t: deterministic, about T * 2^-24
  *     relative to sqrt(V_ii V_jj) from an fp64 evaluation.
- *   - tensor cores (default for N >= 48): x x^H is a dense contraction; every sample is split into two TF32 numbers
+ *   - tensor cores (default): x x^H is a dense contraction; every sample is split into two TF32 numbers
  *     (hi = nearest TF32, lo = a - hi) and every product taken as lo hi + hi lo + hi hi into an fp32 accumulator.  The
- *     dropped parts are below 2^-21 of each product; sums are fp32 in the tensor core's order.  Deterministic (fixed
- *     schedule); meets north_star's bound 1e-5 sqrt(V_ii V_jj) with the same margin as the FMA kernel (tested);
+ *     dropped parts are below 2^-21 of each product.  The tensor core's fp32 accumulator adds by truncation, so it only
+ *     sums 128 samples at a time; the 128-sample partial sums are added in registers (round to nearest).  Deterministic
+ *     (fixed schedule); error against an fp64 evaluation ~1e-6 sqrt(V_ii V_jj) whatever T is (tested up to T = 8192);
  *     integer-valued samples below 2^11 with sums below 2^24 give exact results.
  *   Errors as xc_correlate. */
 int xc_correlate_f32(xc_plan_t* plan, const float* in_dev, float* vis_dev, int accumulate, void* cuda_stream);

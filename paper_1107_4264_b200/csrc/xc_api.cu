@@ -785,9 +785,9 @@ int xc_correlate_f32(xc_plan_t* p, const float* in_dev, float* vis_dev, int accu
     int rc = ensure_device(p);
     if (rc != XC_OK) return rc;
     p->last_launches = 0;
-    // Tensor cores (three TF32 MMAs per product, xc_f32_tc.cuh) once a 64-station pair tile is mostly used; the CUDA-core
-    // kernel (xc_f32.cuh, the paper's own register tiling) below that and on request.
-    const bool tc = p->opt_f32_kernel == XC_F32_KERNEL_TC || (p->opt_f32_kernel == XC_F32_KERNEL_AUTO && p->N >= 48);
+    // Tensor cores (three TF32 MMAs per product, xc_f32_tc.cuh) by default: measured faster at every N (N = 8 .. 256, F T =
+    // 131072: 3.3x .. 4.8x); the CUDA-core kernel (xc_f32.cuh, the paper's own register tiling) on request.
+    const bool tc = p->opt_f32_kernel != XC_F32_KERNEL_CUDA_CORES;
     p->f32_kernel_used = tc ? XC_F32_KERNEL_TC : XC_F32_KERNEL_CUDA_CORES;
     if (tc) return correlate_f32_tc(p, in_dev, vis_dev, accumulate, static_cast<cudaStream_t>(stream));
     xc::F32Params fp;
