@@ -305,9 +305,13 @@ def roofline_entry(w, k_ms, peaks, i8_burst, prof):
 
 
 def useful_over_raw(p, w):
-    """Stored baselines / baselines the scheduled tiles compute (the paper's wasted-work measure)."""
-    raw = sum(si * sj for _, _, si, sj in p.tiles())
-    return (w.N * (w.N + 1) / 2) / raw
+    """Stored baselines / baselines the scheduled tiles compute (the paper's wasted-work measure); with an
+    origin shift the tile count is the mean over the channel classes of the last call."""
+    tiles = p.tiles()
+    si, sj = tiles[0][2:]
+    cls = p.origin_shift
+    n = sum(t for _, t in cls) / len(cls) if cls and cls[0][1] else len(tiles)
+    return (w.N * (w.N + 1) / 2) / (n * si * sj)
 
 
 def main():
@@ -484,6 +488,7 @@ def main():
             xx = torch.from_numpy(wl.make_input(ww)).cuda()
             pp = xcb.Plan(ww.N, ww.F, ww.T)
             vv = pp.new_vis()
+            time.sleep(0.5)          # the previous config's sustained leg must not set this one's burst clocks
             km, em, mhz = kernel_durations(pp, xx, vv, stream, 10)
             prof = ncu_profile(name)
             ent = roofline_entry(ww, km, peaks, i8_burst, prof)
@@ -491,6 +496,7 @@ def main():
             ent.update({"N": ww.N, "F": ww.F, "T": ww.T, "event_ms": em, "sm_mhz_in_kernel": mhz,
                         "back_to_back_ms": back_to_back(pp, xx, vv, stream, 20 if ww.in_bytes > 60e6 else 200),
                         "useful_over_raw": useful_over_raw(pp, ww), "tile": pp.tiles()[0][2:], "t_split": pp.t_split,
+                        "origin_shift_bytes_tiles": pp.origin_shift,
                         "tensor_pipe_active_ncu_pct": prof.get("tensor_pipe_active_pct"),
                         "l2": "cold (input > L2)" if ww.in_bytes > 126e6 else "warm (input fits L2)"})
             ent["tops_back_to_back"] = ww.ops / (ent["back_to_back_ms"] * 1e-3) / 1e12
@@ -499,6 +505,12 @@ def main():
                 s_tops = ww.ops / (s["ms_per_launch"] * 1e-3) / 1e12
                 ent["sustained"] = {"ms_per_launch": s["ms_per_launch"], "tops": s_tops, "frac": s_tops / i8_sustained, "nvml": s["nvml"]}
             per_config[name] = ent
+            if name in ("cfg5_N500", "cfg5_N100"):
+                # the same dense block with the tile grids left unshifted (XC_OPT_ORIGIN_SHIFT = 0: round 1's schedule)
+                pp.set_option(xcb.OPT_ORIGIN_SHIFT, 0)
+                time.sleep(0.5)
+                ent["origin_shift_off_kernel_ms"] = kernel_durations(pp, xx, vv, stream, 10)[0]
+                pp.set_option(xcb.OPT_ORIGIN_SHIFT, 1)
             if name == "cfg5_N500":
                 # the same values in a block whose rows are xc_scratch_pitch() = 2048 bytes apart (xc_set_in_pitch): what the
                 # F-engine and the host-buffer calls hand to the X-engine (line-aligned rows)
@@ -506,6 +518,7 @@ def main():
                 xp = torch.zeros((ww.T, ww.F, pitch), dtype=torch.int8, device="cuda")
                 xp[:, :, :4 * ww.N] = xx.view(ww.T, ww.F, 4 * ww.N)
                 pp.set_in_pitch(pitch)
+                time.sleep(0.5)
                 km2, em2, mhz2 = kernel_durations(pp, xp, vv, stream, 10)
                 ent2 = roofline_entry(ww, km2, peaks, i8_burst, ncu_profile(name + "_p2048"))
                 ent2.pop("ncu", None)

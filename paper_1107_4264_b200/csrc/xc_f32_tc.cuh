@@ -20,34 +20,43 @@
 // Pipeline per CTA of a pair (cta_group::2, 256 x 256 Gram tile = 64 x 64 stations, as in xc_i8_tc.cuh):
 //   warp 0      TMA producer: per 32-sample stage 4 + 4 boxes [32 t][32 floats] (A rows, this CTA's half of the B rows;
 //               diagonal tiles load B only), 128-byte swizzle with 32-byte atoms, MN-major -- time is the slowest input index
-//   warps 2-3   split: read the stage's raw samples, write hi in their place and lo into the stage's second half (the
-//               split is elementwise, so it does not care about the swizzle), fence.proxy.async, signal the leader
+//   warps 2-7   split: read the stage's raw samples, write hi in their place and lo into the stage's second half (the
+//               split is elementwise, so it does not care about the swizzle), fence.proxy.async, then arrive on the leader's
+//               barrier with CTA-scope release (as CUTLASS's ClusterBarrier::arrive does): the bytes are only ever read by
+//               this CTA's own SM on behalf of the pair's MMA.  A cluster-scope release compiles to MEMBAR.ALL.GPU and cost
+//               a quarter of the throughput (0.96 ms against 0.58 ms on config 3's shape, F = 128)
 //   warp 1      MMA issuer (leader CTA): per 8-sample K step three tcgen05.mma.kind::tf32 M = 256, N = 256
-//   warps 4-11  epilogue: per 128-sample chunk tcgen05.ld + add into 128 running sums per thread; per tile lane-pair swap,
+//   warps 8-15  epilogue: per 128-sample chunk tcgen05.ld + add into 128 running sums per thread; per tile lane-pair swap,
 //               float combine, 16-byte streaming stores (same packing as int8)
 // Shared memory per stage: 32 KB raw/hi + 32 KB lo; three stages.  TMEM: two 256-column fp32 accumulators.
+// Registers: the epilogue threads hold 128 running sums each, so the two warpgroups of warps 0-7 drop to 72 registers per thread
+// and the two epilogue warpgroups rise to 184 (setmaxnreg; with two split warps and 384 threads of 168 registers the split was
+// the bottleneck: 0.574 against 0.504 ms on config 3's shape, F = 128).
 #pragma once
 #include "xc_i8_tc.cuh"
 
 namespace xc {
 
-constexpr int FT_BK = 32;                                  // samples per ring stage (four K = 8 steps)
+#ifndef XC_FT_BK
+#define XC_FT_BK 32
+#endif
+constexpr int FT_BK = XC_FT_BK;                            // samples per ring stage (K = 8 steps of three MMAs each)
 constexpr int FT_UMMA_K = 8;                               // samples per tcgen05.mma (kind::tf32)
 constexpr int FT_BOX_BYTES = FT_BK * 128;                  // one TMA box: FT_BK rows of 32 floats
 constexpr int FT_OP_BYTES = 4 * FT_BOX_BYTES;              // 128 Gram rows = 4 boxes = 4 MN atoms of 32 floats
 constexpr int FT_RAW_BYTES = 2 * FT_OP_BYTES;              // A rows + this CTA's half of the B rows
 constexpr int FT_STAGE_BYTES = 2 * FT_RAW_BYTES;           // hi parts (in place of the raw samples) + lo parts
-constexpr int FT_STAGES = 3;
+constexpr int FT_STAGES = 196608 / FT_STAGE_BYTES;          // 192 KB of ring
 #ifndef XC_FT_CHUNK
-#define XC_FT_CHUNK 4
+#define XC_FT_CHUNK (128 / XC_FT_BK)
 #endif
 #ifndef XC_FT_CONV_WARPS
-#define XC_FT_CONV_WARPS 2
+#define XC_FT_CONV_WARPS 6
 #endif
 constexpr int FT_CHUNK_STAGES = XC_FT_CHUNK;               // stages (of 32 samples) summed in one TMEM accumulator, see below
 constexpr int FT_CONV_WARPS = XC_FT_CONV_WARPS;
 constexpr int FT_EPI_WARPS = 8;
-constexpr int FT_THREADS = 64 + 32 * (FT_CONV_WARPS + FT_EPI_WARPS);   // 384: up to 168 registers per thread (the epilogue holds 128 running sums)
+constexpr int FT_THREADS = 64 + 32 * (FT_CONV_WARPS + FT_EPI_WARPS);   // 512 with 6 split warps: 128 registers per thread at launch, re-divided with setmaxnreg
 constexpr int FT_BAR_BYTES = 1024;
 constexpr int FT_SMEM_BYTES = FT_BAR_BYTES + FT_STAGES * FT_STAGE_BYTES + 1024;   // + slack for 1024-byte alignment
 constexpr int FT_INLINE_TILES = 48;
@@ -156,12 +165,11 @@ xc_f32_tc_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t bar0 = smem_u32(smem_raw);
     auto full_bar = [&](uint32_t s) { return bar0 + 8u * s; };                          // local: this CTA's TMA bytes
-    auto conv_bar = [&](uint32_t s) { return bar0 + 8u * (FT_STAGES + s); };            // local: this CTA's stage is split
-    auto peer_bar = [&](uint32_t s) { return bar0 + 8u * (3 * FT_STAGES + 4 + s); };    // leader: the peer CTA's stage is split
+    auto conv_bar = [&](uint32_t s) { return bar0 + 8u * (FT_STAGES + s); };            // leader: both CTAs' stages are split
     auto empty_bar = [&](uint32_t s) { return bar0 + 8u * (2 * FT_STAGES + s); };       // both: the MMAs have read the stage
     auto tfull_bar = [&](uint32_t b) { return bar0 + 8u * (3 * FT_STAGES + b); };
     auto tempty_bar = [&](uint32_t b) { return bar0 + 8u * (3 * FT_STAGES + 2 + b); };
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem_raw + 8 * (4 * FT_STAGES + 4));
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem_raw + 8 * (3 * FT_STAGES + 4));
     const uint32_t ring0 = (bar0 + FT_BAR_BYTES + 1023u) & ~1023u;
 
     const int warp = threadIdx.x >> 5;
@@ -183,8 +191,7 @@ xc_f32_tc_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant
         tma_prefetch_desc(&tmap);
         for (int s = 0; s < FT_STAGES; ++s) {
             mbar_init(full_bar(s), 1);                       // producer's arrive.expect_tx (+ this CTA's TMA bytes)
-            mbar_init(conv_bar(s), FT_CONV_WARPS);           // one arrival per split warp of this CTA
-            mbar_init(peer_bar(s), 1);                       // relayed by warp 1 of the peer CTA
+            mbar_init(conv_bar(s), 2 * FT_CONV_WARPS);       // (on the leader) one arrival per split warp of the pair
             mbar_init(empty_bar(s), 1);                      // tcgen05.commit, multicast to both CTAs
         }
         for (int b = 0; b < 2; ++b) {
@@ -206,109 +213,140 @@ xc_f32_tc_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant
 
     const int KB = (p.T + FT_BK - 1) / FT_BK;
 
-    if (warp == 0) {
-        // ===== TMA producer =====
-        const uint32_t elected = elect_one();
-        uint32_t stage = 0, phase = 0;
-        int w_next = walk(0, unit, nunits, p.total_tiles);
-        uint32_t tb_next = (w_next >= 0) ? ft_tile_at(p, w_next % p.tiles_per_f) : 0u;
-        for (int n = 0; w_next >= 0; ++n) {
-            const int f = w_next / p.tiles_per_f;
-            const uint32_t tb = __shfl_sync(0xffffffffu, tb_next, 0);
-            w_next = walk(n + 1, unit, nunits, p.total_tiles);
-            if (w_next >= 0) tb_next = ft_tile_at(p, w_next % p.tiles_per_f);
-            const int m_a = static_cast<int>(tb & 0xFFFFu) * 256 + 128 * static_cast<int>(rank);   // first Gram row (float) of A
-            const int m_b = static_cast<int>(tb >> 16) * 256 + 128 * static_cast<int>(rank);
-            const bool a_in_b = (m_a == m_b);     // diagonal tile: this CTA's A rows are its B rows
-            for (int kb = 0; kb < KB; ++kb) {
-                mbar_wait(empty_bar(stage), phase ^ 1u);
-                if (elected) {
-                    const uint32_t sa = ring0 + stage * FT_STAGE_BYTES;
-                    const uint32_t sb = sa + FT_OP_BYTES;
-                    const int t0 = kb * FT_BK;
-                    mbar_arrive_expect_tx(full_bar(stage), a_in_b ? FT_OP_BYTES : FT_RAW_BYTES);
-                    if (!a_in_b) {
-#pragma unroll
-                        for (int g = 0; g < 4; ++g) tma_load_3d(sa + g * FT_BOX_BYTES, &tmap, full_bar(stage), m_a + 32 * g, f, t0);
-                    }
-#pragma unroll
-                    for (int g = 0; g < 4; ++g) tma_load_3d(sb + g * FT_BOX_BYTES, &tmap, full_bar(stage), m_b + 32 * g, f, t0);
-                }
-                __syncwarp();
-                if (++stage == FT_STAGES) {
-                    stage = 0;
-                    phase ^= 1u;
-                }
-            }
-        }
-    } else if (warp == 1) {
-        // ===== MMA issuer: leader CTA only =====
-        if (rank == 0) {
+    if (warp < 2 + FT_CONV_WARPS) {
+#if XC_FT_CONV_WARPS == 6
+        // 16 warps = four warpgroups of 128 registers per thread at launch: the two groups that hold the producer, the issuer
+        // and the split warps hand registers to the two epilogue groups (128 running sums per thread): 256 x 72 + 256 x 184 = 64 K
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 72;" ::: "memory");
+#endif
+        if (warp == 0) {
+            // ===== TMA producer =====
             const uint32_t elected = elect_one();
-            constexpr uint32_t idesc = make_idesc_tf32_mn(256, 256);
-            uint32_t stage = 0, phase = 0, buf = 0, tphase = 0;
+            uint32_t stage = 0, phase = 0;
             int w_next = walk(0, unit, nunits, p.total_tiles);
             uint32_t tb_next = (w_next >= 0) ? ft_tile_at(p, w_next % p.tiles_per_f) : 0u;
             for (int n = 0; w_next >= 0; ++n) {
+                const int f = w_next / p.tiles_per_f;
                 const uint32_t tb = __shfl_sync(0xffffffffu, tb_next, 0);
                 w_next = walk(n + 1, unit, nunits, p.total_tiles);
                 if (w_next >= 0) tb_next = ft_tile_at(p, w_next % p.tiles_per_f);
-                const bool a_in_b = ((tb & 0xFFFFu) == (tb >> 16));
-                const uint32_t a_off = a_in_b ? static_cast<uint32_t>(FT_OP_BYTES) : 0u;
+                const int m_a = static_cast<int>(tb & 0xFFFFu) * 256 + 128 * static_cast<int>(rank);   // first Gram row (float) of A
+                const int m_b = static_cast<int>(tb >> 16) * 256 + 128 * static_cast<int>(rank);
+                const bool a_in_b = (m_a == m_b);     // diagonal tile: this CTA's A rows are its B rows
                 for (int kb = 0; kb < KB; ++kb) {
-                    const int kc = kb % FT_CHUNK_STAGES;                     // stage inside the chunk
-                    if (kc == 0) {
-                        mbar_wait(tempty_bar(buf), ((tphase >> buf) & 1u) ^ 1u);   // the epilogues have drained this accumulator
-                        tc_fence_after();
-                    }
-                    const uint32_t d_tmem = tmem_base + buf * 256u;
-                    mbar_wait(conv_bar(stage), phase);                     // this CTA's half of the stage is split ...
-                    mbar_wait_acquire_cluster(peer_bar(stage), phase);     // ... and the peer's (relayed release arrive)
-                    tc_fence_after();
-                    const bool chunk_end = (kc == FT_CHUNK_STAGES - 1) || (kb == KB - 1);
+                    mbar_wait(empty_bar(stage), phase ^ 1u);
                     if (elected) {
                         const uint32_t sa = ring0 + stage * FT_STAGE_BYTES;
-                        // MN-major, 128-byte swizzle with 32-byte atoms: atoms of 4 samples x 32 floats; LBO = one box between
-                        // MN atoms, SBO = 512 B between the two atoms of an 8-sample K step
-                        const uint64_t ahi = make_smem_desc_mn_sw128_32b(sa + a_off, FT_BOX_BYTES, 512);
-                        const uint64_t alo = make_smem_desc_mn_sw128_32b(sa + FT_RAW_BYTES + a_off, FT_BOX_BYTES, 512);
-                        const uint64_t bhi = make_smem_desc_mn_sw128_32b(sa + FT_OP_BYTES, FT_BOX_BYTES, 512);
-                        const uint64_t blo = make_smem_desc_mn_sw128_32b(sa + FT_RAW_BYTES + FT_OP_BYTES, FT_BOX_BYTES, 512);
-                        const int rows = min(FT_BK, p.T - kb * FT_BK);
-                        const int nk = (rows + FT_UMMA_K - 1) / FT_UMMA_K;       // rows beyond T are TMA zero fill
+                        const uint32_t sb = sa + FT_OP_BYTES;
+                        const int t0 = kb * FT_BK;
+                        mbar_arrive_expect_tx(full_bar(stage), a_in_b ? FT_OP_BYTES : FT_RAW_BYTES);
+                        if (!a_in_b) {
 #pragma unroll
-                        for (int ks = 0; ks < FT_BK / FT_UMMA_K; ++ks) {
-                            if (ks < nk) {
-                                const uint64_t adv = static_cast<uint64_t>(ks * 64);   // 8 samples = two atoms = 1024 B
-                                umma_tf32_2cta(d_tmem, alo + adv, bhi + adv, idesc, (kc | ks) ? 1u : 0u);
-                                umma_tf32_2cta(d_tmem, ahi + adv, blo + adv, idesc, 1u);
-                                umma_tf32_2cta(d_tmem, ahi + adv, bhi + adv, idesc, 1u);
-                            }
+                            for (int g = 0; g < 4; ++g) tma_load_3d(sa + g * FT_BOX_BYTES, &tmap, full_bar(stage), m_a + 32 * g, f, t0);
                         }
-                        umma_commit<2>(empty_bar(stage));
-                        if (chunk_end) umma_commit<2>(tfull_bar(buf));      // chunk complete -> epilogues
+#pragma unroll
+                        for (int g = 0; g < 4; ++g) tma_load_3d(sb + g * FT_BOX_BYTES, &tmap, full_bar(stage), m_b + 32 * g, f, t0);
                     }
                     __syncwarp();
-                    if (chunk_end) {
-                        tphase ^= 1u << buf;
-                        buf ^= 1u;
-                    }
                     if (++stage == FT_STAGES) {
                         stage = 0;
                         phase ^= 1u;
+                    }
+                }
+            }
+        } else if (warp == 1) {
+            // ===== MMA issuer: leader CTA only =====
+            if (rank == 0) {
+                const uint32_t elected = elect_one();
+                constexpr uint32_t idesc = make_idesc_tf32_mn(256, 256);
+                uint32_t stage = 0, phase = 0, buf = 0, tphase = 0;
+                int w_next = walk(0, unit, nunits, p.total_tiles);
+                uint32_t tb_next = (w_next >= 0) ? ft_tile_at(p, w_next % p.tiles_per_f) : 0u;
+                for (int n = 0; w_next >= 0; ++n) {
+                    const uint32_t tb = __shfl_sync(0xffffffffu, tb_next, 0);
+                    w_next = walk(n + 1, unit, nunits, p.total_tiles);
+                    if (w_next >= 0) tb_next = ft_tile_at(p, w_next % p.tiles_per_f);
+                    const bool a_in_b = ((tb & 0xFFFFu) == (tb >> 16));
+                    const uint32_t a_off = a_in_b ? static_cast<uint32_t>(FT_OP_BYTES) : 0u;
+                    for (int kb = 0; kb < KB; ++kb) {
+                        const int kc = kb % FT_CHUNK_STAGES;                     // stage inside the chunk
+                        if (kc == 0) {
+                            mbar_wait(tempty_bar(buf), ((tphase >> buf) & 1u) ^ 1u);   // the epilogues have drained this accumulator
+                            tc_fence_after();
+                        }
+                        const uint32_t d_tmem = tmem_base + buf * 256u;
+                        mbar_wait_acquire_cluster(conv_bar(stage), phase);     // both CTAs' halves of the stage are split
+                        tc_fence_after();
+                        const bool chunk_end = (kc == FT_CHUNK_STAGES - 1) || (kb == KB - 1);
+                        if (elected) {
+                            const uint32_t sa = ring0 + stage * FT_STAGE_BYTES;
+                            // MN-major, 128-byte swizzle with 32-byte atoms: atoms of 4 samples x 32 floats; LBO = one box between
+                            // MN atoms, SBO = 512 B between the two atoms of an 8-sample K step
+                            const uint64_t ahi = make_smem_desc_mn_sw128_32b(sa + a_off, FT_BOX_BYTES, 512);
+                            const uint64_t alo = make_smem_desc_mn_sw128_32b(sa + FT_RAW_BYTES + a_off, FT_BOX_BYTES, 512);
+                            const uint64_t bhi = make_smem_desc_mn_sw128_32b(sa + FT_OP_BYTES, FT_BOX_BYTES, 512);
+                            const uint64_t blo = make_smem_desc_mn_sw128_32b(sa + FT_RAW_BYTES + FT_OP_BYTES, FT_BOX_BYTES, 512);
+                            const int rows = min(FT_BK, p.T - kb * FT_BK);
+                            const int nk = (rows + FT_UMMA_K - 1) / FT_UMMA_K;       // rows beyond T are TMA zero fill
+#pragma unroll
+                            for (int ks = 0; ks < FT_BK / FT_UMMA_K; ++ks) {
+                                if (ks < nk) {
+                                    const uint64_t adv = static_cast<uint64_t>(ks * 64);   // 8 samples = two atoms = 1024 B
+                                    umma_tf32_2cta(d_tmem, alo + adv, bhi + adv, idesc, (kc | ks) ? 1u : 0u);
+                                    umma_tf32_2cta(d_tmem, ahi + adv, blo + adv, idesc, 1u);
+                                    umma_tf32_2cta(d_tmem, ahi + adv, bhi + adv, idesc, 1u);
+                                }
+                            }
+                            umma_commit<2>(empty_bar(stage));
+                            if (chunk_end) umma_commit<2>(tfull_bar(buf));      // chunk complete -> epilogues
+                        }
+                        __syncwarp();
+                        if (chunk_end) {
+                            tphase ^= 1u << buf;
+                            buf ^= 1u;
+                        }
+                        if (++stage == FT_STAGES) {
+                            stage = 0;
+                            phase ^= 1u;
+                        }
                     }
                 }
             }
         } else {
-            // ===== relay (peer CTA): "my half of stage s is split" travels to the leader's MMA issuer.  The split warps only
-            // release at CTA scope (cheap); the cluster-scope release -- a MEMBAR.ALL.GPU -- sits in this otherwise idle warp =====
-            const uint32_t lead_peer0 = mapa_u32(peer_bar(0), 0);
+            // ===== split warps: raw fp32 -> hi (in place) + lo =====
+            const uint32_t tid_c = static_cast<uint32_t>((warp - 2) * 32 + lane);
+            const uint32_t lead_conv0 = mapa_u32(conv_bar(0), 0);
             uint32_t stage = 0, phase = 0;
-            for (int n = 0; walk(n, unit, nunits, p.total_tiles) >= 0; ++n) {
+            int w_next = walk(0, unit, nunits, p.total_tiles);
+            uint32_t tb_next = (w_next >= 0) ? ft_tile_at(p, w_next % p.tiles_per_f) : 0u;
+            for (int n = 0; w_next >= 0; ++n) {
+                const uint32_t tb = tb_next;
+                w_next = walk(n + 1, unit, nunits, p.total_tiles);
+                if (w_next >= 0) tb_next = ft_tile_at(p, w_next % p.tiles_per_f);
+                const bool a_in_b = ((tb & 0xFFFFu) == (tb >> 16));
+                const uint32_t first = a_in_b ? static_cast<uint32_t>(FT_OP_BYTES) : 0u;     // diagonal tiles hold B rows only
                 for (int kb = 0; kb < KB; ++kb) {
-                    mbar_wait(conv_bar(stage), phase);
-                    if (lane == 0) mbar_arrive_release_cluster(lead_peer0 + 8u * stage);
+                    mbar_wait(full_bar(stage), phase);
+                    const uint32_t base = ring0 + stage * FT_STAGE_BYTES;
+#pragma unroll 4
+                    for (uint32_t off = first + tid_c * 16u; off < static_cast<uint32_t>(FT_RAW_BYTES); off += FT_CONV_WARPS * 32u * 16u) {
+                        const float4 a = ft_ld_shared_f4(base + off);
+                        float4 hi, lo;
+#ifdef XC_FT_TRUNC
+                        hi.x = __uint_as_float(__float_as_uint(a.x) & 0xFFFFE000u); hi.y = __uint_as_float(__float_as_uint(a.y) & 0xFFFFE000u);
+                        hi.z = __uint_as_float(__float_as_uint(a.z) & 0xFFFFE000u); hi.w = __uint_as_float(__float_as_uint(a.w) & 0xFFFFE000u);
+#else
+                        hi.x = ft_rna_tf32(a.x); hi.y = ft_rna_tf32(a.y); hi.z = ft_rna_tf32(a.z); hi.w = ft_rna_tf32(a.w);
+#endif
+                        lo.x = a.x - hi.x; lo.y = a.y - hi.y; lo.z = a.z - hi.z; lo.w = a.w - hi.w;
+#ifndef XC_FT_TRUNC
+                        ft_st_shared_f4(base + off, hi);
+#endif
+                        ft_st_shared_f4(base + FT_RAW_BYTES + off, lo);
+                    }
+                    fence_proxy_async_smem();          // the tensor core reads these bytes through the async proxy
                     __syncwarp();
+                    if (lane == 0) mbar_arrive_remote_release_cta(lead_conv0 + 8u * stage);
                     if (++stage == FT_STAGES) {
                         stage = 0;
                         phase ^= 1u;
@@ -316,47 +354,10 @@ xc_f32_tc_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant
                 }
             }
         }
-    } else if (warp < 2 + FT_CONV_WARPS) {
-        // ===== split warps: raw fp32 -> hi (in place) + lo =====
-        const uint32_t tid_c = static_cast<uint32_t>((warp - 2) * 32 + lane);
-        uint32_t stage = 0, phase = 0;
-        int w_next = walk(0, unit, nunits, p.total_tiles);
-        uint32_t tb_next = (w_next >= 0) ? ft_tile_at(p, w_next % p.tiles_per_f) : 0u;
-        for (int n = 0; w_next >= 0; ++n) {
-            const uint32_t tb = tb_next;
-            w_next = walk(n + 1, unit, nunits, p.total_tiles);
-            if (w_next >= 0) tb_next = ft_tile_at(p, w_next % p.tiles_per_f);
-            const bool a_in_b = ((tb & 0xFFFFu) == (tb >> 16));
-            const uint32_t first = a_in_b ? static_cast<uint32_t>(FT_OP_BYTES) : 0u;     // diagonal tiles hold B rows only
-            for (int kb = 0; kb < KB; ++kb) {
-                mbar_wait(full_bar(stage), phase);
-                const uint32_t base = ring0 + stage * FT_STAGE_BYTES;
-#pragma unroll 4
-                for (uint32_t off = first + tid_c * 16u; off < static_cast<uint32_t>(FT_RAW_BYTES); off += FT_CONV_WARPS * 32u * 16u) {
-                    const float4 a = ft_ld_shared_f4(base + off);
-                    float4 hi, lo;
-#ifdef XC_FT_TRUNC
-                    hi.x = __uint_as_float(__float_as_uint(a.x) & 0xFFFFE000u); hi.y = __uint_as_float(__float_as_uint(a.y) & 0xFFFFE000u);
-                    hi.z = __uint_as_float(__float_as_uint(a.z) & 0xFFFFE000u); hi.w = __uint_as_float(__float_as_uint(a.w) & 0xFFFFE000u);
-#else
-                    hi.x = ft_rna_tf32(a.x); hi.y = ft_rna_tf32(a.y); hi.z = ft_rna_tf32(a.z); hi.w = ft_rna_tf32(a.w);
-#endif
-                    lo.x = a.x - hi.x; lo.y = a.y - hi.y; lo.z = a.z - hi.z; lo.w = a.w - hi.w;
-#ifndef XC_FT_TRUNC
-                    ft_st_shared_f4(base + off, hi);
-#endif
-                    ft_st_shared_f4(base + FT_RAW_BYTES + off, lo);
-                }
-                fence_proxy_async_smem();          // the tensor core reads these bytes through the async proxy
-                __syncwarp();
-                if (lane == 0) mbar_arrive_release_cta(conv_bar(stage));
-                if (++stage == FT_STAGES) {
-                    stage = 0;
-                    phase ^= 1u;
-                }
-            }
-        }
     } else {
+#if XC_FT_CONV_WARPS == 6
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 184;" ::: "memory");
+#endif
         // ===== epilogue: the last 8 warps; TMEM lane quarter = warp % 4, column half = (warp - first) / 4 =====
         const int q = warp & 3;
         const int half = (warp - 2 - FT_CONV_WARPS) >> 2;

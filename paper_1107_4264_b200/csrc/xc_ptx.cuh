@@ -28,11 +28,6 @@ __device__ __forceinline__ void fence_proxy_async_smem() {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.relaxed.cta.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// Release at CTA scope: the arriving thread's (after __syncwarp: its warp's) earlier shared-memory stores are visible to a
-// thread of the same CTA that observes the phase completion (the default acquire of mbarrier.try_wait).
-__device__ __forceinline__ void mbar_arrive_release_cta(uint32_t bar) {
-    asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
@@ -106,6 +101,14 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {
 // all stall samples of the kernel).
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
     asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+// Arrive on an mbarrier anywhere in the cluster with RELEASE semantics at CTA scope (the PTX default of mbarrier.arrive;
+// what CUTLASS's ClusterBarrier::arrive(cta_id) emits): the arriving CTA's own earlier shared-memory stores (made visible to
+// the async proxy by fence.proxy.async) are ordered before the signal, and no MEMBAR.ALL.GPU is generated.  Used where the
+// signalled CTA itself never reads that memory with ordinary loads: it only issues a tcgen05.mma whose peer half is read
+// from the arriving CTA's shared memory by the arriving CTA's own SM.
+__device__ __forceinline__ void mbar_arrive_remote_release_cta(uint32_t cluster_bar) {
+    asm volatile("mbarrier.arrive.release.cta.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
 }
 // Release at cluster scope: this thread's (and, after __syncwarp, its warp's) earlier st.shared::cluster stores are
 // visible to whoever acquires the barrier's phase at cluster scope (T-split hand-over of partial accumulators).
