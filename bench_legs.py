@@ -86,6 +86,9 @@ def f32_leg(stream, clocks, F=None, launches=5, peaks=None, kernel=None):
                     "frac": w3.ops / (ms * 1e-3) / 1e12 / tf32x3,
                     "peak_source": "bf16_tflops (burst, MEASURED_PEAKS.json) x 0.5 (nominal tf32/bf16 ratio) / 3 (MMAs per product): "
                                    "useful fp32-equivalent flops; NOT a measured tf32 number",
+                    "frac_tensor_nominal": w3.ops / (ms * 1e-3) / 1e12 / (1125.0 / 3.0),
+                    "frac_note": "frac may exceed 1: the denominator is derived from the cuBLAS bf16 measurement (0.73 of the nominal bf16 "
+                                 "peak); frac_tensor_nominal is against the nominal dense TF32 rate 1125 TFLOPS / 3",
                     "hbm_gbs": (in_bytes + vis_bytes) / (ms * 1e-3) / 1e9, "algorithmic_bytes": in_bytes + vis_bytes})
     if kernel in (None, "cuda_cores"):
         p3.set_option(xcb.OPT_F32_KERNEL, xcb.F32_KERNEL_CUDA_CORES)
