@@ -298,6 +298,11 @@ int xc_f32_kernel_used(const xc_plan_t* plan);
  * many bytes = 4 x stations; 0 = not moved) and tiles[c] (tiles scheduled for such a channel).  Either array may be NULL,
  * else it holds 8 ints. */
 int xc_origin_shift(const xc_plan_t* plan, int* shift_bytes, int* tiles);
+/* The same decision for a block at device address base_addr (16-byte aligned) with rows row_pitch_bytes apart (a multiple of
+ * 16, >= 4N), without touching the device: host logic only (used by the tests of the schedule).  Returns the period, 0 on bad
+ * arguments; it also becomes what xc_origin_shift reports until the next compute call.  Tile k of a shifted channel is entry
+ * k of the triangular list (bj = 0, 1, ...; bi = 0 .. bj) in units of the tile's stations, its first station bi * si - shift / 4. */
+int xc_origin_shift_plan(xc_plan_t* plan, uint64_t base_addr, size_t row_pitch_bytes, int* shift_bytes, int* tiles);
 
 /* The paper's closed-form triangular map and its inverse:
  *   g = by(by+1)/2 + bx,  by = floor(-1/2 + sqrt(1/4 + 2g)),  bx = g - by(by+1)/2,

@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = (
     "xc_plan", "xc_destroy", "xc_in_bytes", "xc_in_bytes_f32", "xc_vis_bytes", "xc_n_baselines",
     "xc_workspace_bytes", "xc_set_workspace", "xc_set_option", "xc_correlate", "xc_correlate_acc",
     "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_integrate",
-    "xc_correlate_i4", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get", "xc_t_split", "xc_origin_shift", "xc_f32_kernel_used",
+    "xc_correlate_i4", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get", "xc_t_split", "xc_origin_shift", "xc_origin_shift_plan", "xc_f32_kernel_used",
     "xc_set_in_pitch", "xc_in_pitch", "xc_scratch_pitch", "xc_scratch_in_bytes", "xc_set_timing_buffer",
     "xc_volt_bytes", "xc_cube_bytes", "xc_fengine", "xc_fengine_f32", "xc_fx",
     "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error", "xc_version",
@@ -83,6 +83,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_tile_count": (i, [p]),
         "xc_f32_kernel_used": (i, [p]),
         "xc_origin_shift": (i, [p, ctypes.POINTER(i), ctypes.POINTER(i)]),
+        "xc_origin_shift_plan": (i, [p, ctypes.c_uint64, sz, ctypes.POINTER(i), ctypes.POINTER(i)]),
         "xc_tile_get": (i, [p, i, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i)]),
         "xc_tri_index": (i64, [i64, i64]),
         "xc_tri_inverse": (None, [i64, ctypes.POINTER(i64), ctypes.POINTER(i64)]),
@@ -250,6 +251,12 @@ class Plan:
         """[(shift_bytes, tiles)] per channel class f mod P of the last integer compute call (xc_origin_shift)."""
         sh, tl = (ctypes.c_int * 8)(), (ctypes.c_int * 8)()
         n = int(lib().xc_origin_shift(self._h, sh, tl))
+        return [(int(sh[c]), int(tl[c])) for c in range(n)]
+
+    def origin_shift_plan(self, base_addr: int, row_pitch_bytes: int):
+        """[(shift_bytes, tiles)] per channel class for a block at that address and row pitch (host logic only)."""
+        sh, tl = (ctypes.c_int * 8)(), (ctypes.c_int * 8)()
+        n = int(lib().xc_origin_shift_plan(self._h, base_addr, row_pitch_bytes, sh, tl))
         return [(int(sh[c]), int(tl[c])) for c in range(n)]
 
     def new_scratch(self, n: int = 1, device="cuda"):

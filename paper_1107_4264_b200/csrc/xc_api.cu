@@ -1055,6 +1055,14 @@ int xc_tile_get(const xc_plan_t* p, int k, int* bi, int* bj, int* si, int* sj) {
 
 int xc_t_split(const xc_plan_t* p) { return p ? p->t_split : 0; }
 
+int xc_origin_shift_plan(xc_plan_t* p, uint64_t base_addr, size_t row_pitch_bytes, int* shift_bytes, int* tiles) {
+    if (!p || (base_addr & 15u) || (row_pitch_bytes & 15u) || row_pitch_bytes < static_cast<size_t>(4) * p->N) return 0;
+    xc::TcParams tp;
+    memset(&tp, 0, sizeof tp);
+    plan_origin_shift(p, &tp, reinterpret_cast<const void*>(static_cast<uintptr_t>(base_addr)), row_pitch_bytes, p->F);
+    return xc_origin_shift(p, shift_bytes, tiles);
+}
+
 int xc_origin_shift(const xc_plan_t* p, int* shift_bytes, int* tiles) {
     if (!p) return 0;
     for (int c = 0; c < p->shift_period; ++c) {

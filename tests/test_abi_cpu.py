@@ -180,3 +180,45 @@ def test_tracked_ncu_exports_feed_the_bench_roofline():
         seen += 1
     assert seen == 5
     assert bench.ncu_profile("no_such_workload") == {}
+
+
+@pytest.mark.parametrize("mode", [xcb.TILE_2CTA_256x256, xcb.TILE_1CTA_128x128])
+@pytest.mark.parametrize("N,F", [(500, 64), (100, 64), (36, 16), (68, 32), (12, 8), (1000, 8), (132, 32), (96, 3), (500, 3)])
+def test_origin_shift_schedule_covers_triangle_exactly_once(N, F, mode):
+    """DESIGN.md 4 (XC_OPT_ORIGIN_SHIFT; PAPER.md:112, 149 line-aligned rows): for every channel class the tile grid moved
+    left by shift / 4 stations still covers every pair i <= j < N exactly once; shifts are what the addresses say; a class
+    keeps the unshifted grid when the shift would cost more than a quarter more tiles; no shift at all unless pitch x F is a
+    multiple of 128 bytes."""
+    p = xcb.Plan(N, F, 64)
+    p.set_option(xcb.OPT_TILE, mode)
+    si = p.tiles()[0][2]
+    n0 = -(-N // si)
+    pitch = 4 * N
+    for base in (0x7F0000000000, 0x7F0000000000 + 48):
+        cls = p.origin_shift_plan(base, pitch)
+        if (pitch * F) % 128:
+            assert cls == [(0, n0 * (n0 + 1) // 2)]
+            continue
+        period = len(cls)
+        assert period in (1, 2, 4, 8) and (pitch * period) % 128 == 0 and (period == 1 or (pitch * (period // 2)) % 128 != 0)
+        for c, (shift, tiles) in enumerate(cls):
+            want = (base + c * pitch) % 128
+            n = -(-(4 * N + shift) // (4 * si))
+            assert tiles == n * (n + 1) // 2
+            assert shift in (0, want) and shift % 16 == 0
+            if shift == 0 and want != 0:        # declined: the shifted grid would need more than 1.25 x the tiles
+                nw = -(-(4 * N + want) // (4 * si))
+                assert 4 * nw * (nw + 1) > 5 * n0 * (n0 + 1)
+            cover = np.zeros((N, N), dtype=np.int32)
+            k = 0
+            for bj in range(n):
+                for bi in range(bj + 1):
+                    i0, j0 = bi * si - shift // 4, bj * si - shift // 4
+                    ii = np.arange(max(i0, 0), min(i0 + si, N))[:, None]
+                    jj = np.arange(max(j0, 0), min(j0 + si, N))[None, :]
+                    cover[max(i0, 0):min(i0 + si, N), max(j0, 0):min(j0 + si, N)] += (ii <= jj)
+                    k += 1
+            assert k == tiles
+            iu = np.triu_indices(N)
+            assert (cover[iu] == 1).all() and cover.sum() == N * (N + 1) // 2
+    p.close()
