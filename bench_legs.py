@@ -308,9 +308,52 @@ def extras(stream, clocks, sampler, peaks):
     # ---- T-split of the single-CTA tile (small N, long integration), off / on / what AUTO picks -----------
     out["t_split"] = t_split_leg(stream)
 
+    # ---- small N: what a launch costs with no host in the loop (CUDA-graph replay of back-to-back launches) --------------------
+    out["graph_replay"] = graph_replay_leg()
+
     # ---- F-engine + corner turn, and the FX chain ----------------------------------------------------------
     out["fx"] = fengine_leg(stream, "cfg3")
     return out
+
+
+def graph_replay_leg(n=50):
+    """Config 5's latency-bound sizes (N = 32, 64, 100) and config 1: n xc_correlate launches captured into one CUDA graph (the
+    kernels are plain stream work launched with programmatic stream serialization) and replayed -- microseconds per launch with
+    the host out of the loop, next to the same n calls issued from Python through the C ABI."""
+    import torch
+    import paper_1107_4264_b200 as xcb
+    import xc_workloads as wl
+    res = {}
+    for name in ("cfg1", "cfg5_N32", "cfg5_N64", "cfg5_N100"):
+        w = wl.CONFIGS[name]
+        x = torch.from_numpy(wl.make_input(w)).cuda()
+        p = xcb.Plan(w.N, w.F, w.T)
+        v = p.new_vis()
+        p.correlate(x, v)                                    # plan's device state exists before the capture
+        s = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            cur = torch.cuda.current_stream()
+            for _ in range(n):
+                p.correlate(x, v, stream=cur)
+        torch.cuda.synchronize()
+        for _ in range(3):
+            g.replay()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(5):
+            g.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        us_graph = e0.elapsed_time(e1) * 1e3 / (5 * n)
+        us_calls = _timed(lambda: p.correlate(x, v, stream=s), s, 5 * n) * 1e3
+        floor_us = (w.in_bytes + w.vis_bytes) / 6.5e12 * 1e6
+        res[name] = {"us_per_launch_graph": us_graph, "us_per_launch_calls": us_calls, "hbm_floor_us": floor_us,
+                     "tops_graph": w.ops / (us_graph * 1e-6) / 1e12}
+        p.close()
+        del g, x, v
+    return res
 
 
 def t_split_leg(stream):

@@ -304,8 +304,8 @@ int fengine_launch(xc_plan_t* p, const int8_t* volt, float scale, int8_t* cube, 
     fp.scale = scale;
     const long long grid = static_cast<long long>(fp.nsb) * ((p->T + TT - 1) / TT);
     if (grid > 0x7FFFFFFFLL) return XC_ERR_UNSUPPORTED;
-    // output tile: 2 SB columns (signals) of TT * F two-byte samples, 4 bytes of padding per column
-    const size_t tile = (static_cast<size_t>(2) * SB * (static_cast<size_t>(TT) * p->F * 2 + 4) + 15) & ~static_cast<size_t>(15);
+    // output tile: 2 SB columns (signals) of TT * F two-byte samples, FE_COL_PAD bytes of padding per column
+    const size_t tile = (static_cast<size_t>(2) * SB * (static_cast<size_t>(TT) * p->F * 2 + xc::FE_COL_PAD) + 15) & ~static_cast<size_t>(15);
     switch (p->logf) {
 #define X(L) case L: fe_launch_one<L>(fp, static_cast<unsigned>(grid), tile, st); break;
         XC_FE_FOR_ALL(X)

@@ -16,8 +16,8 @@
 // register-resident butterfly per thread, passes
 // exchanged through a shared-memory work buffer; the first pass reads the int8 samples straight from global memory, the
 // last pass scales, rounds and drops its 2-byte results into a shared-memory tile [signal][tt * F + f] (column-major: a
-// thread's outputs sit at compile-time offsets from one base; columns are padded by 4 bytes so that the row-wise read-out
-// is conflict-free).  When all signals are done the tile is streamed out: every (t, f) row of the CTA is one contiguous run
+// thread's outputs sit at compile-time offsets from one base; columns are padded by FE_COL_PAD bytes so that the last pass's stores
+// and the row-wise read-out are conflict-free).  When all signals are done the tile is streamed out: every (t, f) row of the CTA is one contiguous run
 // of SB x 4 bytes of the cube.
 // Twiddles are computed in fp64 on the host (exact at eighth turns), stored per pass in the order the pass reads them
 // ([k][r - 1] = exp(-2 pi i k r / (NS R))) and kept in shared memory.  Rounding = round-half-even in fp32, symmetric clip.
@@ -37,6 +37,8 @@ namespace xc {
 #endif
 constexpr int FE_THREADS = 256;
 constexpr int FE_MAX_LOGF = 12;            // F <= 4096
+constexpr int FE_COL_PAD = 36;             // bytes of padding per tile column: 9 words (odd: the row-wise read-out of 16 stations
+                                           // hits 16 banks; >= 8: the two signals a warp writes in the last pass use disjoint banks)
 constexpr int FE_TILE_BYTES = 32768;       // target size of the CTA's output tile (53 KB per CTA at F = 512: 4 CTAs per SM)
 
 struct FeParams {
@@ -350,7 +352,7 @@ __global__ void __launch_bounds__(FE_THREADS) xc_fengine_kernel(const FeParams p
     // output tile, column-major: column sp (signal) holds the TT * F samples of the CTA's time blocks, 2 bytes each, columns
     // CS bytes apart (+4: the read-out below walks along sp)
     const int lsb = 32 - __clz(p.SB);                               // log2(2 SB): SB is 8, 16 or 32
-    const uint32_t CS = static_cast<uint32_t>(p.TT) * F * 2u + 4u;
+    const uint32_t CS = static_cast<uint32_t>(p.TT) * F * 2u + FE_COL_PAD;
     const uint32_t tile_bytes = SPEC ? 0u : (2u * p.SB * CS + 15u) & ~15u;
     uint8_t* tile = fe_smem;
     float2* work = reinterpret_cast<float2*>(fe_smem + tile_bytes);                    // [G][FPAD]
