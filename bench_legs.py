@@ -104,6 +104,22 @@ def f32_leg(stream, clocks, F=None, launches=5, peaks=None, kernel=None):
     p3.close()
     del x3, v3
     torch.cuda.empty_cache()
+    if kernel is None and F is None:
+        # the tensor-core kernel against N (T = 2048, F N = 8192: 268 MB of float samples each; random normal floats)
+        sweep = {}
+        for N in (64, 128, 256, 512, 1024):
+            Fn, T = 8192 // N, 2048
+            x = torch.randn((T, Fn, N, 2, 2), device="cuda")
+            p = xcb.Plan(N, Fn, T)
+            v = p.new_vis(torch.float32)
+            ms = _timed(lambda: p.correlate_f32(x, v, stream=stream), stream, launches)
+            ops = 8.0 * Fn * T * N * (2 * N + 1)
+            sweep[f"N{N}"] = {"F": Fn, "T": T, "kernel_ms": ms, "tflops": ops / (ms * 1e-3) / 1e12,
+                              "frac": ops / (ms * 1e-3) / 1e12 / out["peak_tflops"]}
+            p.close()
+            del x, v
+            torch.cuda.empty_cache()
+        out["tensor_core_vs_N"] = sweep
     return out
 
 
