@@ -245,12 +245,13 @@ def back_to_back(p, xd, vis, stream, n):
     return b0.elapsed_time(b1) / n
 
 
-def sustained_leg(p, xd, vis, stream, sampler, seconds, est_ms):
+def sustained_leg(p, xd, vis, stream, sampler, seconds, est_ms, fn=None):
     """>= `seconds` of back-to-back launches; throughput, power and clocks over the SECOND half (steady state under the
     power cap).  Returns dict with ms per launch and the NVML summary."""
     import torch
     batch = max(8, min(2000, int(0.1 / (est_ms * 1e-3))))            # ~0.1 s of work per batch
     marks = []
+    call = fn or (lambda: p.correlate(xd, vis, stream=stream))
     with torch.cuda.stream(stream):
         stream.synchronize()
         t_begin = time.perf_counter()
@@ -259,7 +260,7 @@ def sustained_leg(p, xd, vis, stream, sampler, seconds, est_ms):
         queued = 0
         while True:
             for _ in range(batch):
-                p.correlate(xd, vis, stream=stream)
+                call()
             e = torch.cuda.Event(enable_timing=True)
             e.record(stream)
             queued += 1

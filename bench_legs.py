@@ -60,7 +60,7 @@ def cublas_int8_peak(stream):
         return {"cublas_int8_burst": None, "cublas_int8_sustained": None, "cublas_int8_how": f"unavailable: {e!r}"}
 
 
-def f32_leg(stream, clocks, F=None, launches=5, peaks=None, kernel=None):
+def f32_leg(stream, clocks, F=None, launches=5, peaks=None, kernel=None, sampler=None):
     """xc_correlate_f32 on config 3's values as float32: the tensor-core kernel (three TF32 MMAs per product; what AUTO runs at
     this N) with a tensor roofline, and the CUDA-core kernel (packed FMAs, the paper's scheme) with its ALU roofline.
     kernel = "tc" / "cuda_cores": only that one (ncu captures)."""
@@ -90,7 +90,16 @@ def f32_leg(stream, clocks, F=None, launches=5, peaks=None, kernel=None):
                     "frac_note": "frac may exceed 1: the denominator is derived from the cuBLAS bf16 measurement (0.73 of the nominal bf16 "
                                  "peak); frac_tensor_nominal is against the nominal dense TF32 rate 1125 TFLOPS / 3",
                     "hbm_gbs": (in_bytes + vis_bytes) / (ms * 1e-3) / 1e9, "algorithmic_bytes": in_bytes + vis_bytes})
+        if sampler is not None:
+            from bench import sustained_leg
+            sus = sustained_leg(None, None, None, stream, sampler, 1.5, ms, fn=lambda: p3.correlate_f32(x3, v3, stream=stream))
+            s_tf = w3.ops / (sus["ms_per_launch"] * 1e-3) / 1e12
+            s_peak = ((peaks or {}).get("bf16_sustained") or 1400.0) * 0.5 / 3.0
+            out["sustained"] = {"ms_per_launch": sus["ms_per_launch"], "tflops": s_tf, "peak_tflops": s_peak, "frac": s_tf / s_peak,
+                                "peak_source": "bf16_tflops_sustained x 0.5 / 3 (derived)", "nvml": sus["nvml"]}
     if kernel in (None, "cuda_cores"):
+        if sampler is not None:
+            time.sleep(0.5)                                  # after the sustained leg
         p3.set_option(xcb.OPT_F32_KERNEL, xcb.F32_KERNEL_CUDA_CORES)
         ms = _timed(lambda: p3.correlate_f32(x3, v3, stream=stream), stream, launches)
         fp32_peak = sms * 128 * 2 * ((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
@@ -222,7 +231,7 @@ def extras(stream, clocks, sampler, peaks):
     import xc_workloads as wl
     out = {}
     # ---- S5: fp32-input variant on config 3's values (BASELINE.json configs[2]); ALU-bound ------------------
-    out["f32"] = f32_leg(stream, clocks, peaks=peaks)
+    out["f32"] = f32_leg(stream, clocks, peaks=peaks, sampler=sampler)
 
     # ---- N = 500 from a block with 128-byte-multiple rows (xc_set_in_pitch; what the F-engine / the host paths produce) ----
     w5 = wl.CONFIGS["cfg5_N500"]
