@@ -332,16 +332,9 @@ xc_f32_tc_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant
                     for (uint32_t off = first + tid_c * 16u; off < static_cast<uint32_t>(FT_RAW_BYTES); off += FT_CONV_WARPS * 32u * 16u) {
                         const float4 a = ft_ld_shared_f4(base + off);
                         float4 hi, lo;
-#ifdef XC_FT_TRUNC
-                        hi.x = __uint_as_float(__float_as_uint(a.x) & 0xFFFFE000u); hi.y = __uint_as_float(__float_as_uint(a.y) & 0xFFFFE000u);
-                        hi.z = __uint_as_float(__float_as_uint(a.z) & 0xFFFFE000u); hi.w = __uint_as_float(__float_as_uint(a.w) & 0xFFFFE000u);
-#else
                         hi.x = ft_rna_tf32(a.x); hi.y = ft_rna_tf32(a.y); hi.z = ft_rna_tf32(a.z); hi.w = ft_rna_tf32(a.w);
-#endif
                         lo.x = a.x - hi.x; lo.y = a.y - hi.y; lo.z = a.z - hi.z; lo.w = a.w - hi.w;
-#ifndef XC_FT_TRUNC
                         ft_st_shared_f4(base + off, hi);
-#endif
                         ft_st_shared_f4(base + FT_RAW_BYTES + off, lo);
                     }
                     fence_proxy_async_smem();          // the tensor core reads these bytes through the async proxy

@@ -741,6 +741,39 @@ def test_f32_long_integration_keeps_the_tolerance(kern):
         assert worst < 3e-6, worst          # the bias of one 128-sample chunk, not of 8192 samples
 
 
+def test_f32_tc_graph_capture_accumulate_chain_and_cta_cap():
+    """The tensor-core fp32 kernel is plain stream work launched with programmatic stream serialization: an overwrite + 2
+    accumulate calls (sums stay below 2^24) captured into a CUDA graph keep their read-after-write order (integer-valued input: exact), and a cap on
+    the number of CTAs (XC_OPT_MAX_CTAS) changes the schedule, not the numbers."""
+    N, F, T = 136, 5, 300
+    x = wl.full_range(N, F, T, seed=31)
+    ref = xo.correlate_i8(x).astype(np.float32)
+    xf = torch.from_numpy(x).cuda().to(torch.float32)
+    p = xcb.Plan(N, F, T)
+    vis = p.new_vis(torch.float32)
+    p.correlate_f32(xf, vis)
+    assert p.f32_kernel_used == xcb.F32_KERNEL_TC
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        cur = torch.cuda.current_stream()
+        p.correlate_f32(xf, vis, stream=cur)
+        for _ in range(2):
+            p.correlate_f32(xf, vis, accumulate=True, stream=cur)
+    assert 3 * np.abs(ref).max() < 2 ** 24
+    for fill in (float("nan"), 7.0):
+        vis.fill_(fill)
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(vis.cpu().numpy(), 3 * ref)
+    for cap in (2, 7, 30):
+        p.set_option(xcb.OPT_MAX_CTAS, cap)
+        vis.fill_(float("nan"))
+        p.correlate_f32(xf, vis)
+        assert np.array_equal(vis.cpu().numpy(), ref), cap
+    p.close()
+
+
 def test_f32_tc_wide_dynamic_range():
     """The hi/lo split of the tensor-core kernel on samples whose magnitudes span 2^-20 .. 2^20 and whose mantissas are full
     (a single TF32 product would be off by 2^-11): still inside 1e-5 sqrt(V_ii V_jj) of the fp64 oracle; AUTO picks the
