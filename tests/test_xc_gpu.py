@@ -353,6 +353,29 @@ def test_origin_shift_unaligned_pitch(N, F, T):
         p.close()
 
 
+def test_origin_shift_random_shapes():
+    """Seeded sweep of dense blocks with N % 4 == 0, N % 32 != 0 and F % 8 == 0 (so pitch x F is a multiple of 128 bytes and the
+    shifted schedule runs) through the launch configuration xc_plan picks by itself: bit-exact, overwrite and accumulate."""
+    rng = np.random.default_rng(20261105)
+    done = 0
+    while done < 14:
+        N, F, T = 4 * int(rng.integers(1, 90)), 8 * int(rng.integers(1, 3)), int(rng.integers(1, 500))
+        if N % 32 == 0:
+            continue
+        done += 1
+        x = wl.full_range(N, F, T, seed=11 * N + T)
+        ref = xo.correlate_i8(x)
+        p = xcb.Plan(N, F, T)
+        xd = torch.from_numpy(x).cuda()
+        vis = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+        p.correlate(xd, vis)
+        assert len(p.origin_shift) > 1, (N, F, T)
+        assert np.array_equal(vis.cpu().numpy(), ref), (N, F, T, p.origin_shift)
+        p.correlate_acc(xd, vis)
+        assert np.array_equal(vis.cpu().numpy(), 2 * ref), (N, F, T, "acc")
+        p.close()
+
+
 def test_origin_shift_misaligned_base_pointer():
     """A block whose rows ARE 128 bytes apart but whose base address is not line-aligned: one shift for all channels."""
     N, F, T = 96, 3, 200         # 384-byte rows: 384 + 112 still fits the pair tile's two block rows
