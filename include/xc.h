@@ -202,6 +202,13 @@ int xc_correlate_i4(xc_plan_t* plan, const uint8_t* in4_dev, int32_t* vis_dev, i
  *   Errors as xc_correlate. */
 int xc_correlate_f32(xc_plan_t* plan, const float* in_dev, float* vis_dev, int accumulate, void* cuda_stream);
 
+/* xc_correlate_f32_channels -- xc_correlate_f32 on channels [f0, f0 + nf) of the block: the float counterpart of
+ *   xc_correlate_channels (channels are independent; one channel range per GPU or stream).
+ *   in_dev and vis_dev are the WHOLE block and cube; only the range's visibilities are written.  A proper sub-range runs on
+ *   the tensor-core kernel only (XC_ERR_UNSUPPORTED with XC_F32_KERNEL_CUDA_CORES selected). */
+int xc_correlate_f32_channels(xc_plan_t* plan, const float* in_dev, float* vis_dev, int f0, int nf, int accumulate,
+                              void* cuda_stream);
+
 /* xc_correlate_pipelined -- Algorithm 1 read as textbook double
  *   buffering: n_blocks input blocks of xc_in_bytes() each lie back to back in PINNED host
  *   memory at in_host (dense, 4*N*F*T bytes each); block p+1 is copied host->device on copy_stream into one half of

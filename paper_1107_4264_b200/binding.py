@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = (
     "xc_plan", "xc_destroy", "xc_in_bytes", "xc_in_bytes_f32", "xc_vis_bytes", "xc_n_baselines",
     "xc_workspace_bytes", "xc_set_workspace", "xc_set_option", "xc_correlate", "xc_correlate_acc",
     "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_integrate",
-    "xc_correlate_i4", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get", "xc_t_split", "xc_origin_shift", "xc_origin_shift_plan", "xc_f32_kernel_used",
+    "xc_correlate_i4", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get", "xc_t_split", "xc_origin_shift", "xc_origin_shift_plan", "xc_f32_kernel_used", "xc_correlate_f32_channels",
     "xc_set_in_pitch", "xc_in_pitch", "xc_scratch_pitch", "xc_scratch_in_bytes", "xc_set_timing_buffer",
     "xc_volt_bytes", "xc_cube_bytes", "xc_fengine", "xc_fengine_f32", "xc_fx",
     "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error", "xc_version",
@@ -65,6 +65,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_set_option": (i, [p, i, i]),
         "xc_correlate": (i, [p, p, p, p]), "xc_correlate_acc": (i, [p, p, p, p]),
         "xc_correlate_f32": (i, [p, p, p, i, p]),
+        "xc_correlate_f32_channels": (i, [p, p, p, i, i, i, p]),
         "xc_correlate_i4": (i, [p, p, p, i, p]),
         "xc_in_bytes_i4": (sz, [p]),
         "xc_correlate_channels": (i, [p, p, p, i, i, i, p]),
@@ -336,6 +337,16 @@ class Plan:
         self._chk_vis(vis, torch.float32)
         self._check(lib().xc_correlate_f32(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(vis.data_ptr()),
                                            1 if accumulate else 0, _stream_handle(stream)), "xc_correlate_f32")
+        return vis
+
+    def correlate_f32_channels(self, x, vis, f0: int, nf: int, accumulate=False, stream=None):
+        """vis[f0:f0+nf] (+)= X-engine(x[:, f0:f0+nf]) for float samples; x and vis are the plan's full block and cube."""
+        import torch
+        self._chk_in(x, torch.float32)
+        self._chk_vis(vis, torch.float32)
+        self._check(lib().xc_correlate_f32_channels(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(vis.data_ptr()),
+                                                    f0, nf, 1 if accumulate else 0, _stream_handle(stream)),
+                    "xc_correlate_f32_channels")
         return vis
 
     def correlate_pipelined(self, blocks_host, dev_buf2, vis, compute_stream, copy_stream):

@@ -56,6 +56,7 @@ struct xc_plan_s {
     uint32_t* d_tiles_f32tc = nullptr;
     CUtensorMap tmap_f32;
     const void* tmap_f32_src = nullptr;
+    int tmap_f32_nf = 0;
     int opt_f32_kernel = XC_F32_KERNEL_AUTO, f32_kernel_used = 0;
     std::vector<uint32_t> tiles_tc_ext;                  // the same schedule with one more block row (origin shift): tiles_tc is its prefix
     int shift_period = 1, shift_bytes[8] = {0, 0, 0, 0, 0, 0, 0, 0}, shift_tiles[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // what the last call used
@@ -573,9 +574,12 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
 
 
 // fp32 samples on the tensor cores (xc_f32_tc.cuh): tensor map over the dense float block, persistent CTA pairs.
-int correlate_f32_tc(xc_plan_t* p, const float* in_dev, float* vis_dev, int accumulate, cudaStream_t st) {
-    if (p->tmap_f32_src != in_dev) {
-        const cuuint64_t gdim[3] = {static_cast<cuuint64_t>(4) * p->N, static_cast<cuuint64_t>(p->F), static_cast<cuuint64_t>(p->T)};
+int correlate_f32_tc(xc_plan_t* p, const float* in_dev, float* vis_dev, int accumulate, cudaStream_t st, int f0 = 0, int nf = -1) {
+    if (nf < 0) nf = p->F;
+    in_dev += static_cast<size_t>(4) * p->N * f0;          // channels [f0, f0 + nf): the map starts at row f0, channel pitch stays F
+    vis_dev += static_cast<size_t>(f0) * p->NB * 8;
+    if (p->tmap_f32_src != in_dev || p->tmap_f32_nf != nf) {
+        const cuuint64_t gdim[3] = {static_cast<cuuint64_t>(4) * p->N, static_cast<cuuint64_t>(nf), static_cast<cuuint64_t>(p->T)};
         const cuuint64_t gstride[2] = {static_cast<cuuint64_t>(16) * p->N, static_cast<cuuint64_t>(16) * p->N * p->F};
         const cuuint32_t box[3] = {32, 1, static_cast<cuuint32_t>(xc::FT_BK)};
         const cuuint32_t estr[3] = {1, 1, 1};
@@ -590,11 +594,12 @@ int correlate_f32_tc(xc_plan_t* p, const float* in_dev, float* vis_dev, int accu
             return XC_ERR_CUDA;
         }
         p->tmap_f32_src = in_dev;
+        p->tmap_f32_nf = nf;
     }
     xc::F32TcParams tp;
     memset(&tp, 0, sizeof tp);
     tp.N = p->N;
-    tp.F = p->F;
+    tp.F = nf;
     tp.T = p->T;
     tp.NB = p->NB;
     tp.vis = vis_dev;
@@ -604,7 +609,7 @@ int correlate_f32_tc(xc_plan_t* p, const float* in_dev, float* vis_dev, int accu
     tp.tiles = p->d_tiles_f32tc;
     if (tp.tiles_per_f <= xc::FT_INLINE_TILES)
         for (int k = 0; k < tp.tiles_per_f; ++k) tp.tiles_inline[k] = p->tiles_f32tc[k];
-    const long long total = static_cast<long long>(p->F) * tp.tiles_per_f;
+    const long long total = static_cast<long long>(nf) * tp.tiles_per_f;
     if (total > 0x7FFFFFFFLL) return XC_ERR_UNSUPPORTED;
     tp.total_tiles = static_cast<int>(total);
     long long units = (p->opt_max_ctas > 0 ? p->opt_max_ctas : p->sm_count) / 2;
@@ -807,6 +812,19 @@ int xc_correlate_f32(xc_plan_t* p, const float* in_dev, float* vis_dev, int accu
     XC_CUDA(p, cudaGetLastError());
     p->last_launches = 1;
     return XC_OK;
+}
+
+int xc_correlate_f32_channels(xc_plan_t* p, const float* in_dev, float* vis_dev, int f0, int nf, int accumulate, void* stream) {
+    if (!p || !in_dev || !vis_dev) return XC_ERR_INVALID_ARG;
+    if (f0 < 0 || nf < 1 || f0 + nf > p->F) return XC_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(in_dev) & 15u) || (reinterpret_cast<uintptr_t>(vis_dev) & 15u)) return XC_ERR_ALIGNMENT;
+    if (p->opt_f32_kernel == XC_F32_KERNEL_CUDA_CORES && (f0 != 0 || nf != p->F)) return XC_ERR_UNSUPPORTED;
+    if (f0 == 0 && nf == p->F) return xc_correlate_f32(p, in_dev, vis_dev, accumulate, stream);
+    int rc = ensure_device(p);
+    if (rc != XC_OK) return rc;
+    p->last_launches = 0;
+    p->f32_kernel_used = XC_F32_KERNEL_TC;
+    return correlate_f32_tc(p, in_dev, vis_dev, accumulate, static_cast<cudaStream_t>(stream), f0, nf);
 }
 
 int xc_f32_kernel_used(const xc_plan_t* p) { return p ? p->f32_kernel_used : 0; }

@@ -797,6 +797,50 @@ def test_f32_tc_graph_capture_accumulate_chain_and_cta_cap():
     p.close()
 
 
+def test_f32_channel_sharding():
+    """xc_correlate_f32_channels (PAPER.md:65, 285 for float samples): every shard_channels() range of a 3-way split runs
+    through its own plan on its own stream (on its own GPU when several exist) into a poison-filled cube; the assembled cube
+    equals the whole-block call bit for bit (same kernel, same per-channel schedule), meets the tolerance against the fp64
+    oracle, and no rank writes outside its range; accumulate adds; the CUDA-core kernel refuses proper sub-ranges."""
+    N, F, T, world = 100, 11, 190, 3
+    rng = np.random.default_rng(5)
+    x = (rng.standard_normal((T, F, N, 2, 2)) * 3.0).astype(np.float32)
+    ndev = torch.cuda.device_count()
+    p_all = xcb.Plan(N, F, T)
+    whole = p_all.correlate_f32(torch.from_numpy(x).cuda()).cpu().numpy()
+    f32_tolerance_check(whole.astype(np.float64), xo.channels_f64(x), N)
+    out = np.empty_like(whole)
+    runs = []
+    for r in range(world):
+        lo, hi = xcb.shard_channels(F, world, r)
+        dev = r % ndev
+        with torch.cuda.device(dev):
+            p = xcb.Plan(N, F, T)
+            xd = torch.from_numpy(x).to(f"cuda:{dev}")
+            vis = torch.full(p.vis_shape(), -77.0, dtype=torch.float32, device=f"cuda:{dev}")
+            st = torch.cuda.Stream(device=dev)
+            p.correlate_f32_channels(xd, vis, lo, hi - lo, stream=st)
+            runs.append((p, xd, vis, st, lo, hi))
+    for p, xd, vis, st, lo, hi in runs:
+        st.synchronize()
+        got = vis.cpu().numpy()
+        out[lo:hi] = got[lo:hi]
+        mask = np.ones(F, bool)
+        mask[lo:hi] = False
+        assert (got[mask] == -77.0).all()
+    assert np.array_equal(out, whole)
+    p, xd, vis, st, lo, hi = runs[1]
+    with torch.cuda.device(vis.device):
+        p.correlate_f32_channels(xd, vis, lo, hi - lo, accumulate=True, stream=st)
+        st.synchronize()
+        assert np.array_equal(vis.cpu().numpy()[lo:hi], 2 * whole[lo:hi])
+        p.set_option(xcb.OPT_F32_KERNEL, xcb.F32_KERNEL_CUDA_CORES)
+        with pytest.raises(xcb.XcError):
+            p.correlate_f32_channels(xd, vis, lo, hi - lo)
+        p.correlate_f32_channels(xd, vis, 0, F)              # the whole range is just xc_correlate_f32
+        f32_tolerance_check(vis.cpu().numpy().astype(np.float64), xo.channels_f64(x), N)
+
+
 def test_f32_tc_wide_dynamic_range():
     """The hi/lo split of the tensor-core kernel on samples whose magnitudes span 2^-20 .. 2^20 and whose mantissas are full
     (a single TF32 product would be off by 2^-11): still inside 1e-5 sqrt(V_ii V_jj) of the fp64 oracle; AUTO picks the
