@@ -188,6 +188,36 @@ int xc_correlate_acc(xc_plan_t* plan, const int8_t* in_dev, int32_t* vis_dev, vo
  *   the SIMT kernel selected. */
 int xc_correlate_i4(xc_plan_t* plan, const uint8_t* in4_dev, int32_t* vis_dev, int accumulate, void* cuda_stream);
 
+/* xc_correlate_i4_noalloc -- xc_correlate_i4 for callers that must not (or cannot) allocate device memory.
+ *   Who: a real-time capture loop that cannot take cudaMalloc's device-wide stall in the middle of an observation; a
+ *   plug-in whose host application owns every byte of device memory and forbids plug-ins to allocate; a process in which
+ *   a framework's caching allocator or a memory pool has already taken the HBM that was left, so that an allocation by this
+ *   library would fail.  xc_correlate_i4 needs an int8 workspace for its unpacking pass (the tensor-core kernel reads
+ *   int8 through TMA) and a plan with small device tables; this call needs neither.  It takes the shape directly (no
+ *   plan), keeps the tile table in the kernel parameters, and unpacks into a fixed array of XC_NOALLOC_SCRATCH_BYTES
+ *   that is part of the library's device image: every GPU on which the library's image is loaded holds those 16 MiB until
+ *   the process exits, whether or not this function is ever called.  The call itself issues no cudaMalloc, cudaFree,
+ *   stream/event creation or other allocating CUDA routine, on its first use or later.
+ *   Same operation, formats and result as xc_correlate_i4 (Eq. 4; 4-bit samples PAPER.md:45, 96):
+ *   in4_dev: uint8 [T][F][N][2 pol] DEVICE memory, low nibble = real, high nibble = imaginary, two's complement;
+ *   vis_dev: int32 [F][NB][2][2][2] DEVICE memory, 16-byte aligned, overwritten (accumulate == 0) or added to
+ *   (accumulate != 0); both caller-owned.  Two launches (unpack, X-engine) on cuda_stream, asynchronous.
+ *   Limits: N <= XC_NOALLOC_MAX_N (the tile table must fit the kernel parameters) and
+ *   ((4N rounded up to 128) * F * T) <= XC_NOALLOC_SCRATCH_BYTES (the unpacked block must fit the array), T <= XC_MAX_T.
+ *   Errors: INVALID_ARG (null pointer, N/F/T < 1), OVERFLOW (T > XC_MAX_T), UNSUPPORTED (N > XC_NOALLOC_MAX_N, device
+ *   not sm_100), NO_WORKSPACE (the unpacked block is larger than XC_NOALLOC_SCRATCH_BYTES: use xc_correlate_i4 with
+ *   xc_set_workspace, or cut the block in time and accumulate), ALIGNMENT (vis_dev), CUDA.  Nothing is launched on error.
+ *   First call on a device: it looks up the array's device address (the array's name means nothing to a kernel when it
+ *   comes from host code), the tensor-map encoder and the kernels' shared-memory opt-in, with that device current; make
+ *   that first call outside any stream capture.  Later calls on that device only launch.
+ *   Sharing: there is one array per device and every call on that device uses it, whatever its shape or stream.  Calls
+ *   that may overlap on the GPU (different streams, no event between them) race on it and give garbage; calls on one
+ *   stream, or ordered by events, are safe.  The array keeps the previous call's bytes; nothing has to be cleared by the
+ *   caller: each call rewrites every byte it later reads (padding included).  Host side: thread-safe. */
+#define XC_NOALLOC_SCRATCH_BYTES (16u * 1024u * 1024u)
+#define XC_NOALLOC_MAX_N 576
+int xc_correlate_i4_noalloc(int N, int F, int T, const uint8_t* in4_dev, int32_t* vis_dev, int accumulate, void* cuda_stream);
+
 /* xc_correlate_f32 -- same operation on float samples.  in_dev: float [T][F][N][2][2] (16-byte aligned, dense);
  *   vis_dev: float [F][NB][2][2][2].  accumulate != 0 adds to vis_dev.  Two kernels (XC_OPT_F32_KERNEL):
  *   - CUDA cores: fp32 FMA arithmetic (the paper's own: PAPER.md:75, 16 FMAs per station pair per sample; warp-level

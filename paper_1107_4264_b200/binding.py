@@ -13,6 +13,8 @@ LIB_PATH = os.path.join(HERE, "libxc.so")
 LIB_PROFILE_PATH = os.path.join(HERE, "libxc_profile.so")
 
 MAX_T = 65535
+NOALLOC_SCRATCH_BYTES = 16 * 1024 * 1024   # XC_NOALLOC_SCRATCH_BYTES: the fixed device array xc_correlate_i4_noalloc unpacks into
+NOALLOC_MAX_N = 576                        # XC_NOALLOC_MAX_N
 TIMING_WORDS = 6          # uint64 words of the xc_set_timing_buffer buffer
 TRACE_WORDS = 3 * 256 * 4  # int64 words of the profiling build's trace buffer
 I8_KERNEL_AUTO, I8_KERNEL_TC, I8_KERNEL_SIMT = 0, 1, 2
@@ -26,7 +28,7 @@ EXPORTED_SYMBOLS = (
     "xc_plan", "xc_destroy", "xc_in_bytes", "xc_in_bytes_f32", "xc_vis_bytes", "xc_n_baselines",
     "xc_workspace_bytes", "xc_set_workspace", "xc_set_option", "xc_correlate", "xc_correlate_acc",
     "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_integrate",
-    "xc_correlate_i4", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get", "xc_t_split", "xc_origin_shift", "xc_origin_shift_plan", "xc_f32_kernel_used", "xc_correlate_f32_channels",
+    "xc_correlate_i4", "xc_correlate_i4_noalloc", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get", "xc_t_split", "xc_origin_shift", "xc_origin_shift_plan", "xc_f32_kernel_used", "xc_correlate_f32_channels",
     "xc_set_in_pitch", "xc_in_pitch", "xc_scratch_pitch", "xc_scratch_in_bytes", "xc_set_timing_buffer",
     "xc_volt_bytes", "xc_cube_bytes", "xc_fengine", "xc_fengine_f32", "xc_fx",
     "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error", "xc_version",
@@ -67,6 +69,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_correlate_f32": (i, [p, p, p, i, p]),
         "xc_correlate_f32_channels": (i, [p, p, p, i, i, i, p]),
         "xc_correlate_i4": (i, [p, p, p, i, p]),
+        "xc_correlate_i4_noalloc": (i, [i, i, i, p, p, i, p]),
         "xc_in_bytes_i4": (sz, [p]),
         "xc_correlate_channels": (i, [p, p, p, i, i, i, p]),
         "xc_integrate": (i, [p, p, i, p, p, p, p, p, p]),
@@ -136,6 +139,34 @@ def _stream_handle(stream) -> ctypes.c_void_p:
     import torch
     s = torch.cuda.current_stream() if stream is None else stream
     return ctypes.c_void_p(s.cuda_stream)
+
+
+def correlate_i4_noalloc(x4, vis=None, accumulate=False, stream=None):
+    """xc_correlate_i4_noalloc: the 4-bit X-engine for callers that must not allocate device memory (a real-time capture
+    loop, a plug-in of an application that owns all device memory, a process whose HBM a caching allocator has already
+    claimed).  No plan, no workspace: the library unpacks into a fixed 16 MiB array of its own device image, shared by
+    all calls on the device -- calls that overlap on the GPU race.  x4: uint8 CUDA [T][F][N][2] (low nibble re, high
+    nibble im); vis: int32 CUDA [F][N(N+1)/2][2][2][2], written or (accumulate) added to.  Passing vis=None lets torch
+    allocate the cube, which of course defeats the purpose: hand one in.  Raises XcError(XC_ERR_NO_WORKSPACE) when
+    (4N rounded up to 128) * F * T exceeds NOALLOC_SCRATCH_BYTES, XcError(XC_ERR_UNSUPPORTED) for N > NOALLOC_MAX_N."""
+    import torch
+    if not (isinstance(x4, torch.Tensor) and x4.is_cuda and x4.dtype == torch.uint8 and x4.is_contiguous()
+            and x4.dim() == 4 and x4.shape[3] == 2):
+        raise ValueError("input must be a contiguous CUDA uint8 tensor of shape [T][F][N][2]")
+    T, F, N = (int(d) for d in x4.shape[:3])
+    shape = (F, N * (N + 1) // 2, 2, 2, 2)
+    if vis is None:
+        vis = torch.empty(shape, dtype=torch.int32, device=x4.device)
+    if not (isinstance(vis, torch.Tensor) and vis.is_cuda and vis.dtype == torch.int32 and vis.is_contiguous()
+            and tuple(vis.shape) == shape):
+        raise ValueError(f"vis must be a contiguous CUDA int32 tensor of shape {shape}")
+    rc = lib().xc_correlate_i4_noalloc(N, F, T, ctypes.c_void_p(x4.data_ptr()), ctypes.c_void_p(vis.data_ptr()),
+                                       1 if accumulate else 0, _stream_handle(stream))
+    if rc != 0:
+        pitch = (4 * N + 127) // 128 * 128
+        raise XcError(rc, f"xc_correlate_i4_noalloc(N={N}, F={F}, T={T})",
+                      f"unpacked block {pitch * F * T} bytes, fixed scratch {NOALLOC_SCRATCH_BYTES} bytes, N limit {NOALLOC_MAX_N}")
+    return vis
 
 
 class Plan:

@@ -19,7 +19,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libxc.so")
 LIB_PROFILE = os.path.join(HERE, "libxc_profile.so")
 LIB_PROBE = os.path.join(HERE, "libxc_probe.so")       # measurement aid (csrc/xc_probe.cu), not on the product path
-SOURCES = ["xc_api.cu"]
+SOURCES = ["xc_api.cu", "xc_noalloc.cu"]
 HEADERS = ["xc_ptx.cuh", "xc_i8_tc.cuh", "xc_f32.cuh", "xc_f32_tc.cuh", "xc_fengine.cuh", "xc_simt.cuh", os.path.join("..", "..", "include", "xc.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-shared", "-Xcompiler", "-fPIC"]
