@@ -50,7 +50,8 @@ def lib() -> ctypes.CDLL:
         L.fo_spectra_i8.argtypes = [p, i, i, i, p, i, p]
         L.fo_fengine_i8.argtypes = [p, i, i, i, f32, p, p, p]
         L.fo_quantise_f64.argtypes = [p, sz, f32, p]
-        for n in ("fo_twiddle_f64", "fo_spectrum_i8", "fo_spectra_i8", "fo_fengine_i8", "fo_quantise_f64"):
+        L.fo_margin_f64.argtypes = [p, sz, f32, p]
+        for n in ("fo_twiddle_f64", "fo_spectrum_i8", "fo_spectra_i8", "fo_fengine_i8", "fo_quantise_f64", "fo_margin_f64"):
             getattr(L, n).restype = i
         _lib = L
     return _lib
@@ -119,3 +120,13 @@ def quantise(X: np.ndarray, scale: float) -> np.ndarray:
     if rc:
         raise OracleError(rc, "fo_quantise_f64")
     return q
+
+
+def margin(X: np.ndarray, scale: float) -> np.ndarray:
+    """float32 margins (reading 21) of the given fp64 values, for the pins."""
+    X = np.ascontiguousarray(X, dtype=np.float64)
+    m = np.empty(X.shape, np.float32)
+    rc = lib().fo_margin_f64(_ptr(X), X.size, np.float32(scale), _ptr(m))
+    if rc:
+        raise OracleError(rc, "fo_margin_f64")
+    return m

@@ -203,6 +203,13 @@ int fo_fengine_i8(const int8_t* volt, int N, int F, int T, float scale, double* 
     return rc;
 }
 
+/* The margin alone (reading 21), for its pins: m[i] = margin(X[i], scale). */
+int fo_margin_f64(const double* X, size_t n, float scale, float* m) {
+    if (!X || !m) return FO_ERR_ARG;
+    for (size_t i = 0; i < n; ++i) m[i] = fo_margin(X[i], scale);
+    return FO_OK;
+}
+
 /* The quantiser alone (reading 20), for its pins: q[i] = quantise(X[i], scale). */
 int fo_quantise_f64(const double* X, size_t n, float scale, int8_t* q) {
     if (!X || !q) return FO_ERR_ARG;

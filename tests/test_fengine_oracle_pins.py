@@ -170,6 +170,25 @@ def test_quantiser_ties_to_even_and_symmetric_clip():
     assert cube[0, 0, 0, 0].tolist() == [-127, -127]                       # symmetric clip: never -128
 
 
+def test_margin_hand_examples():
+    """fo_margin against values worked by hand (tests/golden/fengine_hand_examples.txt), not against its own formula; the
+    2^24 + 1 entry fails if the margin were taken from the fp32 product the quantiser uses."""
+    n = 0
+    for head, Xs, ms in _golden("margin"):
+        scale = float(head[0])
+        got = fo.margin(np.array(Xs, float), scale)
+        assert np.allclose(got, np.array(ms, float), rtol=0, atol=1e-7), (scale, got.tolist())
+        n += 1
+    assert n == 2
+    # the same through the whole F-engine: F = 1 is the identity, so X = the sample itself (scale 1/8: 3/8 -> 0.125, 4/8 -> 0)
+    v = np.zeros((1, 2, 1, 2), np.int8)
+    v[0, 0, 0] = (3, 4)
+    v[0, 1, 0] = (-1, 21)
+    cube, margin = fo.fengine(v, 1, 0.125)
+    assert margin[0, 0, 0].tolist() == [[0.125, 0.0], [0.375, 0.125]]
+    assert cube[0, 0, 0].tolist() == [[0, 0], [0, 3]]                       # 0.375 -> 0, 0.5 -> 0 (tie to even), -0.125 -> 0, 2.625 -> 3
+
+
 def test_margin_is_distance_to_rounding_boundary():
     v = wl.voltages(2, 64, 2, seed=11)
     scale = wl.fengine_scale(64)
