@@ -164,6 +164,43 @@ def test_fx_chain_bit_exact_when_no_near_tie(N, F, T, seed):
     assert np.array_equal(vis.cpu().numpy(), 2 * ref_vis)
 
 
+def test_fx_chain_midsize_clean_baselines_bit_exact():
+    """xc_fx against the two oracles chained at a size (N = 64, F = 64, T = 24: 3.9e5 quantised samples) where no seed is free
+    of near-ties.  From the oracle's margins ALONE: station s is 'clean' in channel f when none of its samples there lies
+    within scale * TOL(F) of a rounding boundary; the cube must equal the oracle's on every clean (f, s), and the visibility
+    of every baseline whose two stations are clean must equal X-engine-oracle(F-engine-oracle(volt)) bit for bit (a sample
+    that may round either way touches only baselines of its own station and channel)."""
+    N, F, T = 64, 64, 24
+    volt = wl.voltages(N, F, T, seed=64)
+    scale = wl.fengine_scale(F)
+    ref_cube, margin = fo.fengine(volt, F, scale)
+    ref_vis = xo.correlate_i8(ref_cube)
+    q = np.zeros(F, bool)
+    q[::F // 4] = True                                           # exact bins: ties included
+    clean = (margin > scale * tol(F)).all(axis=(0, 3, 4))        # [F][N]
+    clean[q] = True
+    assert 0.5 < clean.mean() < 1.0                              # the case has near-ties, and most stations have none
+    p = xcb.Plan(N, F, T)
+    vd = torch.from_numpy(volt).cuda()
+    cube = p.new_cube()
+    vis = torch.full(p.vis_shape(), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+    p.fx(vd, scale, cube, vis)
+    torch.cuda.synchronize()
+    got_cube = cube.cpu().numpy()[:, :, :4 * N].reshape(T, F, N, 2, 2)
+    check_cube(got_cube, ref_cube, margin, F, scale)
+    same = (got_cube == ref_cube).all(axis=(0, 3, 4))
+    assert same[clean].all()
+    jj, ii = np.tril_indices(N)                                  # i <= j, baseline b = j (j + 1) / 2 + i
+    b = jj * (jj + 1) // 2 + ii
+    ok = np.zeros((F, N * (N + 1) // 2), bool)
+    ok[:, b] = clean[:, ii] & clean[:, jj]
+    assert ok.mean() > 0.3
+    got_vis = vis.cpu().numpy()
+    assert np.array_equal(got_vis[ok], ref_vis[ok])
+    assert (got_vis != 0x5A5A5A5A).any(axis=(2, 3, 4)).all()     # every baseline was written
+    p.close()
+
+
 def test_fx_chain_config3_shape_sampled():
     """The FX chain at BASELINE.json's config 3 shape class (N = 256, F = 512, T = 64 time blocks): sampled spectra of the
     cube against the oracle (near-tie rule), and xc_fx's visibilities equal to the X-engine run on the very cube the
