@@ -1,6 +1,6 @@
-// xc_probe.cu -- measurement aid, not on the product path: pure-register FFMA2 / FFMA issue-rate probes that give the
-// fp32 X-engine (xc_f32.cuh) its practical ceiling.  Built as libxc_probe.so by `python -m paper_1107_4264_b200.build
-// --probe`; bench.py's f32 leg calls xc_probe_fma() and reports the numbers next to the kernel's own rate, so that the
+// bench_probe.cu -- measurement aid, not on the product path: pure-register FFMA2 / FFMA issue-rate probes that give the
+// fp32 X-engine (xc_f32.cuh) its practical ceiling.  Built as libbench_probe.so by bench_legs.build_probe()
+// on demand; bench.py's f32 leg calls xc_probe_fma() and reports the numbers next to the kernel's own rate, so that the
 // "ceiling" quoted in DESIGN.md is something the tracked bench measures in the same run (round 1 quoted an untracked probe).
 //
 // Every mode runs 2 x 256 threads per SM (the kernel's occupancy) doing 64 packed (or 128 scalar) FMAs per thread and

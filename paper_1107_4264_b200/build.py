@@ -18,7 +18,6 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libxc.so")
 LIB_PROFILE = os.path.join(HERE, "libxc_profile.so")
-LIB_PROBE = os.path.join(HERE, "libxc_probe.so")       # measurement aid (csrc/xc_probe.cu), not on the product path
 SOURCES = ["xc_api.cu", "xc_noalloc.cu"]
 HEADERS = ["xc_ptx.cuh", "xc_i8_tc.cuh", "xc_f32.cuh", "xc_f32_tc.cuh", "xc_fengine.cuh", "xc_simt.cuh", os.path.join("..", "..", "include", "xc.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
@@ -51,18 +50,5 @@ def build(force: bool = False, verbose: bool = False, profile: bool = False) -> 
     return lib
 
 
-def build_probe(force: bool = False) -> str:
-    src = os.path.join(CSRC, "xc_probe.cu")
-    if not force and os.path.exists(LIB_PROBE) and os.path.getmtime(LIB_PROBE) >= os.path.getmtime(src):
-        return LIB_PROBE
-    tmp = LIB_PROBE + f".tmp{os.getpid()}"
-    subprocess.check_call([_nvcc()] + NVCC_FLAGS + ["-o", tmp, src], cwd=CSRC)
-    os.replace(tmp, LIB_PROBE)
-    return LIB_PROBE
-
-
 if __name__ == "__main__":
-    if "--probe" in sys.argv:
-        print(build_probe(force="--force" in sys.argv))
-        sys.exit(0)
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, profile="--profile" in sys.argv))
