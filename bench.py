@@ -35,6 +35,7 @@ sys.path.insert(0, ROOT)
 NOMINAL_I8_OVER_BF16 = 2.0          # 4.5 / 2.25 PFLOP/s dense (B200_PROFILING.md nominal table)
 NOMINAL_I8_TOPS = 4500.0            # dense int8 = fp8 nominal (B200_PROFILING.md)
 FALLBACK_HBM_GBS, FALLBACK_BF16_TF = 6650.0, 1590.0
+NCU_CAPTURE_COMMIT = "0f76063 (2026-11-05, profiles/r2_ncu_*.csv; the X-engine kernel source is unchanged since)"
 SWEEP = ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5_N32", "cfg5_N64", "cfg5_N100", "cfg5_N500", "cfg5_N1024"]
 SUSTAINED = {"cfg2", "cfg3", "cfg4", "cfg5_N500", "cfg5_N1024"}      # the configs north_star's target speaks about (+ cfg2)
 
@@ -50,7 +51,7 @@ def load_peaks():
             "source": "fallback"}
 
 
-def ncu_profile(workload):
+def ncu_profile(workload, kernel="xc_i8_tc_kernel"):
     """Counters of xc_i8_tc_kernel from the tracked ncu export profiles/r2_ncu_<workload>.csv (written by
     `ncu -i <rep> --page raw --csv --print-units base --metrics ...`; the .md beside it names the commands).  Returns
     {} when no capture of this round exists: nothing is hard-coded here."""
@@ -64,7 +65,7 @@ def ncu_profile(workload):
     if hdr is None:
         return {}
     ki = hdr.index("Kernel Name")
-    data = [r for r in rows if len(r) == len(hdr) and "xc_i8_tc_kernel" in r[ki]]
+    data = [r for r in rows if len(r) == len(hdr) and kernel in r[ki]]
     if not data:
         return {}
 
@@ -305,6 +306,38 @@ def roofline_entry(w, k_ms, peaks, i8_burst, prof):
     return e
 
 
+def flat_roofline_keys(per_config, extras, denominators):
+    """Scalar copies of the per-config fractions, directly under `roofline` (a reader that keeps only the scalar keys of
+    `roofline` still sees a fraction for every config north_star's target names, Fig. 5: rate against N).
+    frac_<cfg> = burst fraction of the config's own bound (the `bound_<cfg>` key says which: tensor = bf16 burst x 2, hbm =
+    measured copy bandwidth); frac_<cfg>_hbm = algorithmic bytes / in-kernel time over the HBM peak whatever the bound;
+    sustained_frac_<cfg> = >= 1.5 s back to back against bf16 sustained x 2."""
+    flat = {}
+    for name, e in per_config.items():
+        flat[f"frac_{name}"] = e.get("frac")
+        flat[f"bound_{name}"] = e.get("bound")
+        flat[f"tops_{name}"] = e.get("tops")
+        flat[f"frac_{name}_hbm"] = e.get("frac_hbm_peak")
+        if "sustained" in e:
+            flat[f"sustained_frac_{name}"] = e["sustained"].get("frac")
+        if denominators.get("cublas_int8_burst") and e.get("bound") == "tensor":
+            flat[f"frac_vs_cublas_int8_{name}"] = e["tops"] / denominators["cublas_int8_burst"]
+        if e.get("tensor_pipe_active_ncu_pct") is not None:
+            flat[f"ncu_tensor_pipe_pct_{name}"] = e["tensor_pipe_active_ncu_pct"]
+    fx = extras.get("fx") or {}
+    flat["fengine_frac_hbm"] = fx.get("frac_hbm")
+    flat["fengine_ms"] = fx.get("fengine_ms")
+    f32 = extras.get("f32") or {}
+    flat["f32tc_tflops"] = f32.get("tflops")
+    flat["f32tc_frac"] = f32.get("frac")
+    flat["f32tc_tensor_pipe_pct"] = ncu_profile("f32tc", kernel="xc_f32_tc_kernel").get("tensor_pipe_active_pct")
+    i4 = extras.get("i4") or {}
+    flat["i4_tops"] = i4.get("tops")
+    # the ncu-derived numbers (traffic, tensor_pipe) describe the build that was profiled, not the one timed in this run
+    flat["traffic_captured_at_commit"] = NCU_CAPTURE_COMMIT
+    return flat
+
+
 def useful_over_raw(p, w):
     """Stored baselines / baselines the scheduled tiles compute (the paper's wasted-work measure); with an
     origin shift the tile count is the mean over the channel classes of the last call."""
@@ -540,6 +573,7 @@ def main():
                                    "sustained: >= 1.5 s back to back, frac against bf16 sustained x 2; tensor_pipe_active_ncu_pct from the "
                                    "tracked ncu exports under profiles/ (null = no capture this round)")
         extras = bench_legs.extras(stream, clocks, sampler, peaks)
+        roof.update(flat_roofline_keys(per_config, extras, denominators))
     else:
         del xd, vis, xh
 

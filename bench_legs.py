@@ -132,15 +132,56 @@ def f32_leg(stream, clocks, F=None, launches=5, peaks=None, kernel=None, sampler
     return out
 
 
+def build_probe(force=False):
+    """nvcc bench_probe.cu -> libbench_probe.so (sm_100a), next to this file: a bench aid, not part of the library."""
+    import os
+    import subprocess
+    here = os.path.dirname(os.path.abspath(__file__))
+    src, lib = os.path.join(here, "bench_probe.cu"), os.path.join(here, "libbench_probe.so")
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(src):
+        nvcc = os.path.join(os.environ.get("CUDA_HOME", "/usr/local/cuda"), "bin", "nvcc")
+        tmp = lib + f".tmp{os.getpid()}"
+        subprocess.check_call([nvcc if os.path.exists(nvcc) else "nvcc", "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
+                               "-lineinfo", "-shared", "-Xcompiler", "-fPIC", "-o", tmp, src])
+        os.replace(tmp, lib)
+    return lib
+
+
+def f32_pitch_leg(stream, launches=5):
+    """Float samples at ragged N (rows aligned to the memory line): the tensor-core fp32 kernel on a dense
+    block whose 16N-byte rows straddle 128-byte lines (N % 8 != 0) against the same values in rows padded to a multiple of
+    128 bytes (xc_set_in_pitch_f32).  T = 2048, F N ~ 8192: ~268 MB of random normal floats each."""
+    import torch
+    import paper_1107_4264_b200 as xcb
+    out = {}
+    for N in (100, 500):
+        Fn, T = 8192 // N, 2048
+        x = torch.randn((T, Fn, 4 * N), device="cuda")
+        p = xcb.Plan(N, Fn, T)
+        v = p.new_vis(torch.float32)
+        ops = 8.0 * Fn * T * N * (2 * N + 1)
+        ms_d = _timed(lambda: p.correlate_f32(x.view(T, Fn, N, 2, 2), v, stream=stream), stream, launches)
+        pitch = (16 * N + 127) // 128 * 128
+        xp = torch.zeros((T, Fn, pitch // 4), device="cuda")
+        xp[:, :, :4 * N] = x
+        p.set_in_pitch_f32(pitch)
+        ms_p = _timed(lambda: p.correlate_f32(xp, v, stream=stream), stream, launches)
+        out[f"N{N}"] = {"F": Fn, "T": T, "dense_row_bytes": 16 * N, "dense_ms": ms_d, "dense_tflops": ops / (ms_d * 1e-3) / 1e12,
+                        "pitch_bytes": pitch, "pitched_ms": ms_p, "pitched_tflops": ops / (ms_p * 1e-3) / 1e12}
+        p.close()
+        del x, xp, v
+        torch.cuda.empty_cache()
+    return out
+
+
 def fma_probe(iters=100000):
-    """Pure-register FFMA2 / FFMA streams (csrc/xc_probe.cu, built as libxc_probe.so): what the fp32 pipe delivers for the
+    """Pure-register FFMA2 / FFMA streams (bench_probe.cu beside this file, built on demand as libbench_probe.so): what the fp32 pipe delivers for the
     kernel's operand pattern with no memory traffic at all -- the practical ceiling next to which the kernel's rate is read."""
     import ctypes
-    from paper_1107_4264_b200 import build as xc_build
     names = ["kernel statement order (ptxas schedule)", "scalar FFMA", "FFMA2, all operands re-used", "FFMA2 pair x pair",
              "FFMA2 a-stationary (pinned)", "FFMA2 b-stationary (pinned)"]
     try:
-        L = ctypes.CDLL(xc_build.build_probe())
+        L = ctypes.CDLL(build_probe())
         L.xc_probe_fma.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
         res = {}
         for mode, nm in enumerate(names):
@@ -232,6 +273,7 @@ def extras(stream, clocks, sampler, peaks):
     out = {}
     # ---- S5: fp32-input variant on config 3's values (BASELINE.json configs[2]); ALU-bound ------------------
     out["f32"] = f32_leg(stream, clocks, peaks=peaks, sampler=sampler)
+    out["f32_pitch"] = f32_pitch_leg(stream)
 
     # ---- N = 500 from a block with 128-byte-multiple rows (xc_set_in_pitch; what the F-engine / the host paths produce) ----
     w5 = wl.CONFIGS["cfg5_N500"]

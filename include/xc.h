@@ -93,24 +93,26 @@ enum {
     XC_TILE_2CTA_256x256 = 3  /* 64 x 64 stations on a CTA pair (tcgen05 cta_group::2)             */
 };
 typedef enum {
-    XC_OPT_I8_KERNEL = 0, /* one of XC_I8_KERNEL_*                                            */
-    XC_OPT_MAX_CTAS = 1,  /* cap on persistent CTAs of the tensor-core kernel (0 = SM count)  */
-    XC_OPT_FORCE_STAGE = 2, /* 1 = always run the staging (re-pitch/copy) kernel, for testing S0 */
-    XC_OPT_TILE = 4,       /* one of XC_TILE_*; rebuilds the tile schedule (synchronising on next call) */
-    XC_OPT_PDL = 7,        /* 1 (default) = launch the tensor-core kernels with programmatic stream            */
-                           /* serialization: the prologue overlaps the previous kernel's tail; 0 = plain launch */
-    XC_OPT_TSPLIT = 8      /* T-split of the single-CTA tile over a cluster of 2 (the paper's small-N future    */
-                           /* work): 0 = auto (on when 2 * tiles * F <= SM count and T >= 8192: */
-                           /* the hand-over costs ~3 us), 1 = off, 2 = on whenever T allows it.  Same bits either way. */
-    , XC_OPT_ORIGIN_SHIFT = 9 /* 1 (default) = when the rows of the block are not 128 bytes apart (dense N % 32 != 0) but */
-                           /* row pitch x F is, move every channel's tile grid left by the offset of its rows inside   */
-                           /* their 128-byte line, so that TMA fetches whole lines ("rows aligned to   */
-                           /* the memory line"); 0 = off (for comparison).  Same bits either way.                       */
-    , XC_OPT_F32_KERNEL = 10  /* one of XC_F32_KERNEL_* (xc_correlate_f32)                                               */
+    XC_OPT_I8_KERNEL = 0,     /* one of XC_I8_KERNEL_*                                                                       */
+    XC_OPT_MAX_CTAS = 1,      /* cap on persistent CTAs of the tensor-core kernel (0 = SM count)                             */
+    XC_OPT_FORCE_STAGE = 2,   /* 1 = always run the staging (re-pitch/copy) kernel, for testing S0                           */
+    /* 3 = XC_OPT_DEBUG_SKIP (profiling build only, below); 5 and 6 were round 1's epilogue and schedule choices (staged     */
+    /* bulk-store epilogue, SPLIT/MIXED diagonal schedules): measured slower, removed, ids retired -> XC_ERR_INVALID_ARG     */
+    XC_OPT_TILE = 4,          /* one of XC_TILE_*; rebuilds the tile schedule (synchronising on next call)                   */
+    XC_OPT_PDL = 7,           /* 1 (default) = launch the tensor-core kernels with programmatic stream serialization: the    */
+                              /* prologue overlaps the previous kernel's tail; 0 = plain launch                              */
+    XC_OPT_TSPLIT = 8,        /* T-split of the single-CTA tile over a cluster of 2 (the paper's small-N future work,        */
+                              /* PAPER.md:311-313): 0 = auto (on when 2 * tiles * F <= SM count and T >= 8192: the hand-over */
+                              /* costs ~3 us), 1 = off, 2 = on whenever T allows it.  Same bits either way.                  */
+    XC_OPT_ORIGIN_SHIFT = 9,  /* 1 (default) = when the rows of the block are not 128 bytes apart (dense N % 32 != 0) but    */
+                              /* row pitch x F is, move every channel's tile grid left by the offset of its rows inside      */
+                              /* their 128-byte line, so that TMA fetches whole lines ("rows aligned to    */
+                              /* the memory line"); 0 = off (for comparison).  Same bits either way.                         */
+    XC_OPT_F32_KERNEL = 10    /* one of XC_F32_KERNEL_* (xc_correlate_f32)                                                   */
 #ifdef XC_PROFILE
-    , XC_OPT_DEBUG_SKIP = 3 /* PROFILING BUILD ONLY (-DXC_PROFILE), results become meaningless: bit 0 = no TMA */
-                            /* loads after the first ring fill, bit 1 = no MMAs, bit 2 = no stores, bit 3 =    */
-                            /* all stores wrapped into an 8 MB window                                           */
+    , XC_OPT_DEBUG_SKIP = 3   /* PROFILING BUILD ONLY (-DXC_PROFILE), results become meaningless: bit 0 = no TMA loads after */
+                              /* the first ring fill, bit 1 = no MMAs, bit 2 = no stores, bit 3 = all stores wrapped into    */
+                              /* an 8 MB window                                                                              */
 #endif
 } xc_option;
 
@@ -127,8 +129,8 @@ int xc_plan(xc_plan_t** out, int N, int P, int F, int T, int layout);
 void xc_destroy(xc_plan_t* plan);
 
 /* Sizes in bytes of one input block / one output cube for this plan. */
-size_t xc_in_bytes(const xc_plan_t* plan);      /* int8 path:  xc_in_pitch()*F*T = 4*N*F*T unless xc_set_in_pitch was called */
-size_t xc_in_bytes_f32(const xc_plan_t* plan);  /* fp32 path: 16*N*F*T            */
+size_t xc_in_bytes(const xc_plan_t* plan);      /* int8 path, one DEVICE block: xc_in_pitch()*F*T = 4*N*F*T unless xc_set_in_pitch was called; host blocks are always 4*N*F*T */
+size_t xc_in_bytes_f32(const xc_plan_t* plan);  /* fp32 path, one device block: xc_in_pitch_f32()*F*T = 16*N*F*T unless xc_set_in_pitch_f32 was called */
 size_t xc_in_bytes_i4(const xc_plan_t* plan);   /* 4-bit path: 2*N*F*T            */
 size_t xc_vis_bytes(const xc_plan_t* plan);     /* 32*NB*F (int32 and float alike) */
 /* N(N+1)/2. */
@@ -143,6 +145,12 @@ size_t xc_n_baselines(const xc_plan_t* plan);
  * xc_in_pitch returns the current value. */
 int xc_set_in_pitch(xc_plan_t* plan, size_t row_pitch_bytes);
 size_t xc_in_pitch(const xc_plan_t* plan);
+/* The same for float blocks (xc_correlate_f32 / _f32_channels): rows of 16N bytes, row_pitch_bytes apart (a multiple of 16,
+ * >= 16N; 0 restores the dense default).  With N % 8 != 0 dense float rows straddle 128-byte lines exactly as dense int8
+ * rows with N % 32 != 0 do; a producer that can choose should pad the rows to a multiple of 128 bytes.  Tensor-core kernel
+ * only: with XC_F32_KERNEL_CUDA_CORES selected a pitched plan answers XC_ERR_UNSUPPORTED. */
+int xc_set_in_pitch_f32(xc_plan_t* plan, size_t row_pitch_bytes);
+size_t xc_in_pitch_f32(const xc_plan_t* plan);
 /* The library's own pitch, 4N rounded up to 128 bytes (the row pitch of the staging workspace, of the host-buffer
  * calls' device blocks and of the F-engine's cube), and the size of in_dev_scratch of xc_correlate_host / of each half
  * of dev_buf2 of xc_correlate_pipelined / xc_integrate: one block with that pitch, plus -- when 4N is not already a
@@ -154,7 +162,8 @@ size_t xc_scratch_in_bytes(const xc_plan_t* plan);
 /* Staging.  The tensor-core kernel reads the input through TMA, which
  * needs a 16-byte-aligned base and a 16-byte-multiple row pitch (dense rows: N % 4 == 0).
  * Otherwise the input is first copied by a staging kernel into a workspace of
- * xc_workspace_bytes() = xc_scratch_in_bytes() bytes (the 4-bit path always unpacks into it).  The caller may hand one
+ * xc_workspace_bytes() = xc_scratch_pitch() * F * T bytes (the 4-bit path always unpacks into it; NOT xc_scratch_in_bytes(),
+ * which adds the dense landing area of the host-buffer calls).  The caller may hand one
  * in (device memory, 128-byte aligned, kept until xc_destroy or replaced); if none was set the
  * library cudaMallocs one on first need (a synchronising call) and frees it in xc_destroy.  The workspace is
  * plan-wide: staged calls issued on different streams are ordered against each other by an event. */
@@ -163,7 +172,9 @@ int xc_set_workspace(xc_plan_t* plan, void* ws_dev, size_t bytes);
 
 /* Kernel timing without a profiler: stamps_dev = device buffer of 6 uint64 (or NULL to switch off).  Every CTA of the
  * tensor-core kernel then atomically folds the global nanosecond timer into [0] (min, at kernel entry) and [1] (max, at
- * exit) -- the caller presets [0] = UINT64_MAX and [1] = 0 before the launch, and [1] - [0] is the kernel's duration --
+ * exit) -- the caller presets [0] = UINT64_MAX and [1] = 0 before the launch (in stream order: while a timing buffer is set
+ * the kernels are launched without programmatic serialization, so a preset enqueued before the call is complete when the
+ * kernel's first stamp is taken), and [1] - [0] is the kernel's duration --
  * and CTA 0 writes (clock64, globaltimer) at its entry into [2], [3] and at its exit into [4], [5], from which the SM
  * clock the kernel really ran at follows.  Costs two atomics per CTA; nothing when off. */
 int xc_set_timing_buffer(xc_plan_t* plan, uint64_t* stamps_dev);
@@ -218,7 +229,8 @@ int xc_correlate_i4(xc_plan_t* plan, const uint8_t* in4_dev, int32_t* vis_dev, i
 #define XC_NOALLOC_MAX_N 576
 int xc_correlate_i4_noalloc(int N, int F, int T, const uint8_t* in4_dev, int32_t* vis_dev, int accumulate, void* cuda_stream);
 
-/* xc_correlate_f32 -- same operation on float samples.  in_dev: float [T][F][N][2][2] (16-byte aligned, dense);
+/* xc_correlate_f32 -- same operation on float samples.  in_dev: float [T][F][N][2][2] (16-byte aligned; dense, or rows
+ *   xc_in_pitch_f32() bytes apart after xc_set_in_pitch_f32);
  *   vis_dev: float [F][NB][2][2][2].  accumulate != 0 adds to vis_dev.  Two kernels (XC_OPT_F32_KERNEL):
  *   - CUDA cores: fp32 FMA arithmetic (the paper's own: PAPER.md:75, 16 FMAs per station pair per sample; warp-level
  *     register tiling as in PAPER.md:130-147).  One accumulator per output, ascending t: deterministic, about T * 2^-24
@@ -229,6 +241,9 @@ int xc_correlate_i4_noalloc(int N, int F, int T, const uint8_t* in4_dev, int32_t
  *     sums 128 samples at a time; the 128-sample partial sums are added in registers (round to nearest).  Deterministic
  *     (fixed schedule); error against an fp64 evaluation ~1e-6 sqrt(V_ii V_jj) whatever T is (tested up to T = 8192);
  *     integer-valued samples below 2^11 with sums below 2^24 give exact results.
+ *     Precondition: finite samples with |a| < 2^127.  A sample at or above 0x7F7FF000 (3.4e38), an infinity or a NaN rounds to
+ *     a non-finite hi part, lo = a - hi is then NaN, and every visibility of THAT STATION in that channel comes out NaN (the
+ *     CUDA-core kernel gives Inf or NaN there by ordinary fp32 rules); visibilities of other stations are unaffected.
  *   Errors as xc_correlate. */
 int xc_correlate_f32(xc_plan_t* plan, const float* in_dev, float* vis_dev, int accumulate, void* cuda_stream);
 
@@ -240,8 +255,8 @@ int xc_correlate_f32_channels(xc_plan_t* plan, const float* in_dev, float* vis_d
                               void* cuda_stream);
 
 /* xc_correlate_pipelined -- Algorithm 1 read as textbook double
- *   buffering: n_blocks input blocks of xc_in_bytes() each lie back to back in PINNED host
- *   memory at in_host (dense, 4*N*F*T bytes each); block p+1 is copied host->device on copy_stream into one half of
+ *   buffering: n_blocks input blocks lie back to back in PINNED host memory at in_host, always DENSE, 4*N*F*T bytes
+ *   each whatever xc_set_in_pitch says (xc_in_bytes() follows the device pitch: do not size host blocks with it); block p+1 is copied host->device on copy_stream into one half of
  *   dev_buf2 (2 * xc_scratch_in_bytes() bytes of device memory, 128-byte aligned) while block p is
  *   correlated on compute_stream from the other half; events order the two streams (no host
  *   synchronisation inside).  vis_dev = sum over blocks (first block overwrites).  The result

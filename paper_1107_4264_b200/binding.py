@@ -29,7 +29,7 @@ EXPORTED_SYMBOLS = (
     "xc_workspace_bytes", "xc_set_workspace", "xc_set_option", "xc_correlate", "xc_correlate_acc",
     "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_integrate",
     "xc_correlate_i4", "xc_correlate_i4_noalloc", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get", "xc_t_split", "xc_origin_shift", "xc_origin_shift_plan", "xc_f32_kernel_used", "xc_correlate_f32_channels",
-    "xc_set_in_pitch", "xc_in_pitch", "xc_scratch_pitch", "xc_scratch_in_bytes", "xc_set_timing_buffer",
+    "xc_set_in_pitch", "xc_in_pitch", "xc_set_in_pitch_f32", "xc_in_pitch_f32", "xc_scratch_pitch", "xc_scratch_in_bytes", "xc_set_timing_buffer",
     "xc_volt_bytes", "xc_cube_bytes", "xc_fengine", "xc_fengine_f32", "xc_fx",
     "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error", "xc_version",
 )
@@ -77,6 +77,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_correlate_host": (i, [p, p, p, p, p, p]),
         "xc_correlate_host_i4": (i, [p, p, p, p, p, p]),
         "xc_set_in_pitch": (i, [p, sz]), "xc_in_pitch": (sz, [p]),
+        "xc_set_in_pitch_f32": (i, [p, sz]), "xc_in_pitch_f32": (sz, [p]),
         "xc_scratch_pitch": (sz, [p]), "xc_scratch_in_bytes": (sz, [p]),
         "xc_set_timing_buffer": (i, [p, p]),
         "xc_t_split": (i, [p]),
@@ -262,6 +263,14 @@ class Plan:
     def in_pitch(self) -> int:
         return int(lib().xc_in_pitch(self._h))
 
+    def set_in_pitch_f32(self, row_pitch_bytes: int) -> None:
+        """Float blocks with rows row_pitch_bytes apart (multiple of 16, >= 16N; 0 = dense): pass them as [T][F][pitch / 4]."""
+        self._check(lib().xc_set_in_pitch_f32(self._h, row_pitch_bytes), "xc_set_in_pitch_f32")
+
+    @property
+    def in_pitch_f32(self) -> int:
+        return int(lib().xc_in_pitch_f32(self._h))
+
     @property
     def scratch_pitch(self) -> int:
         return int(lib().xc_scratch_pitch(self._h))
@@ -302,6 +311,10 @@ class Plan:
         ok = isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == dtype and x.is_contiguous()
         if ok and dtype == torch.int8 and tuple(x.shape) == (self.T, self.F, self.in_pitch):
             return                                     # block given as [T][F][row pitch in bytes] (xc_set_in_pitch)
+        if ok and dtype == torch.float32 and tuple(x.shape) == (self.T, self.F, self.in_pitch_f32 // 4):
+            return                                     # float block given as [T][F][row pitch in floats] (xc_set_in_pitch_f32)
+        if ok and dtype == torch.float32 and self.in_pitch_f32 != 16 * self.N:
+            raise ValueError(f"pitched float input must be a contiguous CUDA tensor of shape {(self.T, self.F, self.in_pitch_f32 // 4)}")
         if ok and dtype == torch.int8 and self.in_pitch != 4 * self.N:
             raise ValueError(f"pitched input must be a contiguous CUDA int8 tensor of shape {(self.T, self.F, self.in_pitch)}")
         if not (ok and tuple(x.shape) == self.in_shape()):

@@ -57,6 +57,7 @@ struct xc_plan_s {
     CUtensorMap tmap_f32;
     const void* tmap_f32_src = nullptr;
     int tmap_f32_nf = 0;
+    size_t in_pitch_f32 = 0, tmap_f32_pitch = 0;         // bytes between (t, f) rows of a float block (default 16N; xc_set_in_pitch_f32)
     int opt_f32_kernel = XC_F32_KERNEL_AUTO, f32_kernel_used = 0;
     std::vector<uint32_t> tiles_tc_ext;                  // the same schedule with one more block row (origin shift): tiles_tc is its prefix
     int shift_period = 1, shift_bytes[8] = {0, 0, 0, 0, 0, 0, 0, 0}, shift_tiles[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // what the last call used
@@ -185,7 +186,9 @@ int launch_tc(xc_plan_t* p, const xc::TcParams& tp, cudaStream_t st) {
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = p->opt_pdl ? 2 : 1;
+    // With the timing buffer on, the kernel stamps it in its prologue, i.e. before griddepcontrol.wait: under programmatic
+    // serialization that could run ahead of a preceding kernel that presets the buffer.  Timed launches are plain launches.
+    cfg.numAttrs = (p->opt_pdl && !p->stamps) ? 2 : 1;
     XC_CUDA(p, cudaLaunchKernelEx(&cfg, xc::xc_i8_tc_kernel<UMMA_N, CG, BK, TS>, p->tmap, tp));
     p->last_launches += 1;
     return XC_OK;
@@ -576,11 +579,12 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
 // fp32 samples on the tensor cores (xc_f32_tc.cuh): tensor map over the dense float block, persistent CTA pairs.
 int correlate_f32_tc(xc_plan_t* p, const float* in_dev, float* vis_dev, int accumulate, cudaStream_t st, int f0 = 0, int nf = -1) {
     if (nf < 0) nf = p->F;
-    in_dev += static_cast<size_t>(4) * p->N * f0;          // channels [f0, f0 + nf): the map starts at row f0, channel pitch stays F
+    const size_t pitch = p->in_pitch_f32;                  // bytes between rows (16N unless xc_set_in_pitch_f32 was called)
+    in_dev = reinterpret_cast<const float*>(reinterpret_cast<const char*>(in_dev) + pitch * static_cast<size_t>(f0));   // channels [f0, f0 + nf): the map starts at row f0, channel pitch stays F
     vis_dev += static_cast<size_t>(f0) * p->NB * 8;
-    if (p->tmap_f32_src != in_dev || p->tmap_f32_nf != nf) {
+    if (p->tmap_f32_src != in_dev || p->tmap_f32_nf != nf || p->tmap_f32_pitch != pitch) {
         const cuuint64_t gdim[3] = {static_cast<cuuint64_t>(4) * p->N, static_cast<cuuint64_t>(nf), static_cast<cuuint64_t>(p->T)};
-        const cuuint64_t gstride[2] = {static_cast<cuuint64_t>(16) * p->N, static_cast<cuuint64_t>(16) * p->N * p->F};
+        const cuuint64_t gstride[2] = {static_cast<cuuint64_t>(pitch), static_cast<cuuint64_t>(pitch) * static_cast<cuuint64_t>(p->F)};
         const cuuint32_t box[3] = {32, 1, static_cast<cuuint32_t>(xc::FT_BK)};
         const cuuint32_t estr[3] = {1, 1, 1};
         CUresult r = p->encode(&p->tmap_f32, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(in_dev), gdim, gstride, box, estr,
@@ -595,6 +599,7 @@ int correlate_f32_tc(xc_plan_t* p, const float* in_dev, float* vis_dev, int accu
         }
         p->tmap_f32_src = in_dev;
         p->tmap_f32_nf = nf;
+        p->tmap_f32_pitch = pitch;
     }
     xc::F32TcParams tp;
     memset(&tp, 0, sizeof tp);
@@ -628,7 +633,7 @@ int correlate_f32_tc(xc_plan_t* p, const float* in_dev, float* vis_dev, int accu
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = p->opt_pdl ? 2 : 1;
+    cfg.numAttrs = (p->opt_pdl && !p->stamps) ? 2 : 1;     // timed launches are plain launches (see launch_tc)
     XC_CUDA(p, cudaLaunchKernelEx(&cfg, xc::xc_f32_tc_kernel, p->tmap_f32, tp));
     p->last_launches = 1;
     return XC_OK;
@@ -659,6 +664,7 @@ int xc_plan(xc_plan_t** out, int N, int P, int F, int T, int layout) {
     // staging workspace, the device scratch of the host-buffer calls, the F-engine's cube -- uses the 128-byte pitch.
     p->in_pitch = static_cast<size_t>(4) * N;
     p->pad_pitch = (static_cast<size_t>(4) * N + 127) & ~static_cast<size_t>(127);
+    p->in_pitch_f32 = static_cast<size_t>(16) * N;
     set_tile_mode(p, XC_TILE_AUTO);
     p->tiles_f32 = build_tiles(N, xc::F32_SI, xc::F32_SJ);
     p->tiles_f32tc = build_tiles(N, 64, 64);
@@ -690,7 +696,17 @@ void xc_destroy(xc_plan_t* p) {
 size_t xc_in_bytes(const xc_plan_t* p) { return p ? p->in_pitch * p->F * p->T : 0; }
 size_t xc_in_pitch(const xc_plan_t* p) { return p ? p->in_pitch : 0; }
 size_t xc_in_bytes_i4(const xc_plan_t* p) { return p ? static_cast<size_t>(2) * p->N * p->F * p->T : 0; }
-size_t xc_in_bytes_f32(const xc_plan_t* p) { return p ? static_cast<size_t>(16) * p->N * p->F * p->T : 0; }
+size_t xc_in_bytes_f32(const xc_plan_t* p) { return p ? p->in_pitch_f32 * p->F * p->T : 0; }
+size_t xc_in_pitch_f32(const xc_plan_t* p) { return p ? p->in_pitch_f32 : 0; }
+int xc_set_in_pitch_f32(xc_plan_t* p, size_t row_pitch_bytes) {
+    if (!p) return XC_ERR_INVALID_ARG;
+    const size_t dense = static_cast<size_t>(16) * p->N;
+    if (row_pitch_bytes == 0) row_pitch_bytes = dense;
+    if (row_pitch_bytes < dense || (row_pitch_bytes & 15u)) return XC_ERR_INVALID_ARG;
+    p->in_pitch_f32 = row_pitch_bytes;
+    p->tmap_f32_src = nullptr;
+    return XC_OK;
+}
 size_t xc_vis_bytes(const xc_plan_t* p) { return p ? static_cast<size_t>(32) * p->NB * p->F : 0; }
 size_t xc_n_baselines(const xc_plan_t* p) { return p ? static_cast<size_t>(p->NB) : 0; }
 size_t xc_scratch_pitch(const xc_plan_t* p) { return p ? p->pad_pitch : 0; }
@@ -793,6 +809,7 @@ int xc_correlate_f32(xc_plan_t* p, const float* in_dev, float* vis_dev, int accu
     // Tensor cores (three TF32 MMAs per product, xc_f32_tc.cuh) by default: measured faster at every N (N = 8 .. 256, F T =
     // 131072: 3.3x .. 4.8x); the CUDA-core kernel (xc_f32.cuh, the paper's own register tiling) on request.
     const bool tc = p->opt_f32_kernel != XC_F32_KERNEL_CUDA_CORES;
+    if (!tc && p->in_pitch_f32 != static_cast<size_t>(16) * p->N) return XC_ERR_UNSUPPORTED;   // the CUDA-core kernel reads dense rows
     p->f32_kernel_used = tc ? XC_F32_KERNEL_TC : XC_F32_KERNEL_CUDA_CORES;
     if (tc) return correlate_f32_tc(p, in_dev, vis_dev, accumulate, static_cast<cudaStream_t>(stream));
     xc::F32Params fp;

@@ -339,7 +339,13 @@ xc_f32_tc_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant
                     }
                     fence_proxy_async_smem();          // the tensor core reads these bytes through the async proxy
                     __syncwarp();
+#ifdef XC_FT_RELEASE_CLUSTER
+                    // canary build (-DXC_FT_RELEASE_CLUSTER): the arrive that the PTX memory model formally pairs with the
+                    // leader's cluster-scope acquire; 1.65x slower, run once per round against test_f32_*
+                    if (lane == 0) mbar_arrive_release_cluster(lead_conv0 + 8u * stage);
+#else
                     if (lane == 0) mbar_arrive_remote_release_cta(lead_conv0 + 8u * stage);
+#endif
                     if (++stage == FT_STAGES) {
                         stage = 0;
                         phase ^= 1u;

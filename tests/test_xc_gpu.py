@@ -858,6 +858,73 @@ def test_f32_tc_wide_dynamic_range():
     f32_tolerance_check(got, xo.channels_f64(x), N)
 
 
+@pytest.mark.parametrize("N,F,T", [(100, 3, 130), (37, 2, 64), (500, 2, 96)])
+def test_f32_pitched_rows(N, F, T):
+    """xc_set_in_pitch_f32 (rows aligned to the memory line): the same float samples in rows padded to a
+    multiple of 128 bytes (poisoned padding) give the same bits as the dense block, sub-ranges included, and meet the
+    tolerance against the fp64 oracle; the CUDA-core kernel refuses a pitched plan; pitch 0 restores the dense default."""
+    x = wl.gaussian(N, F, T, seed=300 + N, sigma=20.0).astype(np.float32) * np.float32(0.37)
+    ref = xo.channels_f64(x)
+    p = xcb.Plan(N, F, T)
+    xd = torch.from_numpy(x).cuda()
+    dense = p.correlate_f32(xd).cpu().numpy()
+    f32_tolerance_check(dense.astype(np.float64), ref, N)
+    pitch = (16 * N + 127) // 128 * 128
+    xp = torch.full((T, F, pitch // 4), float("nan"), dtype=torch.float32, device="cuda")
+    xp[:, :, :4 * N] = xd.view(T, F, 4 * N)
+    with pytest.raises(xcb.XcError):
+        p.set_in_pitch_f32(16 * N - 16)
+    with pytest.raises(xcb.XcError):
+        p.set_in_pitch_f32(pitch + 8)
+    p.set_in_pitch_f32(pitch)
+    assert p.in_pitch_f32 == pitch and p.in_bytes_f32 == pitch * F * T
+    vis = torch.full(p.vis_shape(), float("nan"), dtype=torch.float32, device="cuda")
+    p.correlate_f32(xp, vis)
+    assert np.array_equal(vis.cpu().numpy(), dense)
+    vis.fill_(float("nan"))
+    for f0 in range(F):
+        p.correlate_f32_channels(xp, vis, f0, 1)
+    assert np.array_equal(vis.cpu().numpy(), dense)
+    p.set_option(xcb.OPT_F32_KERNEL, xcb.F32_KERNEL_CUDA_CORES)
+    with pytest.raises(xcb.XcError) as e:
+        p.correlate_f32(xp, vis)
+    assert e.value.code == -2
+    p.set_option(xcb.OPT_F32_KERNEL, xcb.F32_KERNEL_AUTO)
+    p.set_in_pitch_f32(0)
+    assert p.in_pitch_f32 == 16 * N
+    assert np.array_equal(p.correlate_f32(xd).cpu().numpy(), dense)
+    p.close()
+
+
+@pytest.mark.parametrize("kern", F32_KERNELS)
+def test_f32_non_finite_sample_stays_inside_its_station(kern):
+    """xc.h's precondition for float samples (finite, |a| < 2^127): one infinite sample and one that rounds to infinity in
+    TF32 (0x7F7FF000 and above) spoil only the visibilities of their own station in their own channel -- non-finite there
+    with either kernel -- while every other baseline still meets the tolerance against the fp64 oracle; a large but
+    admissible sample (1e18: products 1e36) is handled by both kernels."""
+    N, F, T = 40, 2, 64
+    rng = np.random.default_rng(99)
+    x = rng.standard_normal((T, F, N, 2, 2)).astype(np.float32)
+    x[5, 0, 7, 0, 0] = 1e18                                     # admissible
+    ref = xo.channels_f64(x)
+    bad = x.copy()
+    bad[3, 0, 11, 1, 0] = np.inf
+    bad[9, 1, 30, 0, 1] = np.float32(3.4028e38)                 # finite, but rounds to infinity as TF32
+    p = xcb.Plan(N, F, T)
+    p.set_option(xcb.OPT_F32_KERNEL, kern)
+    good = p.correlate_f32(torch.from_numpy(x).cuda()).cpu().numpy().astype(np.float64)
+    f32_tolerance_check(good, ref, N)
+    got = p.correlate_f32(torch.from_numpy(bad).cuda()).cpu().numpy().astype(np.float64)
+    p.close()
+    jj, ii = np.array([(j, i) for j in range(N) for i in range(j + 1)]).T
+    for f, s in [(0, 11), (1, 30)]:
+        touched = (ii == s) | (jj == s)
+        assert not np.isfinite(got[f, s * (s + 1) // 2 + s]).all()               # the station's own autocorrelation is spoilt
+        assert np.isfinite(got[f, ~touched]).all()
+        got[f, touched] = ref[f, touched]                                        # everything else must be as if nothing happened
+    f32_tolerance_check(got, ref, N)
+
+
 @pytest.mark.parametrize("kern", F32_KERNELS)
 def test_f32_gaussian_floats_N256_sampled_channels(kern):
     """Config 3's shape class (N = 256, T = 1000) with genuinely non-integer Gaussian floats: sampled channels (first,
