@@ -174,6 +174,55 @@ def f32_pitch_leg(stream, launches=5):
     return out
 
 
+def two_stream_vs_n(stream, s2, names=("cfg5_N32", "cfg5_N64", "cfg5_N100", "cfg5_N500"), blocks=4):
+    """The paper's Fig. 4 / Fig. 7 analogue over N (kernel time against host-to-device time, "the
+    transfer is hidden for N > ..."; the integrated run): per config of the N sweep, `blocks` pinned host blocks
+    through xc_correlate_pipelined (Algorithm 1) and through xc_integrate (+ int64 widening + D2H of the result), next to the
+    copies alone and the X-engine alone.  compute_over_copy > 1 means PCIe is hidden behind the X-engine."""
+    import torch
+    import paper_1107_4264_b200 as xcb
+    import xc_workloads as wl
+    out = {}
+    for name in names:
+        w = wl.CONFIGS[name]
+        blk = torch.from_numpy(wl.make_input(w))
+        host = torch.empty((blocks,) + tuple(blk.shape), dtype=torch.int8).pin_memory()
+        for k in range(blocks):
+            host[k].copy_(blk)
+        p = xcb.Plan(w.N, w.F, w.T)
+        dev2, v = p.new_scratch(2), p.new_vis()
+        v64 = torch.empty(p.vis_shape(), dtype=torch.int64, device="cuda")
+        v64h = torch.empty(p.vis_shape(), dtype=torch.int64).pin_memory()
+
+        def wall(fn, reps=3):
+            fn()
+            stream.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(reps):
+                fn()
+                stream.synchronize()
+            return (time.perf_counter() - t0) / reps
+        tot = wall(lambda: p.correlate_pipelined(host, dev2, v, stream, s2))
+        tot_i = wall(lambda: p.integrate(host, dev2, v, v64, stream, s2, vis64_host=v64h))
+        dense = dev2[:4 * w.N * w.F * w.T]
+
+        def copies():
+            with torch.cuda.stream(stream):
+                for k in range(blocks):
+                    dense.copy_(host[k].view(-1), non_blocking=True)
+        t_copy = wall(copies)
+        xd = torch.from_numpy(wl.make_input(w)).cuda()
+        t_comp = blocks * 1e-3 * _timed(lambda: p.correlate(xd, v, stream=stream), stream, 20, warm=3)
+        out[name] = {"N": w.N, "F": w.F, "T": w.T, "blocks": blocks, "two_stream_ms": 1e3 * tot, "integrated_ms": 1e3 * tot_i,
+                     "copy_alone_ms": 1e3 * t_copy, "compute_alone_ms": 1e3 * t_comp, "compute_over_copy": t_comp / t_copy,
+                     "h2d_gbs": blocks * w.in_bytes / tot / 1e9, "tops": blocks * w.ops / tot / 1e12,
+                     "tops_integrated": blocks * w.ops / tot_i / 1e12, "overlap_efficiency": max(t_copy, t_comp) / tot}
+        p.close()
+        del host, dev2, v, v64, v64h, xd, dense
+        torch.cuda.empty_cache()
+    return out
+
+
 def fma_probe(iters=100000):
     """Pure-register FFMA2 / FFMA streams (bench_probe.cu beside this file, built on demand as libbench_probe.so): what the fp32 pipe delivers for the
     kernel's operand pattern with no memory traffic at all -- the practical ceiling next to which the kernel's rate is read."""
@@ -371,6 +420,7 @@ def extras(stream, clocks, sampler, peaks):
     p5.close()
     del host, dev2, v5
     torch.cuda.empty_cache()
+    out["two_stream_vs_N"] = two_stream_vs_n(stream, s2)
 
     # ---- T-split of the single-CTA tile (small N, long integration), off / on / what AUTO picks -----------
     out["t_split"] = t_split_leg(stream)

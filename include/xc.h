@@ -279,9 +279,11 @@ int xc_integrate(xc_plan_t* plan, const int8_t* in_host_pinned, int n_blocks, in
  *   independently for every frequency"; the paper's multi-GPU plan hands different channels to
  *   different devices).  in_dev / vis_dev are the FULL block and cube of the plan (the range is
  *   addressed inside them with the plan's F as channel pitch); only vis[f0 .. f0+nf) is written.  accumulate != 0
- *   adds.  Ranges of one block may run concurrently on different streams.  Errors: INVALID_ARG for a range outside
- *   [0, F); UNSUPPORTED when the input needs the staging pass (N % 4 != 0, misaligned pointer) or
- *   the SIMT kernel is selected -- those work on whole blocks only. */
+ *   adds.  Ranges of one block may run concurrently on different streams.  A block that needs the staging pass (N % 4
+ *   != 0, misaligned pointer) is staged range by range: each call copies its own channels' rows into their place in the
+ *   plan-wide workspace (calls on different streams are ordered against each other by the workspace event, so such ranges
+ *   do not overlap on the GPU).  Errors: INVALID_ARG for a range outside [0, F); UNSUPPORTED with the SIMT kernel selected
+ *   (whole blocks only). */
 int xc_correlate_channels(xc_plan_t* plan, const int8_t* in_dev, int32_t* vis_dev, int f0, int nf, int accumulate,
                           void* cuda_stream);
 
@@ -321,6 +323,19 @@ int xc_correlate_host_i4(xc_plan_t* plan, const uint8_t* in4_host, int32_t* vis_
  * xc_fx -- the FX correlator: xc_fengine into cube_scratch_dev (xc_cube_bytes(), 16-byte aligned, pitch
  *   xc_scratch_pitch()), then the X-engine on it: vis (+)= sum_t X X^H.  Two launches on the caller's stream; the
  *   X-engine's prologue overlaps the F-engine's tail (programmatic dependent launch). */
+/* xc_fengine_channels / xc_fx_channels -- the F-engine and the FX chain for ONE channel range [f0, f0 + nf) of the plan's F
+ *   ("evaluated independently for every frequency"; one channel range per GPU, PAPER.md:285 -- every GPU
+ *   receives the station time series, and keeps only its own channels of the corner turn).  The transforms
+ *   are the full F-point ones (same arithmetic, hence the same quantised samples as xc_fengine), but only the range's
+ *   channels are stored: cube_dev / cube_scratch_dev is a PRUNED cube, rows (t, f - f0), nf rows per time block,
+ *   xc_scratch_pitch() (or cube_pitch) bytes apart -- xc_scratch_pitch() * nf * T bytes instead of xc_cube_bytes().
+ *   xc_fx_channels then runs the X-engine on that cube and writes (accumulate: adds to) vis[f0 .. f0 + nf) of the FULL
+ *   visibility cube vis_dev, like xc_correlate_channels.  Errors as xc_fengine / xc_fx; INVALID_ARG for a range outside
+ *   [0, F); UNSUPPORTED with the SIMT kernel or XC_OPT_FORCE_STAGE selected. */
+int xc_fengine_channels(xc_plan_t* plan, const int8_t* volt_dev, float scale, int8_t* cube_dev, size_t cube_pitch, int f0, int nf,
+                        void* cuda_stream);
+int xc_fx_channels(xc_plan_t* plan, const int8_t* volt_dev, float scale, int8_t* cube_scratch_dev, int32_t* vis_dev, int f0, int nf,
+                   int accumulate, void* cuda_stream);
 size_t xc_volt_bytes(const xc_plan_t* plan);   /* 4*N*F*T */
 size_t xc_cube_bytes(const xc_plan_t* plan);   /* xc_scratch_pitch()*F*T */
 int xc_fengine(xc_plan_t* plan, const int8_t* volt_dev, float scale, int8_t* cube_dev, size_t cube_pitch, void* cuda_stream);

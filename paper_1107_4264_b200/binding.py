@@ -30,7 +30,7 @@ EXPORTED_SYMBOLS = (
     "xc_correlate_f32", "xc_correlate_pipelined", "xc_correlate_host", "xc_correlate_channels", "xc_integrate",
     "xc_correlate_i4", "xc_correlate_i4_noalloc", "xc_in_bytes_i4", "xc_correlate_host_i4", "xc_tile_count", "xc_tile_get", "xc_t_split", "xc_origin_shift", "xc_origin_shift_plan", "xc_f32_kernel_used", "xc_correlate_f32_channels",
     "xc_set_in_pitch", "xc_in_pitch", "xc_set_in_pitch_f32", "xc_in_pitch_f32", "xc_scratch_pitch", "xc_scratch_in_bytes", "xc_set_timing_buffer",
-    "xc_volt_bytes", "xc_cube_bytes", "xc_fengine", "xc_fengine_f32", "xc_fx",
+    "xc_volt_bytes", "xc_cube_bytes", "xc_fengine", "xc_fengine_f32", "xc_fx", "xc_fengine_channels", "xc_fx_channels",
     "xc_tri_index", "xc_tri_inverse", "xc_last_launches", "xc_status_string", "xc_last_cuda_error", "xc_version",
 )
 # additionally exported by the profiling build only (libxc_profile.so, -DXC_PROFILE)
@@ -85,6 +85,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
         "xc_fengine": (i, [p, p, ctypes.c_float, p, sz, p]),
         "xc_fengine_f32": (i, [p, p, p, p]),
         "xc_fx": (i, [p, p, ctypes.c_float, p, p, i, p]),
+        "xc_fengine_channels": (i, [p, p, ctypes.c_float, p, sz, i, i, p]),
+        "xc_fx_channels": (i, [p, p, ctypes.c_float, p, p, i, i, i, p]),
         "xc_tile_count": (i, [p]),
         "xc_f32_kernel_used": (i, [p]),
         "xc_origin_shift": (i, [p, ctypes.POINTER(i), ctypes.POINTER(i)]),
@@ -482,6 +484,36 @@ class Plan:
         self._check(lib().xc_fx(self._h, ctypes.c_void_p(volt.data_ptr()), ctypes.c_float(scale),
                                 ctypes.c_void_p(cube_scratch.data_ptr()), ctypes.c_void_p(vis.data_ptr()),
                                 1 if accumulate else 0, _stream_handle(stream)), "xc_fx")
+        return vis
+
+    def new_cube_range(self, nf: int, device="cuda"):
+        """int8 [T][nf][scratch_pitch]: the pruned cube of a channel range (fengine_channels / fx_channels)."""
+        import torch
+        return torch.empty((self.T, nf, self.scratch_pitch), dtype=torch.int8, device=device)
+
+    def fengine_channels(self, volt, scale: float, f0: int, nf: int, cube=None, stream=None):
+        """Pruned cube [T][nf][pitch] holding channels [f0, f0 + nf) of quantise(FFT_F(volt) * scale)."""
+        self._chk_volt(volt)
+        if cube is None:
+            cube = self.new_cube_range(nf, volt.device)
+        if not (cube.is_cuda and cube.is_contiguous() and cube.dim() == 3 and tuple(cube.shape[:2]) == (self.T, nf)
+                and cube.element_size() == 1):
+            raise ValueError("cube must be a contiguous CUDA int8 tensor [T][nf][pitch]")
+        self._check(lib().xc_fengine_channels(self._h, ctypes.c_void_p(volt.data_ptr()), ctypes.c_float(scale),
+                                              ctypes.c_void_p(cube.data_ptr()), int(cube.shape[2]), f0, nf, _stream_handle(stream)),
+                    "xc_fengine_channels")
+        return cube
+
+    def fx_channels(self, volt, scale: float, cube_scratch, vis, f0: int, nf: int, accumulate=False, stream=None):
+        """vis[f0:f0+nf] (+)= X-engine(F-engine(volt)[channels f0 .. f0+nf)).  cube_scratch: new_cube_range(nf); vis: the full cube."""
+        import torch
+        self._chk_volt(volt)
+        if tuple(cube_scratch.shape) != (self.T, nf, self.scratch_pitch) or not cube_scratch.is_contiguous():
+            raise ValueError("cube_scratch must be new_cube_range(nf)")
+        self._chk_vis(vis, torch.int32)
+        self._check(lib().xc_fx_channels(self._h, ctypes.c_void_p(volt.data_ptr()), ctypes.c_float(scale),
+                                         ctypes.c_void_p(cube_scratch.data_ptr()), ctypes.c_void_p(vis.data_ptr()), f0, nf,
+                                         1 if accumulate else 0, _stream_handle(stream)), "xc_fx_channels")
         return vis
 
     def correlate_host_i4(self, x4_host, vis_host, in4_dev, vis_dev, stream=None):

@@ -83,7 +83,7 @@ struct xc_plan_s {
     CUtensorMap tmap;
     const void* tmap_src = nullptr;
     size_t tmap_pitch = 0;
-    int tmap_bk = 0, tmap_nf = 0;
+    int tmap_bk = 0, tmap_nf = 0, tmap_fchan = 0;
     cudaStream_t s_h2d = nullptr, s_d2h = nullptr;       // xc_correlate_host: plan-owned copy streams
     std::vector<cudaEvent_t> ev_chunk;                   // xc_correlate_host: per-chunk events
     cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr}, ev_entry = nullptr;
@@ -277,8 +277,11 @@ int fe_prepare(xc_plan_t* p) {
 int ensure_device(xc_plan_t* p);
 
 // volt -> cube (quantised, rows `pitch` bytes apart) and / or spec (fp32, dense cube order)
-int fengine_launch(xc_plan_t* p, const int8_t* volt, float scale, int8_t* cube, size_t pitch, float* spec, cudaStream_t st) {
+int fengine_launch(xc_plan_t* p, const int8_t* volt, float scale, int8_t* cube, size_t pitch, float* spec, cudaStream_t st,
+                   int f0 = 0, int nf = -1) {
     if (!p || !volt || (!cube && !spec)) return XC_ERR_INVALID_ARG;
+    if (nf < 0) nf = p->F;
+    if (f0 < 0 || nf < 1 || f0 + nf > p->F) return XC_ERR_INVALID_ARG;
     int rc = ensure_device(p);
     if (rc != XC_OK) return rc;
     if (p->logf < 0) {
@@ -301,6 +304,8 @@ int fengine_launch(xc_plan_t* p, const int8_t* volt, float scale, int8_t* cube, 
     fp.TT = static_cast<int>(TT);
     fp.nsb = (p->N + SB - 1) / SB;
     fp.pitch = static_cast<long long>(pitch);
+    fp.f0 = f0;
+    fp.nf = nf;
     fp.volt = volt;
     fp.cube = cube;
     fp.spec = spec;
@@ -417,6 +422,10 @@ int stage_if_needed(xc_plan_t* p, const int8_t* in_dev, cudaStream_t st, const v
             xc::xc_unpack_i4_kernel<<<grid(units), 256, 0, st>>>(
                 reinterpret_cast<const uint8_t*>(in_dev), static_cast<uint32_t*>(p->ws), p->T, p->F, f0, nf, p->N, npad);
         }
+    } else if (f0 != 0 || nf != p->F) {
+        // a channel range of a block that needs staging: only the range's rows are copied (they keep their workspace rows)
+        xc::xc_stage_pad_range_kernel<<<grid(static_cast<long long>(p->T) * nf * npad), 256, 0, st>>>(
+            in_dev, static_cast<uint32_t*>(p->ws), p->T, p->F, f0, nf, p->N, static_cast<long long>(p->in_pitch), npad);
     } else if (p->N % 4 == 0 && p->in_pitch % 16 == 0 && !(reinterpret_cast<uintptr_t>(in_dev) & 15u)) {
         xc::xc_stage_pad16_kernel<<<grid(rows * (npad / 4)), 256, 0, st>>>(
             reinterpret_cast<const uint4*>(in_dev), static_cast<uint4*>(p->ws), rows, p->N / 4,
@@ -434,11 +443,11 @@ int stage_if_needed(xc_plan_t* p, const int8_t* in_dev, cudaStream_t st, const v
 
 // Tensor map over channels [.., nf) of the block that starts at src: rows of 4N valid bytes, `pitch` bytes apart (the
 // channel pitch stays the plan's F).  Bytes beyond 4N of a row, stations beyond N and samples beyond T read as zero.
-int encode_tmap(xc_plan_t* p, const void* src, size_t pitch, int bk, int nf) {
-    if (p->tmap_src == src && p->tmap_pitch == pitch && p->tmap_bk == bk && p->tmap_nf == nf) return XC_OK;
+int encode_tmap(xc_plan_t* p, const void* src, size_t pitch, int bk, int nf, int fchan) {
+    if (p->tmap_src == src && p->tmap_pitch == pitch && p->tmap_bk == bk && p->tmap_nf == nf && p->tmap_fchan == fchan) return XC_OK;
     const cuuint64_t gdim[3] = {static_cast<cuuint64_t>(4) * p->N, static_cast<cuuint64_t>(nf),
                                 static_cast<cuuint64_t>(p->T)};
-    const cuuint64_t gstride[2] = {static_cast<cuuint64_t>(pitch), static_cast<cuuint64_t>(pitch) * static_cast<cuuint64_t>(p->F)};
+    const cuuint64_t gstride[2] = {static_cast<cuuint64_t>(pitch), static_cast<cuuint64_t>(pitch) * static_cast<cuuint64_t>(fchan)};
     const cuuint32_t box[3] = {128, 1, static_cast<cuuint32_t>(bk)};
     const cuuint32_t estr[3] = {1, 1, 1};
     CUresult r = p->encode(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(src), gdim, gstride, box, estr,
@@ -455,6 +464,7 @@ int encode_tmap(xc_plan_t* p, const void* src, size_t pitch, int bk, int nf) {
     p->tmap_pitch = pitch;
     p->tmap_bk = bk;
     p->tmap_nf = nf;
+    p->tmap_fchan = fchan;
     return XC_OK;
 }
 
@@ -505,8 +515,9 @@ long long plan_origin_shift(xc_plan_t* p, xc::TcParams* tp, const void* base, si
 
 // X-engine on channels [f0, f0 + nf) of the block at in_dev / the cube at vis_dev (both addressed with the plan's F).
 // pitch_override != 0: in_dev is a device block with that row pitch (the host paths' re-pitched scratch, the F-engine's cube).
+// range_only: in_dev holds ONLY the range's channels, nf rows per time sample (the F-engine's pruned cube, xc_fx_channels).
 int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* stream, int accumulate, int f0 = 0,
-                 int nf = -1, int fmt_i4 = 0, size_t pitch_override = 0) {
+                 int nf = -1, int fmt_i4 = 0, size_t pitch_override = 0, bool range_only = false) {
     if (!p || !in_dev || !vis_dev) return XC_ERR_INVALID_ARG;
     if (nf < 0) nf = p->F;
     if (f0 < 0 || nf < 1 || f0 + nf > p->F) return XC_ERR_INVALID_ARG;
@@ -521,9 +532,9 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     struct Restore { xc_plan_t* p; size_t v; ~Restore() { p->in_pitch = v; } } restore{p, pitch_saved};
     if (pitch_override) p->in_pitch = pitch_override;
 
-    // a channel sub-range is read in place through its own tensor map: not with the SIMT kernel, not through staging
-    const bool need_stage = needs_staging(p, in_dev, fmt_i4);
-    if (sub && (p->opt_kernel == XC_I8_KERNEL_SIMT || (need_stage && !fmt_i4))) return XC_ERR_UNSUPPORTED;
+    // a channel sub-range is read through its own tensor map (in place, or from its rows of the staging workspace): not
+    // with the SIMT kernel
+    if (sub && p->opt_kernel == XC_I8_KERNEL_SIMT) return XC_ERR_UNSUPPORTED;
     if (fmt_i4 && p->opt_kernel == XC_I8_KERNEL_SIMT) return XC_ERR_UNSUPPORTED;
     if (p->opt_kernel == XC_I8_KERNEL_SIMT) {
         if (p->F > 65535) return XC_ERR_UNSUPPORTED;
@@ -542,7 +553,9 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     if (rc != XC_OK) return rc;
     const bool staged_in = (src != in_dev);
     const bool pair = (p->tile_mode == XC_TILE_2CTA_256x256);
-    rc = encode_tmap(p, static_cast<const int8_t*>(src) + pitch * static_cast<size_t>(f0), pitch, pair ? 128 : 256, nf);
+    if (range_only && staged_in) return XC_ERR_UNSUPPORTED;       // a pruned cube is read in place (the library laid it out itself)
+    const int8_t* base = static_cast<const int8_t*>(src) + (range_only ? 0 : pitch * static_cast<size_t>(f0));
+    rc = encode_tmap(p, base, pitch, pair ? 128 : 256, nf, range_only ? nf : p->F);
     if (rc != XC_OK) return rc;
 
     rc = upload_tiles(p);
@@ -560,7 +573,7 @@ int correlate_i8(xc_plan_t* p, const int8_t* in_dev, int32_t* vis_dev, void* str
     tp.debug_skip = p->opt_debug_skip;
     tp.trace = p->trace;
 #endif
-    const long long total = plan_origin_shift(p, &tp, static_cast<const int8_t*>(src) + pitch * static_cast<size_t>(f0), pitch, nf);
+    const long long total = plan_origin_shift(p, &tp, base, pitch, nf);
     tp.tiles = p->d_tiles_tc;
     if (tp.tiles_per_f <= xc::TC_INLINE_TILES)
         for (int k = 0; k < tp.tiles_per_f; ++k) tp.tiles_inline[k] = p->tiles_tc_ext[k];
@@ -1070,6 +1083,25 @@ int xc_fx(xc_plan_t* p, const int8_t* volt_dev, float scale, int8_t* cube_scratc
     int rc = fengine_launch(p, volt_dev, scale, cube_scratch_dev, p->pad_pitch, nullptr, static_cast<cudaStream_t>(stream));
     if (rc != XC_OK) return rc;
     rc = correlate_i8(p, cube_scratch_dev, vis_dev, stream, accumulate ? 1 : 0, 0, -1, 0, p->pad_pitch);
+    if (rc == XC_OK) p->last_launches += 1;
+    return rc;
+}
+
+int xc_fengine_channels(xc_plan_t* p, const int8_t* volt_dev, float scale, int8_t* cube_dev, size_t cube_pitch, int f0, int nf,
+                        void* stream) {
+    if (!p || !cube_dev) return XC_ERR_INVALID_ARG;
+    return fengine_launch(p, volt_dev, scale, cube_dev, cube_pitch ? cube_pitch : p->pad_pitch, nullptr,
+                          static_cast<cudaStream_t>(stream), f0, nf);
+}
+
+int xc_fx_channels(xc_plan_t* p, const int8_t* volt_dev, float scale, int8_t* cube_scratch_dev, int32_t* vis_dev, int f0, int nf,
+                   int accumulate, void* stream) {
+    if (!p || !cube_scratch_dev || !vis_dev) return XC_ERR_INVALID_ARG;
+    if (reinterpret_cast<uintptr_t>(cube_scratch_dev) & 15u) return XC_ERR_ALIGNMENT;
+    if (p->opt_kernel == XC_I8_KERNEL_SIMT || p->opt_force_stage) return XC_ERR_UNSUPPORTED;
+    int rc = fengine_launch(p, volt_dev, scale, cube_scratch_dev, p->pad_pitch, nullptr, static_cast<cudaStream_t>(stream), f0, nf);
+    if (rc != XC_OK) return rc;
+    rc = correlate_i8(p, cube_scratch_dev, vis_dev, stream, accumulate ? 1 : 0, f0, nf, 0, p->pad_pitch, true);
     if (rc == XC_OK) p->last_launches += 1;
     return rc;
 }

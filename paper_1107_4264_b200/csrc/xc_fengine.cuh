@@ -46,6 +46,7 @@ struct FeParams {
     int SB, TT;               // stations / time blocks per CTA
     int nsb;                  // CTAs along the station axis
     long long pitch;          // bytes between (t, f) rows of the cube
+    int f0, nf;               // channels [f0, f0 + nf) are stored, as rows (t * nf + f - f0) of the cube (whole spectrum: 0, F)
     const int8_t* volt;       // [N][2][T*F][2]
     int8_t* cube;             // quantised output (or null)
     float* spec;              // unquantised fp32 spectra [T][F][N][2][2] (or null); testing aid, strided stores
@@ -443,9 +444,10 @@ __global__ void __launch_bounds__(FE_THREADS) xc_fengine_kernel(const FeParams p
     for (uint32_t rho = (warp << lm) + (lane >> lw); rho < nrows; rho += (FE_THREADS / 32) << lm) {
         const uint32_t tt = rho >> LOGF, f = rho & (F - 1);
         const int t = t0 + static_cast<int>(tt);
-        if (t < p.T && s < p.N) {
+        const uint32_t fr = f - static_cast<uint32_t>(p.f0);      // row inside the stored channel range (unsigned: f < f0 wraps)
+        if (t < p.T && s < p.N && fr < static_cast<uint32_t>(p.nf)) {
             const uint32_t w = static_cast<uint32_t>(c0[rho]) | (static_cast<uint32_t>(c1[rho]) << 16);
-            int8_t* row = p.cube + (static_cast<long long>(t) * F + f) * p.pitch;
+            int8_t* row = p.cube + (static_cast<long long>(t) * p.nf + fr) * p.pitch;
             __stcs(reinterpret_cast<uint32_t*>(row) + s, w);
         }
     }

@@ -83,6 +83,29 @@ __global__ void xc_stage_pad_kernel(const int8_t* __restrict__ in, uint32_t* __r
     }
 }
 
+// The same for channels [f0, f0 + nf) of every time sample only (rows r = t * F + f keep their place in the workspace), so
+// that a block which needs staging can still be correlated range by range (xc_correlate_channels: one range per stream
+// or per GPU); disjoint ranges write disjoint workspace rows.
+__global__ void xc_stage_pad_range_kernel(const int8_t* __restrict__ in, uint32_t* __restrict__ out, int T, int F, int f0, int nf,
+                                          int N, long long pitch, int Npad) {
+    const long long per_t = static_cast<long long>(nf) * Npad;
+    const long long total = per_t * T;
+    for (long long k = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; k < total;
+         k += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long t = k / per_t;
+        const long long rem = k - t * per_t;
+        const long long r = t * F + f0 + rem / Npad;
+        const int s = static_cast<int>(rem % Npad);
+        uint32_t v = 0;
+        if (s < N) {
+            const uint8_t* src = reinterpret_cast<const uint8_t*>(in) + r * pitch + s * 4;
+            v = static_cast<uint32_t>(src[0]) | (static_cast<uint32_t>(src[1]) << 8) |
+                (static_cast<uint32_t>(src[2]) << 16) | (static_cast<uint32_t>(src[3]) << 24);
+        }
+        out[r * Npad + s] = v;
+    }
+}
+
 // Same, 16 bytes (4 stations) per thread, for N % 4 == 0, a 16-byte aligned input and a 16-byte-multiple pitch: only
 // reached with XC_OPT_FORCE_STAGE (a re-pitching copy into the workspace, for testing S0 on aligned shapes).
 __global__ void xc_stage_pad16_kernel(const uint4* __restrict__ in, uint4* __restrict__ out, long long rows, int n4,

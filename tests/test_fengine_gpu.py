@@ -201,6 +201,48 @@ def test_fx_chain_midsize_clean_baselines_bit_exact():
     p.close()
 
 
+@pytest.mark.parametrize("N,F,T", [(9, 16, 20), (40, 64, 12), (130, 256, 5), (33, 1, 7)])
+def test_fengine_and_fx_on_channel_ranges(N, F, T):
+    """xc_fengine_channels / xc_fx_channels (one channel range per GPU): the pruned cube of a range equals
+    those channels of the full cube bit for bit (same transforms, only the stores are pruned; poisoned padding untouched),
+    and the ranges' visibilities, written into the full cube on two streams, equal xc_fx's; accumulate adds to the range only."""
+    volt = wl.voltages(N, F, T, seed=70 + N)
+    scale = wl.fengine_scale(F)
+    p = xcb.Plan(N, F, T)
+    vd = torch.from_numpy(volt).cuda()
+    full_cube = p.fengine(vd, scale)
+    full_vis = p.fx(vd, scale, p.new_cube())
+    torch.cuda.synchronize()
+    cuts = sorted({0, F // 3, (2 * F) // 3 + (1 if F > 2 else 0), F})
+    ranges = [(a, b - a) for a, b in zip(cuts[:-1], cuts[1:]) if b > a]
+    poison = 0x5A5A5A5A
+    vis = torch.full(p.vis_shape(), poison, dtype=torch.int32, device="cuda")
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    scratch = []
+    for k, (f0, nf) in enumerate(ranges):
+        cube = torch.full((T, nf, p.scratch_pitch), 0x55, dtype=torch.int8, device="cuda")
+        p.fengine_channels(vd, scale, f0, nf, cube)
+        torch.cuda.synchronize()
+        assert torch.equal(cube[:, :, :4 * N], full_cube[:, f0:f0 + nf, :4 * N])
+        assert bool((cube[:, :, 4 * N:] == 0x55).all())
+        scratch.append(p.new_cube_range(nf))
+        p.fx_channels(vd, scale, scratch[-1], vis, f0, nf, stream=streams[k % 2])
+        assert p.last_launches == 2
+    torch.cuda.synchronize()
+    assert torch.equal(vis, full_vis)
+    f0, nf = ranges[-1]
+    p.fx_channels(vd, scale, scratch[-1], vis, f0, nf, accumulate=True)
+    torch.cuda.synchronize()
+    want = full_vis.clone()
+    want[f0:f0 + nf] *= 2
+    assert torch.equal(vis, want)
+    for f0, nf in [(-1, 1), (0, 0), (F, 1), (0, F + 1)]:
+        with pytest.raises(xcb.XcError):
+            p.fengine_channels(vd, scale, f0, nf, torch.empty((T, nf, p.scratch_pitch), dtype=torch.int8, device="cuda"))
+    p.close()
+
+
 def test_fx_chain_config3_shape_sampled():
     """The FX chain at BASELINE.json's config 3 shape class (N = 256, F = 512, T = 64 time blocks): sampled spectra of the
     cube against the oracle (near-tie rule), and xc_fx's visibilities equal to the X-engine run on the very cube the

@@ -553,12 +553,28 @@ def test_correlate_channels_ranges():
     for f0, nf in [(-1, 2), (0, 0), (10, 2), (0, 12)]:
         with pytest.raises(xcb.XcError):
             p.correlate_channels(xd, vis, f0, nf)
-    # a block that needs the staging pass works on whole blocks only
-    p2 = xcb.Plan(5, 4, 8)
-    x2 = torch.zeros(p2.in_shape(), dtype=torch.int8, device="cuda")
+    # a block that needs the staging pass (N % 4 != 0) is staged range by range; the SIMT kernel takes whole blocks only
+    N2, F2, T2 = 45, 7, 90
+    x2 = wl.full_range(N2, F2, T2, seed=6)
+    ref2 = xo.correlate_i8(x2)
+    p2 = xcb.Plan(N2, F2, T2)
+    x2d = torch.from_numpy(x2).cuda()
+    vis2 = torch.full(p2.vis_shape(), poison, dtype=torch.int32, device="cuda")
+    p2.correlate_channels(x2d, vis2, 5, 2, stream=s1)
+    p2.correlate_channels(x2d, vis2, 0, 3, stream=s2)
+    torch.cuda.synchronize()
+    assert p2.last_launches == 2                                  # staging + X-engine
+    got2 = vis2.cpu().numpy()
+    assert np.array_equal(got2[0:3], ref2[0:3]) and np.array_equal(got2[5:7], ref2[5:7]) and (got2[3:5] == poison).all()
+    p2.correlate_channels(x2d, vis2, 3, 2)
+    p2.correlate_channels(x2d, vis2, 1, 5, accumulate=True)
+    torch.cuda.synchronize()
+    want2 = ref2.copy()
+    want2[1:6] *= 2
+    assert np.array_equal(vis2.cpu().numpy(), want2)
+    p2.set_option(xcb.OPT_I8_KERNEL, xcb.I8_KERNEL_SIMT)
     with pytest.raises(xcb.XcError):
-        p2.correlate_channels(x2, p2.new_vis(), 1, 2)
-    assert torch.equal(p2.correlate_channels(x2, p2.new_vis(), 0, 4), torch.zeros(p2.vis_shape(), dtype=torch.int32, device="cuda"))
+        p2.correlate_channels(x2d, vis2, 1, 2)
 
 
 # ---------------------------------------------------------------------------------------------
