@@ -372,6 +372,20 @@ def extras(stream, clocks, sampler, peaks):
     p4.close()
     del x4h, x4d, v4, v4h
     torch.cuda.empty_cache()
+    # the no-allocation entry point next to the planned call on a block that fills its fixed 16 MiB scratch (N = 128, F = 32,
+    # T = 1000: 16.4 MB unpacked): same two launches, the scratch is a static device array instead of a cudaMalloc'ed workspace
+    wn = wl.Workload("i4_noalloc", 128, 32, 1000, "uniform", 0.0, 7)
+    xn = torch.from_numpy(wl.packed_i4(wn.N, wn.F, wn.T, seed=7)).cuda()
+    pn = xcb.Plan(wn.N, wn.F, wn.T)
+    vn = pn.new_vis()
+    ms_plan = _timed(lambda: pn.correlate_i4(xn, vn, stream=stream), stream, 50, warm=5)
+    ms_na = _timed(lambda: xcb.correlate_i4_noalloc(xn, vn, stream=stream), stream, 50, warm=5)
+    out["i4_noalloc"] = {"workload": "N=128, F=32, T=1000, 4-bit samples (unpacked block 16.4 MB of the fixed 16.8 MB scratch)",
+                         "xc_correlate_i4_ms": ms_plan, "xc_correlate_i4_noalloc_ms": ms_na,
+                         "tops_noalloc": wn.ops / (ms_na * 1e-3) / 1e12, "scratch_bytes": xcb.NOALLOC_SCRATCH_BYTES}
+    pn.close()
+    del xn, vn
+    torch.cuda.empty_cache()
 
     # ---- S6: two-stream run of config 5: 8 host blocks (the same seeded block 8 times: only the timing matters here;
     # parity of the 8-distinct-block run is tests/test_xc_gpu.py::test_cfg5_two_stream_eight_blocks) -------------------

@@ -59,7 +59,8 @@ typedef enum {
     XC_ERR_OVERFLOW = -3,     /* T > XC_MAX_T: one call could leave int32 (2*128^2*T >= 2^31)  */
     XC_ERR_ALIGNMENT = -4,    /* pointer alignment not met and no staging workspace available  */
     XC_ERR_CUDA = -5,         /* a CUDA call failed; see xc_last_cuda_error                    */
-    XC_ERR_NO_WORKSPACE = -6  /* staging needed but workspace too small                        */
+    XC_ERR_NO_WORKSPACE = -6, /* staging needed but workspace too small                        */
+    XC_ERR_NO_MEMORY = -7     /* host memory for the plan could not be allocated               */
 } xc_status;
 
 typedef enum {
@@ -121,7 +122,7 @@ typedef enum {
  *   (1..XC_MAX_T), layout = XC_LAYOUT_TFSPC.  Builds the triangular tile schedule
  *   (only tiles that intersect i <= j are scheduled) and uploads it to the
  *   current CUDA device (plan-owned, a few KB).  *out receives the plan.
- *   Errors: INVALID_ARG, UNSUPPORTED, OVERFLOW, CUDA. */
+ *   Errors: INVALID_ARG, UNSUPPORTED, OVERFLOW, NO_MEMORY, CUDA. */
 int xc_plan(xc_plan_t** out, int N, int P, int F, int T, int layout);
 
 /* Frees the plan and the device memory it owns (tile table, and a staging workspace only if

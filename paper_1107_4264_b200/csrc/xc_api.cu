@@ -664,7 +664,7 @@ int xc_plan(xc_plan_t** out, int N, int P, int F, int T, int layout) {
     if (T > XC_MAX_T) return XC_ERR_OVERFLOW;
     if (N > 32768) return XC_ERR_UNSUPPORTED;  // tile indices are 16-bit; 4N*F*T must also fit the address space
     xc_plan_t* p = new (std::nothrow) xc_plan_s();
-    if (!p) return XC_ERR_INVALID_ARG;
+    if (!p) return XC_ERR_NO_MEMORY;
     p->N = N;
     p->P = P;
     p->F = F;
@@ -1159,6 +1159,7 @@ const char* xc_status_string(int s) {
         case XC_ERR_ALIGNMENT: return "XC_ERR_ALIGNMENT";
         case XC_ERR_CUDA: return "XC_ERR_CUDA";
         case XC_ERR_NO_WORKSPACE: return "XC_ERR_NO_WORKSPACE";
+        case XC_ERR_NO_MEMORY: return "XC_ERR_NO_MEMORY";
         default: return "XC_ERR_UNKNOWN";
     }
 }

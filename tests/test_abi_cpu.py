@@ -67,7 +67,8 @@ def test_plan_argument_validation():
         assert L.xc_plan(ctypes.byref(h), *args) == code, args
         assert not h.value
     assert L.xc_plan(None, 4, 2, 4, 8, 0) == -1
-    assert L.xc_status_string(-3) == b"XC_ERR_OVERFLOW"
+    assert L.xc_status_string(-3) == b"XC_ERR_OVERFLOW" and L.xc_status_string(-7) == b"XC_ERR_NO_MEMORY"
+    assert L.xc_status_string(-8) == b"XC_ERR_UNKNOWN"
     L.xc_destroy(None)
     # 2 * 128^2 * XC_MAX_T still fits int32, one more sample does not (PAPER.md:96 reading 7)
     assert 2 * 128 * 128 * xcb.MAX_T < 2 ** 31 <= 2 * 128 * 128 * (xcb.MAX_T + 1)
