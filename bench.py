@@ -35,7 +35,8 @@ sys.path.insert(0, ROOT)
 NOMINAL_I8_OVER_BF16 = 2.0          # 4.5 / 2.25 PFLOP/s dense (B200_PROFILING.md nominal table)
 NOMINAL_I8_TOPS = 4500.0            # dense int8 = fp8 nominal (B200_PROFILING.md)
 FALLBACK_HBM_GBS, FALLBACK_BF16_TF = 6650.0, 1590.0
-NCU_CAPTURE_COMMIT = "0f76063 (2026-11-05, profiles/r2_ncu_*.csv; the X-engine kernel source is unchanged since)"
+NCU_CAPTURE_COMMIT = ("headline cfg5_N1024: round 3's build (2026-11-06, profiles/r3_ncu_cfg5_N1024.csv); other configs: 0f76063 "
+                      "(2026-11-05, profiles/r2_ncu_*.csv; the X-engine kernel source is unchanged since)")
 SWEEP = ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5_N32", "cfg5_N64", "cfg5_N100", "cfg5_N500", "cfg5_N1024"]
 SUSTAINED = {"cfg2", "cfg3", "cfg4", "cfg5_N500", "cfg5_N1024"}      # the configs north_star's target speaks about (+ cfg2)
 
@@ -55,7 +56,9 @@ def ncu_profile(workload, kernel="xc_i8_tc_kernel"):
     """Counters of xc_i8_tc_kernel from the tracked ncu export profiles/r2_ncu_<workload>.csv (written by
     `ncu -i <rep> --page raw --csv --print-units base --metrics ...`; the .md beside it names the commands).  Returns
     {} when no capture of this round exists: nothing is hard-coded here."""
-    path = os.path.join(ROOT, "profiles", f"r2_ncu_{workload}.csv")
+    path = os.path.join(ROOT, "profiles", f"r3_ncu_{workload}.csv")       # this round's capture where one was made
+    if not os.path.exists(path):
+        path = os.path.join(ROOT, "profiles", f"r2_ncu_{workload}.csv")   # else round 2's (the kernel source is unchanged)
     if not os.path.exists(path):
         return {}
     with open(path, newline="") as fh:
@@ -360,7 +363,7 @@ def main():
     ap.add_argument("--no-sustained", action="store_true", help="skip the sustained legs")
     ap.add_argument("--sustained-seconds", type=float, default=2.0)
     ap.add_argument("--pitch", type=int, default=0, help="profiling aid: run the workload from a block with this row pitch")
-    ap.add_argument("--only", default="", choices=["", "f32", "f32tc", "fengine", "trace"],
+    ap.add_argument("--only", default="", choices=["", "f32", "f32tc", "fengine", "trace", "noalloc"],
                     help="profiling aid: run only a few launches of that leg (for ncu) and print a short JSON line; trace = pipeline "
                          "timeline of CTA 0 from the -DXC_PROFILE build")
     args = ap.parse_args()

@@ -304,6 +304,15 @@ def only_leg(which, workload, stream):
         return {"only": "f32tc", **f32_leg(stream, None, F=128, launches=3, kernel="tc")}
     if which == "fengine":
         return {"only": "fengine", **fengine_leg(stream, workload, launches=3, with_fx=False)}
+    if which == "noalloc":
+        import torch
+        import paper_1107_4264_b200 as xcb
+        import xc_workloads as wl
+        N, F, T = 128, 32, 1000                             # unpacked block 16.4 MB of the fixed 16.8 MB scratch
+        xn = torch.from_numpy(wl.packed_i4(N, F, T, seed=7)).cuda()
+        vn = torch.empty((F, N * (N + 1) // 2, 2, 2, 2), dtype=torch.int32, device="cuda")
+        ms = _timed(lambda: xcb.correlate_i4_noalloc(xn, vn, stream=stream), stream, 3, warm=3)
+        return {"only": "noalloc", "N": N, "F": F, "T": T, "ms_per_call": ms}
     raise ValueError(which)
 
 

@@ -225,7 +225,8 @@ int xc_correlate_i4(xc_plan_t* plan, const uint8_t* in4_dev, int32_t* vis_dev, i
  *   Sharing: there is one array per device and every call on that device uses it, whatever its shape or stream.  Calls
  *   that may overlap on the GPU (different streams, no event between them) race on it and give garbage; calls on one
  *   stream, or ordered by events, are safe.  The array keeps the previous call's bytes; nothing has to be cleared by the
- *   caller: each call rewrites every byte it later reads (padding included).  Host side: thread-safe. */
+ *   caller: every byte a call's X-engine reads was written by that call's own unpacking pass (row bytes beyond 4N are never
+ *   read: the tensor map ends there).  Host side: thread-safe. */
 #define XC_NOALLOC_SCRATCH_BYTES (16u * 1024u * 1024u)
 #define XC_NOALLOC_MAX_N 576
 int xc_correlate_i4_noalloc(int N, int F, int T, const uint8_t* in4_dev, int32_t* vis_dev, int accumulate, void* cuda_stream);

@@ -45,9 +45,9 @@ __device__ __forceinline__ uint32_t na_unpack_station(uint32_t w) {
 }
 
 // Unpacking pass: in4 [T*F rows][N][2 pol] packed bytes -> ws [T*F rows][Npad stations] of 4 int8, one thread per
-// destination station.  Stations N..Npad of every row are written as zero, so a call overwrites every byte of the rows it
-// uses and nothing of an earlier call (another N, another F) can show through; rows beyond T*F are not touched and not
-// read.
+// destination station.  Stations N..Npad of every row are written as zero (not that anybody reads them: the tensor map over
+// the scratch ends at 4N bytes per row).  Every byte the X-engine reads was written by this call's own unpacking pass, so
+// nothing of an earlier call (another N, another F) can show through; rows beyond T*F are not touched and not read.
 __global__ void xc_noalloc_unpack_i4_kernel(const uint8_t* __restrict__ in4, uint32_t* __restrict__ ws, long long rows, int N,
                                             int Npad) {
     const long long total = rows * Npad;
@@ -61,6 +61,27 @@ __global__ void xc_noalloc_unpack_i4_kernel(const uint8_t* __restrict__ in4, uin
             v = na_unpack_station(static_cast<uint32_t>(src[0]) | (static_cast<uint32_t>(src[1]) << 8));
         }
         ws[k] = v;
+    }
+}
+
+// The same for N % 8 == 0 and a 16-byte aligned input: 16 packed bytes (8 stations) -> 32 int8 per thread (n8 = N / 8 groups
+// per row, workspace rows npad8 * 32 bytes apart).  Bytes of a workspace row beyond 4N are not written here -- and never
+// read: the tensor map over the scratch ends at 4N bytes per row, what lies beyond is hardware zero fill.
+__global__ void xc_noalloc_unpack_i4x8_kernel(const uint4* __restrict__ in4, uint4* __restrict__ ws, long long rows, int n8,
+                                              int npad8) {
+    const long long total = rows * n8;
+    for (long long k = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; k < total;
+         k += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long r = k / n8;
+        const long long c = k - r * n8;
+        const uint4 w = __ldcs(in4 + k);
+        uint4 a, b;
+        a.x = na_unpack_station(w.x & 0xFFFFu); a.y = na_unpack_station(w.x >> 16);
+        a.z = na_unpack_station(w.y & 0xFFFFu); a.w = na_unpack_station(w.y >> 16);
+        b.x = na_unpack_station(w.z & 0xFFFFu); b.y = na_unpack_station(w.z >> 16);
+        b.z = na_unpack_station(w.w & 0xFFFFu); b.w = na_unpack_station(w.w >> 16);
+        ws[2 * (r * npad8 + c)] = a;
+        ws[2 * (r * npad8 + c) + 1] = b;
     }
 }
 
@@ -208,12 +229,17 @@ extern "C" int xc_correlate_i4_noalloc(int N, int F, int T, const uint8_t* in4_d
 
     // 1. unpack the 4-bit block into the scratch (`d->scratch` is the array's device address, see na_setup)
     const int npad = static_cast<int>(pitch / 4);
-    const long long items = static_cast<long long>(rows) * npad;
+    const bool wide = (N % 8 == 0) && !(reinterpret_cast<uintptr_t>(in4_dev) & 15u);
+    const long long items = static_cast<long long>(rows) * (wide ? N / 8 : npad);
     long long blocks = (items + 255) / 256;
     const long long cap = static_cast<long long>(d->sm_count) * 32;
     if (blocks > cap) blocks = cap;
-    xc_noalloc_unpack_i4_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in4_dev, static_cast<uint32_t*>(d->scratch),
-                                                                            static_cast<long long>(rows), N, npad);
+    if (wide)
+        xc_noalloc_unpack_i4x8_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(
+            reinterpret_cast<const uint4*>(in4_dev), static_cast<uint4*>(d->scratch), static_cast<long long>(rows), N / 8, npad / 8);
+    else
+        xc_noalloc_unpack_i4_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in4_dev, static_cast<uint32_t*>(d->scratch),
+                                                                                static_cast<long long>(rows), N, npad);
     if (cudaGetLastError() != cudaSuccess) return XC_ERR_CUDA;
 
     // 2. tensor map over the scratch (host-only encode; bytes beyond 4N of a row, samples beyond T read as zero)
